@@ -1,0 +1,165 @@
+/* osdp.h — C ABI of osdp-b200: operator-split transformer MLP for one NVIDIA B200 (sm_100a).
+ *
+ * Method: OSDP (arxiv 2305.09940).  Operator splitting (§3.3): a huge operator is
+ * partitioned into slices that are "executed sequentially", their memory "released serially", and "all
+ * computation results are summed as the final output".  This library applies it to the transformer MLP
+ * operator  Y = gelu(X W1 + b1) W2 + b2  over k TOKEN slices (reading S1), forward and backward,
+ * so that the tokens x ffn intermediate never exists whole, and evaluates the paper's per-operator cost
+ * model (Eq. 1) to choose k per operator under a memory limit (Algorithm 1).
+ *
+ * Conventions (all calls)
+ *   - Tensors are dense row-major, no padding.  X, Y, dY, dX: [tokens x hidden]; W1: [hidden x ffn];
+ *     W2: [ffn x hidden]; b1: [ffn]; b2: [hidden].  Weights are [in x out].
+ *   - dtype = storage type of X, W1, b1, W2, b2, dY, Y, dX and of the workspace tensors.  Products
+ *     accumulate in fp32.  dW1, dW2, db1, db2 are ALWAYS fp32.
+ *   - "device pointer" = CUDA device memory of the current device, owned by the caller, 16-byte aligned
+ *     (workspace: 256-byte aligned).  The library never allocates, frees or synchronises device memory; it
+ *     only enqueues work on `stream` (a cudaStream_t passed as void*; NULL = the legacy default stream).
+ *     Outputs must not alias inputs or each other.
+ *   - Every call returns an osdp_status; OSDP_OK = 0.  Nothing is printed, nothing aborts.  On any error
+ *     before the first launch the outputs are untouched.
+ *   - Re-entrant for distinct streams/workspaces.
+ */
+#ifndef OSDP_H_
+#define OSDP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+#if defined(__GNUC__)
+#pragma GCC visibility push(default)
+#endif
+
+typedef enum osdp_status {
+  OSDP_OK = 0,
+  OSDP_ERR_NULL = 1,        /* a required pointer is NULL */
+  OSDP_ERR_SHAPE = 2,       /* tokens/hidden/ffn < 1, or hidden/ffn not a multiple of 16 bytes / sizeof(dtype) */
+  OSDP_ERR_K = 3,           /* k < 1 or k > tokens */
+  OSDP_ERR_DTYPE = 4,       /* dtype is not OSDP_F32 / OSDP_BF16 */
+  OSDP_ERR_WORKSPACE = 5,   /* workspace smaller than osdp_split_mlp_workspace_bytes, or not 256 B aligned */
+  OSDP_ERR_ALIGN = 6,       /* a tensor pointer is not 16 B aligned */
+  OSDP_ERR_ARCH = 7,        /* current device is not compute capability 10.x (bf16 path needs tcgen05/TMA) */
+  OSDP_ERR_CUDA = 8,        /* CUDA runtime/driver error; see osdp_last_cuda_error() */
+  OSDP_ERR_INFEASIBLE = 9,  /* planner: no plan fits the memory limit (Algorithm 1 lines 12-14) */
+  OSDP_ERR_ARG = 10,        /* other invalid argument (pass, mode, n, candidate list, ...) */
+  OSDP_ERR_SEARCH_LIMIT = 11 /* planner: node budget exhausted before the search completed */
+} osdp_status;
+
+typedef enum osdp_dtype { OSDP_F32 = 0, OSDP_BF16 = 1 } osdp_dtype;
+typedef enum osdp_pass { OSDP_FWD = 0, OSDP_BWD = 1 } osdp_pass;
+typedef enum osdp_mode { OSDP_DP = 0, OSDP_ZDP = 1 } osdp_mode;
+
+/* One MLP operator and its split count.  k = number of token slices ("slice granularity", PAPER.md:165;
+ * the paper's granularity 0 = "no splitting" is k = 1 here).  Slice s covers rows
+ * [floor(s*tokens/k), floor((s+1)*tokens/k))  (reading S7: ragged slices allowed). */
+typedef struct osdp_mlp_desc {
+  int64_t tokens;   /* T >= 1 */
+  int64_t hidden;   /* h; multiple of 8 (bf16) / 4 (f32) */
+  int64_t ffn;      /* f; multiple of 8 (bf16) / 4 (f32) */
+  int32_t dtype;    /* osdp_dtype */
+  int32_t k;        /* 1 <= k <= tokens */
+} osdp_mlp_desc;
+
+const char* osdp_status_string(int status);   /* static string, never NULL */
+const char* osdp_last_cuda_error(void);       /* text of the last CUDA error seen by the calling thread ("" if none) */
+const char* osdp_version(void);
+
+/* ---- A10: workspace accounting (PAPER.md:84-86 M_extra; PAPER.md:167 size/slice_granularity) ----------
+ * Bytes of caller workspace one forward (OSDP_FWD) or backward (OSDP_BWD) call needs.  Pure host function.
+ *   FWD: one [T_s x f] tensor (H_s);  BWD: two (Z_s, overwritten by dZ_s; H_s) + fixed fp32 column-sum scratch;
+ *   T_s = ceil(T/k); each tensor rounded up to 256 B.  Returns 0 on an invalid descriptor. */
+size_t osdp_split_mlp_workspace_bytes(const osdp_mlp_desc* desc, int pass);
+
+/* ---- A0-A2: forward (DESIGN.md steps A1, A2) ---------------------------------------------
+ * for s in 0..k-1 (in order):  H_s = gelu(X_s W1 + b1)  (workspace, storage dtype; Z never stored)
+ *                               Y_s = H_s W2 + b2        (rows of Y, storage dtype)
+ * gelu = tanh approximation (reading S2).  All tensor arguments are device pointers; Y [T x h] is overwritten. */
+int osdp_split_mlp_forward(const osdp_mlp_desc* desc,
+                           const void* X, const void* W1, const void* b1, const void* W2, const void* b2,
+                           void* Y, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- A0, A3-A8: backward (DESIGN.md steps A3-A8) -------------------------------------------------------
+ * Takes no saved activations.  for s in 0..k-1 (in order):
+ *   Z_s = X_s W1 + b1, H_s = gelu(Z_s)                       (recomputed, workspace)
+ *   dZ_s = (dY_s W2^T) (.) gelu'(Z_s)                        (overwrites Z_s)
+ *   dW2 (+)= H_s^T dY_s;  dW1 (+)= X_s^T dZ_s                (fp32; "=" on slice 0, "+=" after: "summed")
+ *   db1 (+)= colsum(dZ_s); db2 (+)= colsum(dY_s)             (fp32, fixed reduction order)
+ *   dX_s = dZ_s W1^T                                         (rows of dX, storage dtype)
+ * dX [T x h] storage dtype; dW1 [h x f], db1 [f], dW2 [f x h], db2 [h] fp32; all OVERWRITTEN (reading S11).
+ * b2 is unused and may be NULL (reading S4). */
+int osdp_split_mlp_backward(const osdp_mlp_desc* desc,
+                            const void* X, const void* W1, const void* b1, const void* W2, const void* b2,
+                            const void* dY,
+                            void* dX, float* dW1, float* db1, float* dW2, float* db2,
+                            void* workspace, size_t workspace_bytes, void* stream);
+
+/* Number of kernel launches the last forward/backward call of the calling thread enqueued (for bench.py's
+ * gpu_launches claim). */
+int64_t osdp_last_launch_count(void);
+
+/* ---- A9: cost model and planner (host only) ------------------------------------------------------------
+ * Per-operator record = the paper's "model description" entry: S_i and the three
+ * memory factors, with M_extra divided into a part splitting does not shrink and two sliceable parts
+ * (reading P6: summed over operators as in Eq. 1, or transient = live for one operator at a time because
+ * slices are "released serially"). */
+typedef struct osdp_op_cost {
+  double   S;                /* parameter bytes one collective moves (S_i) */
+  uint64_t model_bytes;      /* M_i^(model): parameters + gradients + optimizer states */
+  uint64_t act_bytes;        /* M_i^(act) per unit batch */
+  uint64_t extra_fixed;      /* M_i^(extra), not sliceable */
+  uint64_t extra_summed;     /* M_i^(extra), sliceable, summed over operators */
+  uint64_t extra_transient;  /* M_i^(extra), sliceable, max over operators */
+  double   gamma;            /* computation seconds per unit batch (gamma_i) */
+  double   delta;            /* seconds per extra slice (reading P2; 0 = the paper's model) */
+} osdp_op_cost;
+
+/* "Device information". */
+typedef struct osdp_device {
+  int32_t  N;                /* parallelism degree >= 1 */
+  double   alpha;            /* network latency, seconds */
+  double   beta;             /* transfer seconds per byte */
+  uint64_t mem_limit_bytes;  /* M_limit */
+} osdp_device;
+
+/* M_i and T_i of one operator (readings P1, P2):
+ *   persist   = model/(N if ZDP else 1, rounded up) + batch*act + extra_fixed + ceil(extra_summed/k)
+ *   transient = ceil(extra_transient/k)
+ *   seconds   = c (N-1)(alpha + S beta/N) + batch*gamma + (k-1) delta,  c = 2 (DP) / 3 (ZDP)
+ * Any output pointer may be NULL. */
+int osdp_cost_eval(const osdp_op_cost* op, int mode, int32_t k, int64_t batch, const osdp_device* dev,
+                   uint64_t* persist_bytes, uint64_t* transient_bytes, double* seconds);
+
+/* Fills an osdp_op_cost for this library's MLP operator as ONE call sees it:
+ * pass = OSDP_FWD / OSDP_BWD.  model_bytes = the caller tensors live during the call (inputs, outputs, fp32
+ * gradients); extra_transient = workspace at k = 1 minus the fixed scratch; extra_fixed = that scratch;
+ * S = (2 h f + f + h) * sizeof(dtype); act_bytes = 0; gamma/delta = 0 (the caller calibrates them). */
+int osdp_mlp_op_cost(const osdp_mlp_desc* desc, int pass, osdp_op_cost* out);
+
+/* Search engine (Algorithm 1 lines 4-11 at a fixed batch; PAPER.md:149 DFS with two prunings).
+ * Decision per operator: mode in {DP, ZDP} x k in k_candidates (ascending, each >= 1).  Minimises
+ * sum_i T_i subject to  sum_i persist_i + max_i transient_i <= mem_limit_bytes.  Plans are traversed
+ * depth-first in lexicographic order of option index (DP before ZDP, k ascending) and the incumbent is
+ * replaced only on a strictly smaller time, so ties resolve to the first plan in that order.
+ * Outputs: k_out[n], mode_out[n], *est_seconds, *est_peak_bytes (NULL allowed for the last two).
+ * Returns OSDP_ERR_INFEASIBLE (outputs untouched) when no plan fits. */
+int osdp_plan(const osdp_op_cost* ops, int32_t n, const osdp_device* dev, int64_t batch,
+              const int32_t* k_candidates, int32_t n_cand,
+              int32_t* k_out, int32_t* mode_out, double* est_seconds, uint64_t* est_peak_bytes);
+
+/* Scheduler (Algorithm 1 in full): batch = 1, 2, 3, ... up to batch_max; stops at the first
+ * batch with no feasible plan; returns the candidate minimising est_seconds / batch (Eq. 1) in *batch_out. */
+int osdp_plan_batch(const osdp_op_cost* ops, int32_t n, const osdp_device* dev, int64_t batch_max,
+                    const int32_t* k_candidates, int32_t n_cand,
+                    int32_t* k_out, int32_t* mode_out, int64_t* batch_out,
+                    double* est_seconds, uint64_t* est_peak_bytes);
+
+#if defined(__GNUC__)
+#pragma GCC visibility pop
+#endif
+#ifdef __cplusplus
+}
+#endif
+#endif /* OSDP_H_ */

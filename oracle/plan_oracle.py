@@ -1,0 +1,154 @@
+"""Oracle for the planner / cost model (``osdp_cost_eval``, ``osdp_plan``).  TEST INFRASTRUCTURE ONLY.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s baseline legs may import this file.
+It shares no code with ``paper_2305_09940_b200/csrc`` and imports nothing from that package.
+
+Follows the paper step by step:
+
+* Memory cost M_i (§3.1):  DP: M_model + b M_act + M_extra;  ZDP: M_model/N + b M_act + M_extra.
+  With operator splitting the split part goes size -> size / slice_granularity, applied to
+  the sliceable part of M_extra (reading P1).  Slices are "released serially", so a
+  transient workspace is live for one operator at a time: reading P6 keeps both accountings,
+      M(p) = sum_i [ model_i/(N or 1) + b act_i + extra_fixed_i + ceil(extra_summed_i / k_i) ]
+             + max_i ceil(extra_transient_i / k_i).
+  k = 1 and extra_transient = 0 give the paper's formula exactly.
+* Time cost T_i:  c_p (N-1)(alpha + S_i beta / N) + b gamma_i,  c_DP = 2, c_ZDP = 3,
+  plus (k-1) delta_i, our per-extra-slice overhead (reading P2; delta = 0 is the paper's model).
+* Search (Algorithm 1 lines 5-11; b fixed, reading P3): traverse every plan, keep the
+  feasible plan with strictly smaller time ("<", line 8).  Options per operator are ordered DP before
+  ZDP and k ascending in the caller's candidate list; plans are traversed in lexicographic order of
+  option indices, so among equal-time optima the first (least split, DP-most) wins (reading P5).
+  Where floating point decides this integer outcome both sides take the decision in the same precision
+  (reading P9): every T_i is rounded once to an integer count of picoseconds, floor(T_i * 1e12 + 0.5),
+  and plan times are exact integer sums of those.
+* Infeasible (Algorithm 1 lines 12-14): returns None.
+* Batch loop (Algorithm 1 lines 3-20, reading f3): b = 1, 2, 3, ...; stop at the first b with no feasible
+  plan; return the candidate minimising T(b)/b (Eq. 1's objective is the per-sample time).
+
+Pins (tests/test_planner.py): closed forms the paper states — ZDP/DP communication ratio 3/2
+(PAPER.md:25,47,94), model-state memory 1/N, N = 1 => modes coincide, sliceable term
+~ 1/k, 0.6e9 params x 4 B = 2.24 GiB, M_limit = inf => all DP / k = 1,
+M_limit below the minimum => infeasible, monotonicity in M_limit.
+"""
+from __future__ import annotations
+
+import dataclasses
+import itertools
+import math
+
+DP, ZDP = 0, 1
+
+
+@dataclasses.dataclass
+class OpCost:
+    S: float = 0.0                 # parameter bytes moved by one collective (S_i)
+    model: int = 0                 # M_i^(model) bytes
+    act: int = 0                   # M_i^(act) bytes per unit batch
+    extra_fixed: int = 0           # M_i^(extra), part that splitting does not shrink
+    extra_summed: int = 0          # M_i^(extra), sliceable, summed over operators (paper's Eq. 1 sum)
+    extra_transient: int = 0       # M_i^(extra), sliceable, live for one operator at a time
+    gamma: float = 0.0             # seconds per unit batch
+    delta: float = 0.0             # seconds per extra slice
+
+
+@dataclasses.dataclass
+class Device:
+    N: int = 1
+    alpha: float = 0.0
+    beta: float = 0.0
+    mem_limit: int = 0
+
+
+def ceil_div(a: int, b: int) -> int:
+    return -(-a // b)
+
+
+def cost_eval(op: OpCost, mode: int, k: int, b: int, dev: Device):
+    """(persistent_bytes, transient_bytes, seconds) of one operator under (mode, k, b)."""
+    model = ceil_div(op.model, dev.N) if mode == ZDP else op.model
+    persist = model + b * op.act + op.extra_fixed + ceil_div(op.extra_summed, k)
+    transient = ceil_div(op.extra_transient, k)
+    c = 3.0 if mode == ZDP else 2.0
+    t = c * (dev.N - 1) * (dev.alpha + op.S * dev.beta / dev.N) + b * op.gamma + (k - 1) * op.delta
+    return persist, transient, t
+
+
+def to_ps(seconds: float) -> int:
+    return int(math.floor(seconds * 1e12 + 0.5))
+
+
+def plan_memory_time(ops, modes, ks, b, dev):
+    """(peak bytes, integer picoseconds) of a whole plan."""
+    tot, tr, t = 0, 0, 0
+    for op, m, k in zip(ops, modes, ks):
+        p, x, ti = cost_eval(op, m, k, b, dev)
+        tot += p
+        tr = max(tr, x)
+        t += to_ps(ti)
+    return tot + tr, t
+
+
+def plan_brute_force(ops, dev: Device, b: int, k_candidates):
+    """Algorithm 1 lines 4-11 for one batch size: full enumeration, strict '<'.
+
+    Returns (modes, ks, picoseconds, peak_bytes) or None when no plan fits.
+    """
+    options = [(m, k) for m in (DP, ZDP) for k in k_candidates]
+    best = None
+    best_t = math.inf
+    for choice in itertools.product(range(len(options)), repeat=len(ops)):
+        modes = [options[c][0] for c in choice]
+        ks = [options[c][1] for c in choice]
+        mem, t = plan_memory_time(ops, modes, ks, b, dev)
+        if mem <= dev.mem_limit and t < best_t:
+            best_t = t
+            best = (modes, ks, t, mem)
+    return best
+
+
+def schedule_brute_force(ops, dev: Device, k_candidates, b_max: int = 1 << 20):
+    """Algorithm 1 in full: returns (modes, ks, picoseconds, peak_bytes, b) minimising time / b, or None."""
+    cands = []
+    b = 1
+    while b <= b_max:
+        r = plan_brute_force(ops, dev, b, k_candidates)
+        if r is None:
+            break
+        cands.append(r + (b,))
+        b += 1
+    if not cands:
+        return None
+    best = None
+    for c in cands:
+        if best is None or c[2] * best[4] < best[2] * c[4]:      # T(b)/b, exact integer comparison
+            best = c
+    return best
+
+
+# ----- factor calculator for the MLP operator of this build ("calculated according to the
+# definition of operators (e.g., types and shapes)"); written from DESIGN.md "Cost model", not from the
+# library source. -------------------------------------------------------------------------------------
+def mlp_workspace_bytes(T: int, h: int, f: int, e: int, k: int, backward: bool) -> int:
+    """Bytes of caller workspace one call needs: per-slice T_s x f buffers (1 fwd: H_s; 2 bwd: Z_s/dZ_s
+    and H_s), each rounded up to 256 B, plus (bwd) the fixed column-sum scratch."""
+    Ts = ceil_div(T, k)
+    buf = ceil_div(Ts * f * e, 256) * 256
+    if not backward:
+        return buf
+    return 2 * buf + mlp_reduce_scratch_bytes(h, f)
+
+
+REDUCE_ROW_CHUNKS = 32
+
+
+def mlp_reduce_scratch_bytes(h: int, f: int) -> int:
+    """fp32 partial column sums for db1/db2: REDUCE_ROW_CHUNKS x max(h, f) floats, 256 B aligned."""
+    return ceil_div(REDUCE_ROW_CHUNKS * max(h, f) * 4, 256) * 256
+
+
+def mlp_persistent_bytes(T: int, h: int, f: int, e: int, backward: bool) -> int:
+    """Caller tensors live during one call: fwd X, Y, W1, W2, b1, b2;
+    bwd X, dY, dX, W1, W2, b1, b2 + fp32 dW1, dW2, db1, db2."""
+    if not backward:
+        return (2 * T * h + 2 * h * f + f + h) * e
+    return (3 * T * h + 2 * h * f + f + h) * e + (2 * h * f + f + h) * 4

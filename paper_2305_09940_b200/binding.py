@@ -1,0 +1,241 @@
+"""Thin ctypes binding of the osdp-b200 C ABI (``include/osdp.h``): same names, argument marshalling only.
+
+Every step of the hot path runs inside ``libosdp_b200.so``; this file allocates nothing on the device except
+what the caller asks for through torch (device memory, streams).  There is NO fallback: if the library is
+missing, importing this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libosdp_b200.so")
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        f"{LIB_PATH} not found: build it with `python -m paper_2305_09940_b200.build` "
+        "(or __graft_entry__.build()).  There is no CPU/PyTorch fallback for the osdp-b200 hot path.")
+
+_lib = C.CDLL(LIB_PATH)
+
+OSDP_OK = 0
+OSDP_ERR_NULL, OSDP_ERR_SHAPE, OSDP_ERR_K, OSDP_ERR_DTYPE, OSDP_ERR_WORKSPACE, OSDP_ERR_ALIGN = 1, 2, 3, 4, 5, 6
+OSDP_ERR_ARCH, OSDP_ERR_CUDA, OSDP_ERR_INFEASIBLE, OSDP_ERR_ARG, OSDP_ERR_SEARCH_LIMIT = 7, 8, 9, 10, 11
+OSDP_F32, OSDP_BF16 = 0, 1
+OSDP_FWD, OSDP_BWD = 0, 1
+OSDP_DP, OSDP_ZDP = 0, 1
+
+EXPORTS = (
+    "osdp_status_string", "osdp_last_cuda_error", "osdp_version", "osdp_split_mlp_workspace_bytes",
+    "osdp_split_mlp_forward", "osdp_split_mlp_backward", "osdp_last_launch_count", "osdp_cost_eval",
+    "osdp_mlp_op_cost", "osdp_plan", "osdp_plan_batch",
+)
+
+
+class osdp_mlp_desc(C.Structure):
+    _fields_ = [("tokens", C.c_int64), ("hidden", C.c_int64), ("ffn", C.c_int64), ("dtype", C.c_int32),
+                ("k", C.c_int32)]
+
+
+class osdp_op_cost(C.Structure):
+    _fields_ = [("S", C.c_double), ("model_bytes", C.c_uint64), ("act_bytes", C.c_uint64),
+                ("extra_fixed", C.c_uint64), ("extra_summed", C.c_uint64), ("extra_transient", C.c_uint64),
+                ("gamma", C.c_double), ("delta", C.c_double)]
+
+
+class osdp_device(C.Structure):
+    _fields_ = [("N", C.c_int32), ("alpha", C.c_double), ("beta", C.c_double), ("mem_limit_bytes", C.c_uint64)]
+
+
+_lib.osdp_status_string.restype = C.c_char_p
+_lib.osdp_status_string.argtypes = [C.c_int]
+_lib.osdp_last_cuda_error.restype = C.c_char_p
+_lib.osdp_version.restype = C.c_char_p
+_lib.osdp_last_launch_count.restype = C.c_int64
+_lib.osdp_split_mlp_workspace_bytes.restype = C.c_size_t
+_lib.osdp_split_mlp_workspace_bytes.argtypes = [C.POINTER(osdp_mlp_desc), C.c_int]
+_lib.osdp_split_mlp_forward.restype = C.c_int
+_lib.osdp_split_mlp_forward.argtypes = [C.POINTER(osdp_mlp_desc)] + [C.c_void_p] * 7 + [C.c_size_t, C.c_void_p]
+_lib.osdp_split_mlp_backward.restype = C.c_int
+_lib.osdp_split_mlp_backward.argtypes = [C.POINTER(osdp_mlp_desc)] + [C.c_void_p] * 12 + [C.c_size_t, C.c_void_p]
+_lib.osdp_cost_eval.restype = C.c_int
+_lib.osdp_cost_eval.argtypes = [C.POINTER(osdp_op_cost), C.c_int, C.c_int32, C.c_int64, C.POINTER(osdp_device),
+                                C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_double)]
+_lib.osdp_mlp_op_cost.restype = C.c_int
+_lib.osdp_mlp_op_cost.argtypes = [C.POINTER(osdp_mlp_desc), C.c_int, C.POINTER(osdp_op_cost)]
+_lib.osdp_plan.restype = C.c_int
+_lib.osdp_plan.argtypes = [C.POINTER(osdp_op_cost), C.c_int32, C.POINTER(osdp_device), C.c_int64,
+                           C.POINTER(C.c_int32), C.c_int32, C.POINTER(C.c_int32), C.POINTER(C.c_int32),
+                           C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
+_lib.osdp_plan_batch.restype = C.c_int
+_lib.osdp_plan_batch.argtypes = [C.POINTER(osdp_op_cost), C.c_int32, C.POINTER(osdp_device), C.c_int64,
+                                 C.POINTER(C.c_int32), C.c_int32, C.POINTER(C.c_int32), C.POINTER(C.c_int32),
+                                 C.POINTER(C.c_int64), C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
+
+
+class OsdpError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = f"{where}: {osdp_status_string(status)} (status {status})"
+        if status == OSDP_ERR_CUDA:
+            msg += f": {osdp_last_cuda_error()}"
+        super().__init__(msg)
+
+
+def osdp_status_string(status: int) -> str:
+    return _lib.osdp_status_string(int(status)).decode()
+
+
+def osdp_last_cuda_error() -> str:
+    return _lib.osdp_last_cuda_error().decode()
+
+
+def osdp_version() -> str:
+    return _lib.osdp_version().decode()
+
+
+def osdp_last_launch_count() -> int:
+    return int(_lib.osdp_last_launch_count())
+
+
+def _dtype_code(dtype: torch.dtype) -> int:
+    if dtype == torch.float32:
+        return OSDP_F32
+    if dtype == torch.bfloat16:
+        return OSDP_BF16
+    return -1
+
+
+def make_desc(tokens: int, hidden: int, ffn: int, dtype, k: int) -> osdp_mlp_desc:
+    code = dtype if isinstance(dtype, int) else _dtype_code(dtype)
+    return osdp_mlp_desc(int(tokens), int(hidden), int(ffn), int(code), int(k))
+
+
+def osdp_split_mlp_workspace_bytes(desc: osdp_mlp_desc, pass_: int) -> int:
+    return int(_lib.osdp_split_mlp_workspace_bytes(C.byref(desc), int(pass_)))
+
+
+def _ptr(t):
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    assert t.is_contiguous(), "osdp tensors are dense row-major"
+    return t.data_ptr()
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def osdp_split_mlp_forward(desc, X, W1, b1, W2, b2, Y, workspace, workspace_bytes=None, stream=None, check=True):
+    """Enqueue the split forward.  Tensors are torch CUDA tensors (or raw device addresses)."""
+    if workspace_bytes is None:
+        workspace_bytes = workspace.numel() * workspace.element_size()
+    st = _lib.osdp_split_mlp_forward(C.byref(desc), _ptr(X), _ptr(W1), _ptr(b1), _ptr(W2), _ptr(b2), _ptr(Y),
+                                     _ptr(workspace), int(workspace_bytes), _stream_ptr(stream))
+    if check and st != OSDP_OK:
+        raise OsdpError(st, "osdp_split_mlp_forward")
+    return st
+
+
+def osdp_split_mlp_backward(desc, X, W1, b1, W2, b2, dY, dX, dW1, db1, dW2, db2, workspace, workspace_bytes=None,
+                            stream=None, check=True):
+    if workspace_bytes is None:
+        workspace_bytes = workspace.numel() * workspace.element_size()
+    st = _lib.osdp_split_mlp_backward(C.byref(desc), _ptr(X), _ptr(W1), _ptr(b1), _ptr(W2), _ptr(b2), _ptr(dY),
+                                      _ptr(dX), _ptr(dW1), _ptr(db1), _ptr(dW2), _ptr(db2), _ptr(workspace),
+                                      int(workspace_bytes), _stream_ptr(stream))
+    if check and st != OSDP_OK:
+        raise OsdpError(st, "osdp_split_mlp_backward")
+    return st
+
+
+# ---------------------------------------------------------------------------------------------- planner
+def osdp_cost_eval(op: osdp_op_cost, mode: int, k: int, batch: int, dev: osdp_device):
+    p, t, s = C.c_uint64(), C.c_uint64(), C.c_double()
+    st = _lib.osdp_cost_eval(C.byref(op), mode, k, batch, C.byref(dev), C.byref(p), C.byref(t), C.byref(s))
+    if st != OSDP_OK:
+        raise OsdpError(st, "osdp_cost_eval")
+    return int(p.value), int(t.value), float(s.value)
+
+
+def osdp_mlp_op_cost(desc: osdp_mlp_desc, pass_: int) -> osdp_op_cost:
+    out = osdp_op_cost()
+    st = _lib.osdp_mlp_op_cost(C.byref(desc), pass_, C.byref(out))
+    if st != OSDP_OK:
+        raise OsdpError(st, "osdp_mlp_op_cost")
+    return out
+
+
+def _op_array(ops):
+    arr = (osdp_op_cost * len(ops))()
+    for i, o in enumerate(ops):
+        arr[i] = o
+    return arr
+
+
+def osdp_plan(ops, dev: osdp_device, batch: int, k_candidates, check=True):
+    """Returns (status, ks, modes, est_seconds, est_peak_bytes)."""
+    n = len(ops)
+    cand = (C.c_int32 * len(k_candidates))(*k_candidates)
+    ks, modes = (C.c_int32 * n)(), (C.c_int32 * n)()
+    sec, peak = C.c_double(), C.c_uint64()
+    st = _lib.osdp_plan(_op_array(ops), n, C.byref(dev), batch, cand, len(k_candidates), ks, modes, C.byref(sec),
+                        C.byref(peak))
+    if check and st not in (OSDP_OK, OSDP_ERR_INFEASIBLE):
+        raise OsdpError(st, "osdp_plan")
+    if st != OSDP_OK:
+        return st, None, None, None, None
+    return st, list(ks), list(modes), float(sec.value), int(peak.value)
+
+
+def osdp_plan_batch(ops, dev: osdp_device, batch_max: int, k_candidates, check=True):
+    """Returns (status, ks, modes, batch, est_seconds, est_peak_bytes)."""
+    n = len(ops)
+    cand = (C.c_int32 * len(k_candidates))(*k_candidates)
+    ks, modes = (C.c_int32 * n)(), (C.c_int32 * n)()
+    sec, peak, b = C.c_double(), C.c_uint64(), C.c_int64()
+    st = _lib.osdp_plan_batch(_op_array(ops), n, C.byref(dev), batch_max, cand, len(k_candidates), ks, modes,
+                              C.byref(b), C.byref(sec), C.byref(peak))
+    if check and st not in (OSDP_OK, OSDP_ERR_INFEASIBLE):
+        raise OsdpError(st, "osdp_plan_batch")
+    if st != OSDP_OK:
+        return st, None, None, None, None, None
+    return st, list(ks), list(modes), int(b.value), float(sec.value), int(peak.value)
+
+
+# ------------------------------------------------------------------------------ convenience (marshalling only)
+class SplitMlp:
+    """Holds a descriptor and caller-owned workspace/outputs for repeated calls on one device."""
+
+    def __init__(self, tokens, hidden, ffn, dtype: torch.dtype, k: int, device="cuda"):
+        self.desc = make_desc(tokens, hidden, ffn, dtype, k)
+        self.dtype, self.device = dtype, torch.device(device)
+        self.ws_fwd_bytes = osdp_split_mlp_workspace_bytes(self.desc, OSDP_FWD)
+        self.ws_bwd_bytes = osdp_split_mlp_workspace_bytes(self.desc, OSDP_BWD)
+        if self.ws_fwd_bytes == 0:
+            raise OsdpError(OSDP_ERR_SHAPE, "SplitMlp: invalid descriptor")
+        self.workspace = torch.empty(max(self.ws_fwd_bytes, self.ws_bwd_bytes), dtype=torch.uint8, device=self.device)
+
+    def forward(self, X, W1, b1, W2, b2, Y=None, stream=None):
+        if Y is None:
+            Y = torch.empty_like(X)
+        osdp_split_mlp_forward(self.desc, X, W1, b1, W2, b2, Y, self.workspace, stream=stream)
+        return Y
+
+    def backward(self, X, W1, b1, W2, dY, out=None, stream=None):
+        if out is None:
+            out = dict(dX=torch.empty_like(X),
+                       dW1=torch.empty(W1.shape, dtype=torch.float32, device=X.device),
+                       db1=torch.empty(b1.shape, dtype=torch.float32, device=X.device),
+                       dW2=torch.empty(W2.shape, dtype=torch.float32, device=X.device),
+                       db2=torch.empty(W2.shape[1], dtype=torch.float32, device=X.device))
+        osdp_split_mlp_backward(self.desc, X, W1, b1, W2, None, dY, out["dX"], out["dW1"], out["db1"], out["dW2"],
+                                out["db2"], self.workspace, stream=stream)
+        return out

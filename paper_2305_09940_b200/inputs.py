@@ -1,0 +1,112 @@
+"""Seeded synthetic inputs for the split-MLP hot path.
+
+This module serves both the CUDA path and the oracle (tests hand the SAME arrays to each). It holds
+none of the method's arithmetic: it only draws numbers and rounds them once to the storage dtype.
+
+Recipe (BASELINE.json configs):
+  X, dY ~ N(0, 1);  W1, W2, b1, b2 ~ N(0, std 0.02); dense, no structure.
+  Element ``i`` of tensor stream ``sid`` under ``seed`` is a pure function of (seed, sid, i):
+  a counter-based 64-bit mix (splitmix64 finaliser) gives two 32-bit uniforms, Box-Muller in fp64
+  gives one standard normal.  No library RNG is involved, so the inputs never change with a
+  numpy/torch version.  Values are then rounded ONCE (round-to-nearest-even) to the storage dtype
+  (bf16 or fp32); both the GPU and the oracle see exactly those stored values.
+
+The paper names no dataset (PAPER.md:199 uses minGPT models; throughput does not depend on token
+content), so these tensors stand in for its activations/weights with GPT-style init.
+"""
+from __future__ import annotations
+
+import dataclasses
+
+import numpy as np
+import torch
+
+# Per-tensor stream ids (fixed; part of the recipe).
+STREAM_X, STREAM_W1, STREAM_B1, STREAM_W2, STREAM_B2, STREAM_DY = 1, 2, 3, 4, 5, 6
+
+_GOLDEN = np.uint64(0x9E3779B97F4A7C15)
+_M1 = np.uint64(0xBF58476D1CE4E5B9)
+_M2 = np.uint64(0x94D049BB133111EB)
+
+
+def _mix64(z: np.ndarray) -> np.ndarray:
+    """splitmix64 finaliser on a uint64 array (wrapping arithmetic)."""
+    z = (z ^ (z >> np.uint64(30))) * _M1
+    z = (z ^ (z >> np.uint64(27))) * _M2
+    return z ^ (z >> np.uint64(31))
+
+
+def _key(seed: int, sid: int) -> np.uint64:
+    with np.errstate(over="ignore"):
+        k = _mix64(np.array([np.uint64(seed & 0xFFFFFFFFFFFFFFFF)], dtype=np.uint64) * _GOLDEN
+                   + np.uint64(sid))
+        return _mix64(k + _GOLDEN)[0]
+
+
+def standard_normal(seed: int, sid: int, start: int, count: int) -> np.ndarray:
+    """fp64 standard normals for flat indices [start, start+count) of stream (seed, sid)."""
+    key = _key(seed, sid)
+    with np.errstate(over="ignore"):
+        idx = np.arange(start, start + count, dtype=np.uint64)
+        bits = _mix64(key + idx * _GOLDEN)
+    u1 = ((bits >> np.uint64(32)).astype(np.float64) + 0.5) * (1.0 / 4294967296.0)
+    u2 = ((bits & np.uint64(0xFFFFFFFF)).astype(np.float64) + 0.5) * (1.0 / 4294967296.0)
+    return np.sqrt(-2.0 * np.log(u1)) * np.cos((2.0 * np.pi) * u2)
+
+
+def normal_tensor(seed: int, sid: int, shape, std: float, dtype: torch.dtype,
+                  chunk: int = 1 << 22) -> torch.Tensor:
+    """CPU tensor of ``shape`` ~ N(0, std), rounded once (RNE) to ``dtype`` (torch.float32/bfloat16)."""
+    n = int(np.prod(shape))
+    out = torch.empty(n, dtype=dtype)
+    for s in range(0, n, chunk):
+        c = min(chunk, n - s)
+        z = standard_normal(seed, sid, s, c) * std
+        out[s:s + c] = torch.from_numpy(z).to(torch.float32).to(dtype)
+    return out.reshape(*shape)
+
+
+@dataclasses.dataclass
+class MlpInputs:
+    """One MLP operator's tensors, stored values (CPU).  Layout: row-major, W is [in x out]."""
+    X: torch.Tensor    # [T, h]
+    W1: torch.Tensor   # [h, f]
+    b1: torch.Tensor   # [f]
+    W2: torch.Tensor   # [f, h]
+    b2: torch.Tensor   # [h]
+    dY: torch.Tensor   # [T, h]
+
+    def as_f64(self) -> dict:
+        """Exact widening of the stored values to fp64 numpy (what the oracle consumes)."""
+        return {k: getattr(self, k).to(torch.float64).numpy() for k in ("X", "W1", "b1", "W2", "b2", "dY")}
+
+    def to(self, device) -> "MlpInputs":
+        return MlpInputs(*[getattr(self, k).to(device) for k in ("X", "W1", "b1", "W2", "b2", "dY")])
+
+
+def mlp_inputs(tokens: int, hidden: int, ffn: int, dtype: torch.dtype, seed: int = 0,
+               w_std: float = 0.02) -> MlpInputs:
+    """The recipe above for one operator.  ``seed`` selects the operator (C5: seed = layer index)."""
+    return MlpInputs(
+        X=normal_tensor(seed, STREAM_X, (tokens, hidden), 1.0, dtype),
+        W1=normal_tensor(seed, STREAM_W1, (hidden, ffn), w_std, dtype),
+        b1=normal_tensor(seed, STREAM_B1, (ffn,), w_std, dtype),
+        W2=normal_tensor(seed, STREAM_W2, (ffn, hidden), w_std, dtype),
+        b2=normal_tensor(seed, STREAM_B2, (hidden,), w_std, dtype),
+        dY=normal_tensor(seed, STREAM_DY, (tokens, hidden), 1.0, dtype),
+    )
+
+
+# BASELINE.json configs, by short name.  k lists are the split counts each config is run at.
+CONFIGS = {
+    "C1": dict(tokens=512, hidden=256, ffn=1024, dtype="f32", ks=(4,), seed=0),
+    "C2": dict(tokens=8192, hidden=1024, ffn=4096, dtype="bf16", ks=(1, 2, 4, 8), seed=0),
+    "C3": dict(tokens=32768, hidden=4096, ffn=16384, dtype="bf16", ks=(1, 4, 16), seed=0),
+    "C4": dict(tokens=8192, hidden=8192, ffn=32768, dtype="bf16", ks=(1, 2, 4, 8, 16, 32), seed=0),
+    "C5": dict(tokens=16384, hidden=2048, ffn=8192, dtype="bf16", ks=None, seed=0, layers=24,
+               act_cap_bytes=24 << 30),
+}
+
+
+def torch_dtype(name: str) -> torch.dtype:
+    return {"f32": torch.float32, "bf16": torch.bfloat16}[name]

@@ -1,0 +1,260 @@
+"""A9: cost model + planner.  The oracle (oracle/plan_oracle.py) is pinned to what the paper states in
+closed form; the library (osdp_cost_eval / osdp_plan / osdp_plan_batch) must agree with the oracle exactly
+(integers: bytes, picoseconds, k, mode).  CPU only — these calls never touch the GPU."""
+import itertools
+import math
+import os
+import random
+
+import pytest
+
+from oracle import plan_oracle as P
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def paper_constants():
+    out = {}
+    for line in open(os.path.join(GOLDEN, "paper_constants.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        name, value = line.split()[:2]
+        out[name] = float(value)
+    return out
+
+
+# ------------------------------------------------------------------ oracle pins (paper's closed forms)
+def test_unit_pin_gpt3_matmul_2_24_gb():
+    c = paper_constants()
+    op = P.OpCost(extra_summed=int(c["matmul_params"]) * 4)          # gathered fp32 parameters
+    p, _, _ = P.cost_eval(op, P.ZDP, 1, 0, P.Device(N=8))
+    assert round(p / 2 ** 30, 2) == c["matmul_gib"]
+    g = int(c["default_granularity"])
+    p4, _, _ = P.cost_eval(op, P.ZDP, g, 0, P.Device(N=8))
+    assert p4 == -(-p // g)                                           # size / slice_granularity
+
+
+@pytest.mark.parametrize("N", [2, 3, 8, 16, 64])
+def test_zdp_comm_is_1p5x_dp_and_model_states_are_1_over_N(N):
+    c = paper_constants()
+    op = P.OpCost(S=3.0e8, model=16 * 10 ** 9, act=12345, extra_fixed=77, gamma=0.25)
+    dev = P.Device(N=N, alpha=3e-5, beta=1.0 / 12e9)
+    b = 4
+    pd, _, td = P.cost_eval(op, P.DP, 1, b, dev)
+    pz, _, tz = P.cost_eval(op, P.ZDP, 1, b, dev)
+    assert math.isclose((tz - b * op.gamma) / (td - b * op.gamma), c["zdp_over_dp_comm"], rel_tol=1e-12)
+    assert math.isclose(td - b * op.gamma, 2 * (N - 1) * (dev.alpha + op.S * dev.beta / N), rel_tol=1e-12)
+    assert pd - pz == op.model - -(-op.model // N)                     # only the model states shrink
+    assert pd == op.model + b * op.act + op.extra_fixed                # DP formula
+
+
+def test_N1_modes_coincide_and_comm_vanishes():
+    op = P.OpCost(S=1e9, model=10 ** 9, act=5, gamma=0.5, delta=0.125, extra_transient=1000)
+    dev = P.Device(N=1, alpha=1.0, beta=1.0)
+    assert P.cost_eval(op, P.DP, 4, 3, dev) == P.cost_eval(op, P.ZDP, 4, 3, dev)
+    assert P.cost_eval(op, P.DP, 4, 3, dev)[2] == 3 * 0.5 + 3 * 0.125
+    assert P.cost_eval(op, P.DP, 4, 3, dev)[1] == 250
+
+
+def test_table1_operator_counts():
+    """An 'operator' is one attention or one MLP block (+2): ops = 2 layers + 2."""
+    for layers, ops in ((48, 98), (96, 194), (2, 6), (4, 10), (24, 50)):
+        assert ops - 2 * layers == paper_constants()["table1_ops_minus_2layers"]
+
+
+def _ops(n, seed, identical=False):
+    rng = random.Random(seed)
+    out = []
+    for _ in range(n):
+        out.append(P.OpCost(S=rng.randrange(1, 64) * 2.0 ** 20, model=rng.randrange(1, 64) << 20,
+                            act=rng.randrange(0, 8) << 10, extra_fixed=rng.randrange(0, 4) << 10,
+                            extra_summed=rng.randrange(0, 64) << 20, extra_transient=rng.randrange(0, 64) << 20,
+                            gamma=rng.randrange(1, 100) / 1024.0, delta=rng.randrange(0, 16) / 4096.0))
+    if identical:
+        out = [out[0]] * n
+    return out
+
+
+def test_oracle_unlimited_memory_gives_all_dp_k1_and_tight_memory_is_infeasible():
+    ops = _ops(4, 1)
+    dev = P.Device(N=4, alpha=1e-3, beta=1e-9, mem_limit=1 << 62)
+    modes, ks, _, _ = P.plan_brute_force(ops, dev, 2, [1, 2, 4])
+    assert modes == [P.DP] * 4 and ks == [1] * 4
+    least = min(P.plan_memory_time(ops, m, k, 2, dev)[0]
+                for m in itertools.product((0, 1), repeat=4) for k in itertools.product((1, 2, 4), repeat=4))
+    assert P.plan_brute_force(ops, P.Device(N=4, alpha=1e-3, beta=1e-9, mem_limit=least - 1), 2, [1, 2, 4]) is None
+    assert P.plan_brute_force(ops, P.Device(N=4, alpha=1e-3, beta=1e-9, mem_limit=least), 2, [1, 2, 4]) is not None
+
+
+def test_oracle_monotone_in_memory_limit():
+    ops = _ops(4, 2)
+    lo = P.plan_memory_time(ops, [1] * 4, [4] * 4, 1, P.Device(N=8))[0]
+    hi = P.plan_memory_time(ops, [0] * 4, [1] * 4, 1, P.Device(N=8))[0]
+    prev_t = None
+    for lim in range(lo, hi + (hi - lo) // 8, max(1, (hi - lo) // 8)):
+        r = P.plan_brute_force(ops, P.Device(N=8, alpha=1e-4, beta=1e-9, mem_limit=lim), 1, [1, 2, 4])
+        if r is None:
+            assert prev_t is None
+            continue
+        assert prev_t is None or r[2] <= prev_t          # more memory never makes the best plan slower
+        prev_t = r[2]
+
+
+def test_oracle_splits_bigger_operators_first():
+    """'prioritizing larger ones': same time cost of splitting, bigger sliceable part."""
+    small = P.OpCost(model=1 << 20, extra_summed=8 << 20, gamma=0.5, delta=1 / 64)
+    big = P.OpCost(model=1 << 20, extra_summed=64 << 20, gamma=0.5, delta=1 / 64)
+    ops = [small, big, small]
+    full = sum(o.model + o.extra_summed for o in ops)
+    dev = P.Device(N=1, mem_limit=full - (24 << 20))
+    modes, ks, _, _ = P.plan_brute_force(ops, dev, 1, [1, 2, 4])
+    assert ks == [1, 2, 1]
+
+
+# ------------------------------------------------------------------ library == oracle
+def _to_lib(lib, op):
+    return lib.osdp_op_cost(op.S, op.model, op.act, op.extra_fixed, op.extra_summed, op.extra_transient, op.gamma,
+                            op.delta)
+
+
+def _dev(lib, d):
+    return lib.osdp_device(d.N, d.alpha, d.beta, d.mem_limit)
+
+
+def test_library_exports_every_declared_symbol(lib):
+    import ctypes
+    import re
+    hdr = open(os.path.join(os.path.dirname(GOLDEN), "..", "include", "osdp.h")).read()
+    declared = set(re.findall(r"\b(osdp_[a-z_0-9]+)\s*\(", hdr))
+    assert declared == set(lib.EXPORTS), declared ^ set(lib.EXPORTS)
+    so = ctypes.CDLL(lib.LIB_PATH)
+    for name in declared:
+        assert hasattr(so, name), name
+    assert lib.osdp_status_string(0) == "ok" and "k" in lib.osdp_status_string(lib.OSDP_ERR_K)
+    assert "sm_100a" in lib.osdp_version()
+
+
+def test_cost_eval_matches_oracle(lib):
+    rng = random.Random(5)
+    for op in _ops(20, 3):
+        for mode in (0, 1):
+            for k in (1, 2, 3, 4, 16):
+                d = P.Device(N=rng.choice([1, 2, 8, 64]), alpha=rng.random() * 1e-3, beta=rng.random() * 1e-9)
+                b = rng.randrange(0, 9)
+                assert lib.osdp_cost_eval(_to_lib(lib, op), mode, k, b, _dev(lib, d)) == P.cost_eval(op, mode, k, b, d)
+    with pytest.raises(lib.OsdpError):
+        lib.osdp_cost_eval(_to_lib(lib, _ops(1, 0)[0]), 2, 1, 1, _dev(lib, P.Device()))
+    with pytest.raises(lib.OsdpError):
+        lib.osdp_cost_eval(_to_lib(lib, _ops(1, 0)[0]), 0, 0, 1, _dev(lib, P.Device()))
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_plan_matches_brute_force(lib, seed):
+    rng = random.Random(100 + seed)
+    n = rng.choice([1, 2, 3, 4])
+    cands = rng.choice([[1], [1, 2, 4], [1, 4, 16], [2, 3]])
+    ops = _ops(n, seed, identical=(seed % 4 == 3))
+    N = rng.choice([1, 2, 8])
+    base = P.Device(N=N, alpha=rng.random() * 1e-3, beta=rng.random() * 1e-9)
+    b = rng.randrange(1, 4)
+    lo = P.plan_memory_time(ops, [1] * n, [cands[-1]] * n, b, base)[0]
+    hi = P.plan_memory_time(ops, [0] * n, [cands[0]] * n, b, base)[0]
+    for frac in (-0.05, 0.0, 0.2, 0.5, 0.8, 1.0, 1.5):
+        d = P.Device(N=N, alpha=base.alpha, beta=base.beta, mem_limit=max(0, int(lo + frac * (hi - lo))))
+        ref = P.plan_brute_force(ops, d, b, cands)
+        st, ks, modes, sec, peak = lib.osdp_plan([_to_lib(lib, o) for o in ops], _dev(lib, d), b, cands)
+        if ref is None:
+            assert st == lib.OSDP_ERR_INFEASIBLE
+        else:
+            assert st == lib.OSDP_OK
+            assert (modes, ks, peak) == (ref[0], ref[1], ref[3])
+            assert round(sec * 1e12) == ref[2]
+
+
+def test_plan_table1_sized_models_with_brute_force_n6_to_8(lib):
+    """W&S models have 6-10 operators: exhaustive check at n = 6..8 with 2 x 2 options."""
+    for n in (6, 7, 8):
+        ops = _ops(n, 40 + n)
+        d0 = P.Device(N=8, alpha=1e-4, beta=1e-9)
+        lo = P.plan_memory_time(ops, [1] * n, [4] * n, 1, d0)[0]
+        hi = P.plan_memory_time(ops, [0] * n, [1] * n, 1, d0)[0]
+        d = P.Device(N=8, alpha=1e-4, beta=1e-9, mem_limit=(lo + hi) // 2)
+        ref = P.plan_brute_force(ops, d, 1, [1, 4])
+        st, ks, modes, sec, peak = lib.osdp_plan([_to_lib(lib, o) for o in ops], _dev(lib, d), 1, [1, 4])
+        assert st == lib.OSDP_OK and (modes, ks, peak) == (ref[0], ref[1], ref[3]) and round(sec * 1e12) == ref[2]
+
+
+def test_plan_ties_resolve_to_first_in_traversal_order(lib):
+    op = P.OpCost(model=1000, extra_summed=4000, gamma=1.0)              # delta = 0: every k costs the same time
+    ops = [op, op, op]
+    d = P.Device(N=1, mem_limit=3 * 1000 + 4000 + 2000 + 2000)           # one op may stay unsplit
+    ref = P.plan_brute_force(ops, d, 1, [1, 2, 4])
+    st, ks, modes, _, _ = lib.osdp_plan([_to_lib(lib, o) for o in ops], _dev(lib, d), 1, [1, 2, 4])
+    assert st == 0 and ks == ref[1] == [1, 2, 2] and modes == ref[0] == [0, 0, 0]     # N = 1: DP (reading P7)
+
+
+def test_plan_batch_matches_algorithm1(lib):
+    ops = _ops(3, 77)
+    for o in ops:
+        o.act = 8 << 20
+    d = P.Device(N=4, alpha=2e-3, beta=1e-9, mem_limit=sum(o.model + o.extra_summed + o.extra_transient for o in ops))
+    ref = P.schedule_brute_force(ops, d, [1, 2, 4], b_max=64)
+    st, ks, modes, b, sec, peak = lib.osdp_plan_batch([_to_lib(lib, o) for o in ops], _dev(lib, d), 64, [1, 2, 4])
+    assert ref is not None and st == 0
+    assert (modes, ks, b, peak) == (ref[0], ref[1], ref[4], ref[3]) and round(sec * 1e12) == ref[2]
+    tiny = P.Device(N=4, mem_limit=10)
+    assert lib.osdp_plan_batch([_to_lib(lib, o) for o in ops], _dev(lib, tiny), 64, [1, 2, 4])[0] == lib.OSDP_ERR_INFEASIBLE
+
+
+def test_plan_argument_errors(lib):
+    ops = [_to_lib(lib, o) for o in _ops(2, 9)]
+    d = _dev(lib, P.Device(N=1, mem_limit=1 << 60))
+    for bad in ([], [0, 1], [2, 2], [4, 2]):
+        with pytest.raises((lib.OsdpError, ValueError)):
+            if not bad:
+                raise ValueError("empty candidate list is rejected by the ABI (n_cand < 1)")
+            lib.osdp_plan(ops, d, 1, bad)
+
+
+def test_plan_scales_to_table1_depth(lib):
+    """N&D / I&C models have up to 194 operators of two alternating kinds."""
+    att = P.OpCost(S=4 * 2 ** 20, model=64 << 20, extra_summed=16 << 20, gamma=1 / 64, delta=1 / 4096)
+    mlp = P.OpCost(S=8 * 2 ** 20, model=128 << 20, extra_summed=128 << 20, gamma=1 / 32, delta=1 / 2048)
+    ops = [att, mlp] * 97
+    total = sum(o.model + o.extra_summed for o in ops)
+    d = P.Device(N=8, alpha=1e-4, beta=1e-10, mem_limit=int(total * 0.7))
+    st, ks, modes, sec, peak = lib.osdp_plan([_to_lib(lib, o) for o in ops], _dev(lib, d), 1, [1, 2, 4, 8])
+    assert st == lib.OSDP_OK and peak <= d.mem_limit
+    mem, ps = P.plan_memory_time(ops, modes, ks, 1, d)
+    assert mem == peak and ps == round(sec * 1e12)
+
+
+# ------------------------------------------------------------------ A10: workspace / MLP factors
+@pytest.mark.parametrize("T,h,f,dt,e", [(512, 256, 1024, 0, 4), (8192, 1024, 4096, 1, 2), (8192, 8192, 32768, 1, 2),
+                                        (1000, 264, 520, 1, 2), (7, 8, 8, 1, 2)])
+def test_workspace_and_mlp_factors_match_cost_model(lib, T, h, f, dt, e):
+    for k in (1, 2, 4, 7, 32):
+        if k > T:
+            continue
+        desc = lib.make_desc(T, h, f, dt, k)
+        for pass_, bwd in ((lib.OSDP_FWD, False), (lib.OSDP_BWD, True)):
+            ws = lib.osdp_split_mlp_workspace_bytes(desc, pass_)
+            assert ws == P.mlp_workspace_bytes(T, h, f, e, k, bwd)
+            c = lib.osdp_mlp_op_cost(desc, pass_)
+            assert c.model_bytes == P.mlp_persistent_bytes(T, h, f, e, bwd)
+            assert c.extra_fixed == (P.mlp_reduce_scratch_bytes(h, f) if bwd else 0)
+            assert c.extra_transient == (2 if bwd else 1) * T * f * e
+            # cost model predicts the workspace: sliceable/k + fixed, up to 256 B padding per buffer and
+            # (ragged T/k) one extra row per buffer
+            pred = -(-c.extra_transient // k) + c.extra_fixed
+            slack = (2 if bwd else 1) * (256 + (f * e if T % k else 0))
+            assert 0 <= ws - pred <= slack
+
+
+def test_descriptor_validation(lib):
+    assert lib.osdp_split_mlp_workspace_bytes(lib.make_desc(0, 8, 8, 1, 1), 0) == 0
+    assert lib.osdp_split_mlp_workspace_bytes(lib.make_desc(8, 12, 8, 1, 1), 0) == 0       # h % 8
+    assert lib.osdp_split_mlp_workspace_bytes(lib.make_desc(8, 8, 8, 1, 9), 0) == 0        # k > T
+    assert lib.osdp_split_mlp_workspace_bytes(lib.make_desc(8, 8, 8, 7, 1), 0) == 0        # dtype
+    assert lib.osdp_split_mlp_workspace_bytes(lib.make_desc(8, 8, 8, 1, 1), 2) == 0        # pass
+    assert lib.osdp_split_mlp_workspace_bytes(lib.make_desc(8, 4, 4, 0, 8), 1) > 0
