@@ -1,0 +1,450 @@
+#!/usr/bin/env python
+"""bench.py — split-MLP forward+backward throughput on B200 (BASELINE.json metric), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C4] [--k 4] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W
+
+A "step" is one pass of the whole hot path (steps A0-A8: osdp_split_mlp_forward then osdp_split_mlp_backward
+through the C ABI) over one batch of seeded synthetic input of the named workload.  `value` is executed
+TFLOP/s (14 T h f per step: 4 forward + 8 backward + 2 for the slice recompute of Z the method itself needs),
+summed over ranks (each rank runs the operator on its own token batch: data parallelism, weak scaling, no
+data-path collective).  Inputs are resident in HBM for `value`; `e2e` is the same metric with host (pinned)
+buffers, host<->device copies inside the timed region.
+
+`--impl reference` times the fp64 CPU oracle (oracle/mlp_oracle.py) as it stands on the box's host cores on a
+bounded token sample of the same workload (the reference arm of this tier); only rank 0 runs it.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import torch  # noqa: E402
+
+METRIC = "split_mlp_fwd_bwd_tflops"
+UNIT = "TFLOP/s"
+NOMINAL_BF16_TFLOPS = 2250.0      # dense bf16, B200 (B200_PROFILING.md; context only)
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+L2_BYTES = 126 << 20
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        d["source"] = "measured"
+        return d
+    d = dict(FALLBACK_PEAKS)
+    d["source"] = "fallback"
+    return d
+
+
+def executed_flops(T, h, f):
+    return 14.0 * T * h * f
+
+
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.lines, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._pump, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [x.strip() for x in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def dist_setup(n_gpus):
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        torch.cuda.set_device(local)
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    else:
+        torch.cuda.set_device(0)
+    return world, rank, local
+
+
+def barrier(world):
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    torch.cuda.synchronize()
+
+
+def max_over_ranks(x, world):
+    if world > 1:
+        import torch.distributed as dist
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+    return x
+
+
+# --------------------------------------------------------------------------------------------- reference arm
+def oracle_sample_tokens(h, f, target_flops=2.5e12):
+    """Token sample for the CPU oracle: about 10-30 s of fp64 work on a few dozen cores."""
+    t = int(target_flops / (14.0 * h * f))
+    return max(8, min(4096, 1 << max(0, t.bit_length() - 1)))
+
+
+def time_oracle(cfg, steps, warmup, sample_tokens=None):
+    """Times oracle.mlp_forward_backward as it stands on the first T' tokens of the workload."""
+    import numpy as np  # noqa: F401
+    from oracle import mlp_oracle as O
+    from paper_2305_09940_b200 import inputs as I
+    T, h, f = cfg["tokens"], cfg["hidden"], cfg["ffn"]
+    Ts = sample_tokens or oracle_sample_tokens(h, f)
+    Ts = min(Ts, T)
+    dt = I.torch_dtype(cfg["dtype"])
+    t0 = time.time()
+    inp = I.mlp_inputs(Ts, h, f, dt, seed=cfg["seed"])
+    x = inp.as_f64()
+    log(f"[oracle] inputs for T'={Ts} tokens generated in {time.time() - t0:.1f}s")
+    times = []
+    for i in range(warmup + steps):
+        t0 = time.perf_counter()
+        O.mlp_forward_backward(**x)
+        dtm = time.perf_counter() - t0
+        if i >= warmup:
+            times.append(dtm)
+    sec = sum(times) / len(times)
+    cores = torch.get_num_threads() if False else (os.cpu_count() or 1)
+    try:
+        import threadpoolctl
+        infos = [i for i in threadpoolctl.threadpool_info() if i.get("user_api") == "blas"]
+        if infos:
+            cores = max(i["num_threads"] for i in infos)
+    except Exception:
+        pass
+    return {"value": executed_flops(Ts, h, f) / sec / 1e12, "unit": UNIT, "cores": int(cores), "kind": "oracle",
+            "sample": f"first {Ts} of {T} tokens, full hidden={h} ffn={f}, fp64 numpy; cost is linear in tokens",
+            "seconds_per_sample": sec, "sample_tokens": Ts}
+
+
+def run_reference(args, cfg, rank):
+    if rank != 0:
+        return
+    r = time_oracle(cfg, max(1, min(args.steps, 3)), min(args.warmup, 1))
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": max(1, min(args.steps, 3)), "warmup": min(args.warmup, 1),
+            "ms_per_step": r["seconds_per_sample"] * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args, cfg), "tokens": cfg["tokens"], "hidden": cfg["hidden"],
+                       "ffn": cfg["ffn"], "k": args.k, "sample_tokens": r["sample_tokens"]},
+            "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_name(args, cfg):
+    return (f"{args.config}: MLP operator tokens={cfg['tokens']} hidden={cfg['hidden']} ffn={cfg['ffn']} "
+            f"{cfg['dtype']}, fwd+bwd at k={args.k} token slices")
+
+
+# --------------------------------------------------------------------------------------------------- our arm
+class Workload:
+    def __init__(self, lib, cfg, k, seed):
+        from paper_2305_09940_b200 import inputs as I
+        self.lib = lib
+        self.T, self.h, self.f = cfg["tokens"], cfg["hidden"], cfg["ffn"]
+        self.dtype = I.torch_dtype(cfg["dtype"])
+        t0 = time.time()
+        self.host = I.mlp_inputs(self.T, self.h, self.f, self.dtype, seed=seed, pin=True)
+        log(f"[bench] seeded host inputs generated in {time.time() - t0:.1f}s")
+        self.dev = self.host.to("cuda")
+        e = torch.empty
+        self.Y = e((self.T, self.h), dtype=self.dtype, device="cuda")
+        self.g = dict(dX=e((self.T, self.h), dtype=self.dtype, device="cuda"),
+                      dW1=e((self.h, self.f), dtype=torch.float32, device="cuda"),
+                      db1=e((self.f,), dtype=torch.float32, device="cuda"),
+                      dW2=e((self.f, self.h), dtype=torch.float32, device="cuda"),
+                      db2=e((self.h,), dtype=torch.float32, device="cuda"))
+        self.set_k(k)
+        # host-side result buffers for the e2e leg
+        self.hY = e((self.T, self.h), dtype=self.dtype, pin_memory=True)
+        self.hg = {n: e(t.shape, dtype=t.dtype, pin_memory=True) for n, t in self.g.items()}
+
+    def set_k(self, k):
+        self.k = k
+        self.op = self.lib.SplitMlp(self.T, self.h, self.f, self.dtype, k)
+
+    def step(self):
+        d = self.dev
+        self.op.forward(d.X, d.W1, d.b1, d.W2, d.b2, Y=self.Y)
+        n = self.lib.osdp_last_launch_count()
+        self.op.backward(d.X, d.W1, d.b1, d.W2, d.dY, out=self.g)
+        return n + self.lib.osdp_last_launch_count()
+
+    def step_e2e(self):
+        """Host buffers in, host buffers out: H2D of every input, the path, D2H of every output."""
+        h, d = self.host, self.dev
+        for n in ("X", "W1", "b1", "W2", "b2", "dY"):
+            getattr(d, n).copy_(getattr(h, n), non_blocking=True)
+        self.step()
+        self.hY.copy_(self.Y, non_blocking=True)
+        for n, t in self.g.items():
+            self.hg[n].copy_(t, non_blocking=True)
+
+    def h2d_bytes(self):
+        return sum(getattr(self.host, n).numel() * getattr(self.host, n).element_size()
+                   for n in ("X", "W1", "b1", "W2", "b2", "dY"))
+
+    def d2h_bytes(self):
+        return self.hY.numel() * self.hY.element_size() + sum(t.numel() * t.element_size() for t in self.hg.values())
+
+    def resident_bytes(self):
+        return self.h2d_bytes() + self.d2h_bytes()
+
+
+def timed_steps(fn, steps, world, flush=None):
+    """EXACTLY `steps` steps between barrier+synchronize brackets; per-step CUDA events on the current stream.
+    Returns (sum of step ms, wall ms of the bracket)."""
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    barrier(world)
+    t0 = time.perf_counter()
+    for a, b in evs:
+        if flush is not None:
+            flush.zero_()
+        a.record()
+        fn()
+        b.record()
+    barrier(world)
+    wall = (time.perf_counter() - t0) * 1e3
+    return sum(a.elapsed_time(b) for a, b in evs), wall
+
+
+def measure_peak_bytes(lib, cfg, k):
+    """Peak device bytes of ONE forward call and ONE backward call, each with only its own tensors live,
+    against the cost model (osdp_mlp_op_cost + osdp_cost_eval)."""
+    from paper_2305_09940_b200 import inputs as I
+    T, h, f = cfg["tokens"], cfg["hidden"], cfg["ffn"]
+    dt = I.torch_dtype(cfg["dtype"])
+    out = {}
+    for name, pass_ in (("fwd", lib.OSDP_FWD), ("bwd", lib.OSDP_BWD)):
+        torch.cuda.synchronize()
+        torch.cuda.empty_cache()
+        base = torch.cuda.memory_allocated()
+        torch.cuda.reset_peak_memory_stats()
+        desc = lib.make_desc(T, h, f, dt, k)
+        mk = lambda *s, d=dt: torch.empty(s, dtype=d, device="cuda")
+        X, W1, b1, W2, b2 = mk(T, h), mk(h, f), mk(f), mk(f, h), mk(h)
+        ws = torch.empty(lib.osdp_split_mlp_workspace_bytes(desc, pass_), dtype=torch.uint8, device="cuda")
+        for t in (X, W1, b1, W2, b2):
+            t.zero_()
+        if pass_ == lib.OSDP_FWD:
+            Y = mk(T, h)
+            lib.osdp_split_mlp_forward(desc, X, W1, b1, W2, b2, Y, ws)
+        else:
+            dY, dX = mk(T, h), mk(T, h)
+            dY.zero_()
+            f32 = torch.float32
+            dW1, db1, dW2, db2 = mk(h, f, d=f32), mk(f, d=f32), mk(f, h, d=f32), mk(h, d=f32)
+            lib.osdp_split_mlp_backward(desc, X, W1, b1, W2, b2, dY, dX, dW1, db1, dW2, db2, ws)
+        torch.cuda.synchronize()
+        measured = torch.cuda.max_memory_allocated() - base
+        c = lib.osdp_mlp_op_cost(desc, pass_)
+        dev = lib.osdp_device(1, 0.0, 0.0, 1 << 62)
+        p, tr, _ = lib.osdp_cost_eval(c, lib.OSDP_DP, k, 1, dev)
+        out[name] = {"measured": int(measured), "model": int(p + tr), "workspace": int(ws.numel())}
+        del X, W1, b1, W2, b2, ws
+        if pass_ == lib.OSDP_FWD:
+            del Y
+        else:
+            del dY, dX, dW1, db1, dW2, db2
+    torch.cuda.empty_cache()
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--k", type=int, default=4)
+    ap.add_argument("--no-sweep", action="store_true", help="skip the per-k TFLOP/s and peak-bytes table")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    from paper_2305_09940_b200 import inputs as I
+    cfg = dict(I.CONFIGS[args.config])
+
+    if args.impl == "reference":
+        rank = int(os.environ.get("RANK", "0"))
+        run_reference(args, cfg, rank)
+        return 0
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the osdp-b200 hot path has no CPU fallback")
+    from paper_2305_09940_b200 import binding as lib     # raises if the library was not built
+    world, rank, local = dist_setup(args.gpus)
+    peaks = load_peaks()
+    T, h, f = cfg["tokens"], cfg["hidden"], cfg["ffn"]
+    wl = Workload(lib, cfg, args.k, seed=cfg["seed"] + rank)
+    flops = executed_flops(T, h, f)
+    small = wl.resident_bytes() < 2 * L2_BYTES
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda") if small else None
+    l2_note = "flush: 256 MiB memset between timed steps" if small else "inputs+outputs exceed L2 (126 MB); no flush"
+
+    # ---- device-resident timing
+    for _ in range(args.warmup):
+        launches = wl.step()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ms_sum, wall_ms = timed_steps(wl.step, args.steps, world, flush)
+    clocks = sampler.stop()
+    ms_step = max_over_ranks(ms_sum / args.steps, world)
+    value = world * flops / (ms_step * 1e-3) / 1e12
+
+    # ---- per-launch trace of the same steps (CUDA events on the call's stream, inside the library)
+    lib.osdp_trace_enable(True)
+    for _ in range(args.steps):
+        if flush is not None:
+            flush.zero_()
+        wl.step()
+    trace = lib.osdp_trace_read()
+    lib.osdp_trace_enable(False)
+    per = {}
+    for sid, ms in trace:
+        per.setdefault(sid, []).append(ms)
+    total_traced = sum(sum(v) for v in per.values())
+    gemm_flops = 2.0 * T * h * f / args.k          # every GEMM launch of a slice: 2 T_s h f
+    kernels = {}
+    for sid, v in sorted(per.items()):
+        avg = sum(v) / len(v)
+        ent = {"step": lib.osdp_step_name(sid), "launches_per_step": len(v) // args.steps, "avg_ms": avg,
+               "share": sum(v) / total_traced}
+        if sid <= 7:
+            ent["tflops"] = gemm_flops / (avg * 1e-3) / 1e12
+        kernels[f"A{sid}" if sid <= 8 else "db1"] = ent
+    dom = max((s for s in per if s <= 7), key=lambda s: sum(per[s]))
+    dom_avg = sum(per[dom]) / len(per[dom])
+    achieved = gemm_flops / (dom_avg * 1e-3) / 1e12
+    peak = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]) if cfg["dtype"] == "bf16" else None
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get(f"{args.config}:k{args.k}:A{dom}")
+    roofline = {"bound": "tensor", "kernel": f"gemm_bf16_sm100_kernel [{lib.osdp_step_name(dom)}]",
+                "achieved": achieved, "peak": peak, "unit": UNIT, "frac": (achieved / peak) if peak else None,
+                "traffic": traffic, "peak_source": f"{peaks['source']} (bf16_tflops_sustained: kernel timed inside a long step)",
+                "frac_of_burst": achieved / peaks["bf16_tflops"], "frac_of_nominal": achieved / NOMINAL_BF16_TFLOPS,
+                "flops_per_launch": gemm_flops, "avg_launch_ms": dom_avg,
+                "how": "per-launch CUDA events recorded by the library on the call's stream over K traced steps"}
+    if cfg["dtype"] != "bf16":
+        roofline.update({"bound": "alu", "peak": 148 * 128 * 2 * 1.965e-3,
+                         "frac": achieved / (148 * 128 * 2 * 1.965e-3),
+                         "peak_source": "148 SMs x 128 FFMA/clk x 2 flop x 1.965 GHz (fp32 FFMA path)"})
+
+    # ---- end to end: host buffers, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        wl.step_e2e()
+        torch.cuda.synchronize()
+        e_sum, _ = timed_steps(wl.step_e2e, args.steps, world, None)
+        e_ms = max_over_ranks(e_sum / args.steps, world)
+        e2e = {"value": world * flops / (e_ms * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": e_ms,
+               "h2d_bytes_per_step": wl.h2d_bytes(), "d2h_bytes_per_step": wl.d2h_bytes()}
+
+    # ---- per-k table: TFLOP/s and peak bytes vs the cost model (rank 0, N = 1 only)
+    per_k = None
+    if not args.no_sweep and world == 1 and cfg.get("ks"):
+        per_k = []
+        for k in cfg["ks"]:
+            wl.set_k(k)
+            for _ in range(2):
+                wl.step()
+            s_ms, _ = timed_steps(wl.step, max(3, args.steps // 2), 1, flush)
+            s_ms /= max(3, args.steps // 2)
+            per_k.append({"k": k, "ms_per_step": s_ms, "tflops": flops / (s_ms * 1e-3) / 1e12,
+                          "frac_of_sustained_peak": flops / (s_ms * 1e-3) / 1e12 / peak if peak else None})
+        wl.set_k(args.k)
+        del wl
+        torch.cuda.empty_cache()
+        for ent in per_k:
+            ent["peak_bytes"] = measure_peak_bytes(lib, cfg, ent["k"])
+    cpu = None
+    if not args.no_cpu_baseline and rank == 0 and world == 1:
+        r = time_oracle(cfg, 1, 0)
+        cpu = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": cfg["dtype"], "data": "synthetic",
+                "config": {"workload": workload_name(args, cfg), "tokens_per_gpu": T, "hidden": h, "ffn": f,
+                           "k": args.k, "flops_per_step": flops, "flops_counted": "14*T*h*f executed (12*T*h*f model)",
+                           "l2": l2_note, "parallelism": f"dp{world} (independent token batches, no collective)"},
+                "value_model_flops_12x": value * 12.0 / 14.0,
+                "frac_of_sustained_peak": value / world / peak if peak else None,
+                "frac_of_nominal_peak": value / world / NOMINAL_BF16_TFLOPS,
+                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches) * args.steps,
+                "roofline": roofline, "kernels": kernels, "per_k": per_k, "cpu_baseline": cpu,
+                "wall_ms_timed_region": wall_ms}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -100,6 +100,17 @@ int osdp_split_mlp_backward(const osdp_mlp_desc* desc,
  * gpu_launches claim). */
 int64_t osdp_last_launch_count(void);
 
+/* ---- per-launch timing (measurement aid; bench.py's roofline) -------------------------------------------
+ * osdp_trace_enable(1): from now on every kernel launch of the calling thread's forward/backward calls is
+ * bracketed by two CUDA events recorded on the call's stream (nothing else changes; no synchronisation).
+ * osdp_trace_read: waits for the recorded events, writes up to max_entries (step id, milliseconds) pairs in
+ * launch order, clears the trace and returns the number of launches recorded since the last read (which may
+ * exceed max_entries), or -1 on a CUDA error.  Step ids: 1..7 = A1..A7 GEMMs, 8 = A8 db2 column sum, 9 = db1
+ * column sum (each column sum is two launches).  osdp_step_name(id) returns a static string. */
+int osdp_trace_enable(int on);
+int64_t osdp_trace_read(int64_t max_entries, int32_t* step_ids, float* ms);
+const char* osdp_step_name(int step_id);
+
 /* ---- A9: cost model and planner (host only) ------------------------------------------------------------
  * Per-operator record = the paper's "model description" entry: S_i and the three
  * memory factors, with M_extra divided into a part splitting does not shrink and two sliceable parts

@@ -31,7 +31,7 @@ OSDP_DP, OSDP_ZDP = 0, 1
 EXPORTS = (
     "osdp_status_string", "osdp_last_cuda_error", "osdp_version", "osdp_split_mlp_workspace_bytes",
     "osdp_split_mlp_forward", "osdp_split_mlp_backward", "osdp_last_launch_count", "osdp_cost_eval",
-    "osdp_mlp_op_cost", "osdp_plan", "osdp_plan_batch",
+    "osdp_mlp_op_cost", "osdp_plan", "osdp_plan_batch", "osdp_trace_enable", "osdp_trace_read", "osdp_step_name",
 )
 
 
@@ -76,6 +76,14 @@ _lib.osdp_plan_batch.argtypes = [C.POINTER(osdp_op_cost), C.c_int32, C.POINTER(o
                                  C.POINTER(C.c_int64), C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
 
 
+_lib.osdp_trace_enable.restype = C.c_int
+_lib.osdp_trace_enable.argtypes = [C.c_int]
+_lib.osdp_trace_read.restype = C.c_int64
+_lib.osdp_trace_read.argtypes = [C.c_int64, C.POINTER(C.c_int32), C.POINTER(C.c_float)]
+_lib.osdp_step_name.restype = C.c_char_p
+_lib.osdp_step_name.argtypes = [C.c_int]
+
+
 class OsdpError(RuntimeError):
     def __init__(self, status: int, where: str):
         self.status = status
@@ -99,6 +107,24 @@ def osdp_version() -> str:
 
 def osdp_last_launch_count() -> int:
     return int(_lib.osdp_last_launch_count())
+
+
+def osdp_trace_enable(on: bool) -> None:
+    _lib.osdp_trace_enable(1 if on else 0)
+
+
+def osdp_trace_read(max_entries: int = 1 << 16):
+    """[(step_id, milliseconds)] for every launch since the last read (waits for them)."""
+    ids, ms = (C.c_int32 * max_entries)(), (C.c_float * max_entries)()
+    n = int(_lib.osdp_trace_read(max_entries, ids, ms))
+    if n < 0:
+        raise OsdpError(OSDP_ERR_CUDA, "osdp_trace_read")
+    n = min(n, max_entries)
+    return [(int(ids[i]), float(ms[i])) for i in range(n)]
+
+
+def osdp_step_name(step_id: int) -> str:
+    return _lib.osdp_step_name(int(step_id)).decode()
 
 
 def _dtype_code(dtype: torch.dtype) -> int:

@@ -47,6 +47,15 @@ __host__ __device__ constexpr float kGeluA() { return 0.044715f; }
 // ---- host-side error bookkeeping (osdp_api.cu) -------------------------------------------------------------
 void note_cuda_error(cudaError_t e, const char* where);
 void count_launch();
+// Per-launch event trace (osdp_trace_*): launch wrappers bracket every kernel with LaunchTrace.
+void trace_set_step(int step_id);
+void trace_before(cudaStream_t st);
+void trace_after(cudaStream_t st);
+struct LaunchTrace {
+  cudaStream_t st;
+  explicit LaunchTrace(cudaStream_t s) : st(s) { trace_before(st); }
+  ~LaunchTrace() { trace_after(st); count_launch(); }
+};
 
 #define OSDP_CUDA_TRY(expr)                                   \
   do {                                                        \

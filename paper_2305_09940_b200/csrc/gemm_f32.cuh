@@ -93,8 +93,10 @@ __global__ void __launch_bounds__(F32_THREADS) gemm_f32_kernel(StridedOperands o
 template <int EPI>
 inline int launch_gemm_f32(const StridedOperands& op, const GemmShape& s, const EpiParams& ep, cudaStream_t st) {
   dim3 grid((s.N + F32_BN - 1) / F32_BN, (s.M + F32_BM - 1) / F32_BM);
-  gemm_f32_kernel<EPI><<<grid, F32_THREADS, 0, st>>>(op, s, ep);
-  count_launch();
+  {
+    LaunchTrace tr(st);
+    gemm_f32_kernel<EPI><<<grid, F32_THREADS, 0, st>>>(op, s, ep);
+  }
   OSDP_CUDA_TRY(cudaGetLastError());
   return OSDP_OK;
 }

@@ -446,8 +446,10 @@ inline int launch_gemm_bf16(const void* A, int64_t lda, const void* B, int64_t l
   const int tiles = num_m * num_n;
   const int sms = num_sms();
   const int grid = tiles < sms ? tiles : sms;
-  kernel<<<grid, kThreads, kSmemBytes, st>>>(ta, tb, s, ep);
-  count_launch();
+  {
+    LaunchTrace tr(st);
+    kernel<<<grid, kThreads, kSmemBytes, st>>>(ta, tb, s, ep);
+  }
   OSDP_CUDA_TRY(cudaGetLastError());
   return OSDP_OK;
 }

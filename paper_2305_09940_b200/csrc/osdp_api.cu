@@ -5,6 +5,7 @@
 // (dW1, dW2, db1, db2) are summed: "=" on slice 0, "+=" afterwards, in fixed slice order.
 #include <mutex>
 #include <string>
+#include <vector>
 
 #include "common.cuh"
 #include "gemm_f32.cuh"
@@ -22,6 +23,38 @@ void note_cuda_error(cudaError_t e, const char* where) {
   g_last_error = std::string(cudaGetErrorName(e)) + ": " + cudaGetErrorString(e) + " at " + where;
 }
 void count_launch() { ++g_launches; }
+
+namespace {
+struct TraceState {
+  bool on = false;
+  int step = 0;
+  std::vector<cudaEvent_t> pool;    // 2 events per recorded launch, reused across reads
+  std::vector<int32_t> steps;       // step id per recorded launch
+  bool failed = false;
+  cudaEvent_t get(size_t i) {
+    while (pool.size() <= i) {
+      cudaEvent_t e = nullptr;
+      if (cudaEventCreate(&e) != cudaSuccess) { failed = true; return nullptr; }
+      pool.push_back(e);
+    }
+    return pool[i];
+  }
+};
+thread_local TraceState g_trace;
+}  // namespace
+
+void trace_set_step(int step_id) { g_trace.step = step_id; }
+void trace_before(cudaStream_t st) {
+  if (!g_trace.on) return;
+  cudaEvent_t e = g_trace.get(2 * g_trace.steps.size());
+  if (e && cudaEventRecord(e, st) != cudaSuccess) g_trace.failed = true;
+}
+void trace_after(cudaStream_t st) {
+  if (!g_trace.on) return;
+  cudaEvent_t e = g_trace.get(2 * g_trace.steps.size() + 1);
+  if (e && cudaEventRecord(e, st) != cudaSuccess) g_trace.failed = true;
+  g_trace.steps.push_back(g_trace.step);
+}
 
 namespace sm100 {
 EncodeTiledFn encode_tiled_fn() {
@@ -144,6 +177,47 @@ const char* osdp_last_cuda_error(void) { return g_last_error.c_str(); }
 const char* osdp_version(void) { return "osdp-b200 0.1.0 (sm_100a)"; }
 int64_t osdp_last_launch_count(void) { return g_launches; }
 
+int osdp_trace_enable(int on) {
+  g_trace.on = on != 0;
+  if (!g_trace.on) g_trace.steps.clear();
+  return OSDP_OK;
+}
+
+int64_t osdp_trace_read(int64_t max_entries, int32_t* step_ids, float* ms) {
+  const int64_t n = (int64_t)g_trace.steps.size();
+  bool bad = g_trace.failed;
+  for (int64_t i = 0; i < n && !bad; ++i) {
+    float t = 0.f;
+    if (cudaEventSynchronize(g_trace.pool[2 * i + 1]) != cudaSuccess ||
+        cudaEventElapsedTime(&t, g_trace.pool[2 * i], g_trace.pool[2 * i + 1]) != cudaSuccess) {
+      bad = true;
+      break;
+    }
+    if (i < max_entries) {
+      if (step_ids) step_ids[i] = g_trace.steps[i];
+      if (ms) ms[i] = t;
+    }
+  }
+  g_trace.steps.clear();
+  g_trace.failed = false;
+  return bad ? -1 : n;
+}
+
+const char* osdp_step_name(int step_id) {
+  switch (step_id) {
+    case 1: return "A1 fwd GEMM1 + bias + GeLU";
+    case 2: return "A2 fwd GEMM2 + bias";
+    case 3: return "A3 bwd recompute GEMM1 (Z, H)";
+    case 4: return "A4 bwd dH GEMM + GeLU'";
+    case 5: return "A5 dW2 += H^T dY";
+    case 6: return "A6 dW1 += X^T dZ";
+    case 7: return "A7 dX = dZ W1^T";
+    case 8: return "A8 db2 column sum";
+    case 9: return "db1 column sum";
+    default: return "unknown";
+  }
+}
+
 size_t osdp_split_mlp_workspace_bytes(const osdp_mlp_desc* desc, int pass) {
   if (check_desc(desc) != OSDP_OK || (pass != OSDP_FWD && pass != OSDP_BWD)) return 0;
   return workspace_bytes(desc, pass);
@@ -192,9 +266,11 @@ int osdp_split_mlp_forward(const osdp_mlp_desc* desc, const void* X, const void*
     const char* Xs = (const char*)X + (size_t)lo * h * e;
     char* Ys = (char*)Y + (size_t)lo * h * e;
     // A1: H_s = gelu(X_s W1 + b1)
+    trace_set_step(1);
     EpiParams e1 = {b1, Hs, nullptr, nullptr, f, 0};
     OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_BIAS_GELU>(dt, Xs, h, W1, f, GemmShape{Ts, (int)f, (int)h}, e1, st)));
     // A2: Y_s = H_s W2 + b2
+    trace_set_step(2);
     EpiParams e2 = {b2, Ys, nullptr, nullptr, h, 0};
     OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_BIAS>(dt, Hs, f, W2, h, GemmShape{Ts, (int)h, (int)f}, e2, st)));
   }
@@ -233,21 +309,28 @@ int osdp_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const void
     const char* dYs = (const char*)dY + (size_t)lo * h * e;
     char* dXs = (char*)dX + (size_t)lo * h * e;
     // A3: Z_s = X_s W1 + b1, H_s = gelu(Z_s)
+    trace_set_step(3);
     EpiParams e3 = {b1, Zs, Hs, nullptr, f, 0};
     OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_BIAS_GELU_DUAL>(dt, Xs, h, W1, f, GemmShape{Ts, (int)f, (int)h}, e3, st)));
     // A4: dZ_s = (dY_s W2^T) (.) gelu'(Z_s), in place over Z_s
+    trace_set_step(4);
     EpiParams e4 = {nullptr, Zs, nullptr, Zs, f, 0};
     OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_DGELU>(dt, dYs, h, W2, h, GemmShape{Ts, (int)f, (int)h}, e4, st)));
     // A5: dW2 (+)= H_s^T dY_s
+    trace_set_step(5);
     EpiParams e5 = {nullptr, dW2, nullptr, nullptr, h, beta};
     OSDP_TRY((gemm<MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32>(dt, Hs, f, dYs, h, GemmShape{(int)f, (int)h, Ts}, e5, st)));
     // A8: db2 (+)= colsum(dY_s);  db1 (+)= colsum(dZ_s)
+    trace_set_step(8);
     OSDP_TRY(colsum(dt, dYs, Ts, (int)h, h, scratch, db2, beta, st));
+    trace_set_step(9);
     OSDP_TRY(colsum(dt, Zs, Ts, (int)f, f, scratch, db1, beta, st));
     // A6: dW1 (+)= X_s^T dZ_s
+    trace_set_step(6);
     EpiParams e6 = {nullptr, dW1, nullptr, nullptr, f, beta};
     OSDP_TRY((gemm<MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32>(dt, Xs, h, Zs, f, GemmShape{(int)h, (int)f, Ts}, e6, st)));
     // A7: dX_s = dZ_s W1^T
+    trace_set_step(7);
     EpiParams e7 = {nullptr, dXs, nullptr, nullptr, h, 0};
     OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_PLAIN>(dt, Zs, f, W1, f, GemmShape{Ts, (int)h, (int)f}, e7, st)));
   }

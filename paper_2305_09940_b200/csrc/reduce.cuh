@@ -83,11 +83,15 @@ inline int launch_colsum(const T* src, int rows, int cols, int64_t ld, float* sc
   constexpr int V = VecOf<T>::N;
   const int rows_per_chunk = (rows + kReduceRowChunks - 1) / kReduceRowChunks;
   dim3 grid((cols + 32 * V - 1) / (32 * V), kReduceRowChunks);
-  colsum_partial_kernel<T><<<grid, kReduceThreads, 0, st>>>(src, rows, cols, ld, scratch, rows_per_chunk);
-  count_launch();
+  {
+    LaunchTrace tr(st);
+    colsum_partial_kernel<T><<<grid, kReduceThreads, 0, st>>>(src, rows, cols, ld, scratch, rows_per_chunk);
+  }
   OSDP_CUDA_TRY(cudaGetLastError());
-  colsum_final_kernel<<<(cols + 255) / 256, 256, 0, st>>>(scratch, cols, out, beta);
-  count_launch();
+  {
+    LaunchTrace tr(st);
+    colsum_final_kernel<<<(cols + 255) / 256, 256, 0, st>>>(scratch, cols, out, beta);
+  }
   OSDP_CUDA_TRY(cudaGetLastError());
   return OSDP_OK;
 }

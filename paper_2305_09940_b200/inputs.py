@@ -24,45 +24,65 @@ import torch
 # Per-tensor stream ids (fixed; part of the recipe).
 STREAM_X, STREAM_W1, STREAM_B1, STREAM_W2, STREAM_B2, STREAM_DY = 1, 2, 3, 4, 5, 6
 
-_GOLDEN = np.uint64(0x9E3779B97F4A7C15)
-_M1 = np.uint64(0xBF58476D1CE4E5B9)
-_M2 = np.uint64(0x94D049BB133111EB)
+_MASK64 = (1 << 64) - 1
+_GOLDEN = 0x9E3779B97F4A7C15
+_M1 = 0xBF58476D1CE4E5B9
+_M2 = 0x94D049BB133111EB
 
 
-def _mix64(z: np.ndarray) -> np.ndarray:
-    """splitmix64 finaliser on a uint64 array (wrapping arithmetic)."""
-    z = (z ^ (z >> np.uint64(30))) * _M1
-    z = (z ^ (z >> np.uint64(27))) * _M2
-    return z ^ (z >> np.uint64(31))
+def _s64(v: int) -> int:
+    """Two's-complement reinterpretation of a 64-bit pattern as a signed Python int (torch has no uint64 math)."""
+    v &= _MASK64
+    return v - (1 << 64) if v >> 63 else v
 
 
-def _key(seed: int, sid: int) -> np.uint64:
-    with np.errstate(over="ignore"):
-        k = _mix64(np.array([np.uint64(seed & 0xFFFFFFFFFFFFFFFF)], dtype=np.uint64) * _GOLDEN
-                   + np.uint64(sid))
-        return _mix64(k + _GOLDEN)[0]
+def _mix64_int(z: int) -> int:
+    """splitmix64 finaliser on one Python int (64-bit wrapping)."""
+    z = ((z ^ (z >> 30)) * _M1) & _MASK64
+    z = ((z ^ (z >> 27)) * _M2) & _MASK64
+    return z ^ (z >> 31)
+
+
+def _lsr(z: torch.Tensor, s: int) -> torch.Tensor:
+    """Logical shift right of 64-bit patterns held in an int64 tensor."""
+    return (z >> s) & ((1 << (64 - s)) - 1)
+
+
+def _mix64(z: torch.Tensor) -> torch.Tensor:
+    """splitmix64 finaliser on 64-bit patterns held in an int64 tensor (wrapping multiply)."""
+    z = (z ^ _lsr(z, 30)) * _s64(_M1)
+    z = (z ^ _lsr(z, 27)) * _s64(_M2)
+    return z ^ _lsr(z, 31)
+
+
+def _key(seed: int, sid: int) -> int:
+    k = _mix64_int(((seed & _MASK64) * _GOLDEN + sid) & _MASK64)
+    return _mix64_int((k + _GOLDEN) & _MASK64)
+
+
+def standard_normal_t(seed: int, sid: int, start: int, count: int) -> torch.Tensor:
+    """fp64 standard normals (torch CPU tensor) for flat indices [start, start+count) of stream (seed, sid)."""
+    idx = torch.arange(start, start + count, dtype=torch.int64)
+    bits = _mix64(idx * _s64(_GOLDEN) + _s64(_key(seed, sid)))
+    u1 = (_lsr(bits, 32).to(torch.float64) + 0.5) * (1.0 / 4294967296.0)
+    u2 = ((bits & 0xFFFFFFFF).to(torch.float64) + 0.5) * (1.0 / 4294967296.0)
+    return torch.sqrt(-2.0 * torch.log(u1)) * torch.cos((2.0 * np.pi) * u2)
 
 
 def standard_normal(seed: int, sid: int, start: int, count: int) -> np.ndarray:
-    """fp64 standard normals for flat indices [start, start+count) of stream (seed, sid)."""
-    key = _key(seed, sid)
-    with np.errstate(over="ignore"):
-        idx = np.arange(start, start + count, dtype=np.uint64)
-        bits = _mix64(key + idx * _GOLDEN)
-    u1 = ((bits >> np.uint64(32)).astype(np.float64) + 0.5) * (1.0 / 4294967296.0)
-    u2 = ((bits & np.uint64(0xFFFFFFFF)).astype(np.float64) + 0.5) * (1.0 / 4294967296.0)
-    return np.sqrt(-2.0 * np.log(u1)) * np.cos((2.0 * np.pi) * u2)
+    return standard_normal_t(seed, sid, start, count).numpy()
 
 
 def normal_tensor(seed: int, sid: int, shape, std: float, dtype: torch.dtype,
-                  chunk: int = 1 << 22) -> torch.Tensor:
-    """CPU tensor of ``shape`` ~ N(0, std), rounded once (RNE) to ``dtype`` (torch.float32/bfloat16)."""
+                  chunk: int = 1 << 22, pin: bool = False) -> torch.Tensor:
+    """CPU tensor of ``shape`` ~ N(0, std), rounded once (RNE) to ``dtype`` (torch.float32/bfloat16).
+
+    The generator is counter-based, so the result does not depend on the chunk size or thread count."""
     n = int(np.prod(shape))
-    out = torch.empty(n, dtype=dtype)
+    out = torch.empty(n, dtype=dtype, pin_memory=pin)
     for s in range(0, n, chunk):
         c = min(chunk, n - s)
-        z = standard_normal(seed, sid, s, c) * std
-        out[s:s + c] = torch.from_numpy(z).to(torch.float32).to(dtype)
+        out[s:s + c] = (standard_normal_t(seed, sid, s, c) * std).to(torch.float32).to(dtype)
     return out.reshape(*shape)
 
 
@@ -85,15 +105,15 @@ class MlpInputs:
 
 
 def mlp_inputs(tokens: int, hidden: int, ffn: int, dtype: torch.dtype, seed: int = 0,
-               w_std: float = 0.02) -> MlpInputs:
+               w_std: float = 0.02, pin: bool = False) -> MlpInputs:
     """The recipe above for one operator.  ``seed`` selects the operator (C5: seed = layer index)."""
     return MlpInputs(
-        X=normal_tensor(seed, STREAM_X, (tokens, hidden), 1.0, dtype),
-        W1=normal_tensor(seed, STREAM_W1, (hidden, ffn), w_std, dtype),
-        b1=normal_tensor(seed, STREAM_B1, (ffn,), w_std, dtype),
-        W2=normal_tensor(seed, STREAM_W2, (ffn, hidden), w_std, dtype),
-        b2=normal_tensor(seed, STREAM_B2, (hidden,), w_std, dtype),
-        dY=normal_tensor(seed, STREAM_DY, (tokens, hidden), 1.0, dtype),
+        X=normal_tensor(seed, STREAM_X, (tokens, hidden), 1.0, dtype, pin=pin),
+        W1=normal_tensor(seed, STREAM_W1, (hidden, ffn), w_std, dtype, pin=pin),
+        b1=normal_tensor(seed, STREAM_B1, (ffn,), w_std, dtype, pin=pin),
+        W2=normal_tensor(seed, STREAM_W2, (ffn, hidden), w_std, dtype, pin=pin),
+        b2=normal_tensor(seed, STREAM_B2, (hidden,), w_std, dtype, pin=pin),
+        dY=normal_tensor(seed, STREAM_DY, (tokens, hidden), 1.0, dtype, pin=pin),
     )
 
 

@@ -1,0 +1,169 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 oracle.  GPU only (-m gpu).
+
+Bar (BASELINE.json north_star): per output tensor, max|gpu - ref| <= tol * max|ref| with tol = 2e-2 for bf16
+storage / fp32 accumulation and 1e-4 for the fp32 config; split-invariance across k <= 1e-5 relative (fp32).
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import mlp_oracle as O
+from paper_2305_09940_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+TOL = {torch.bfloat16: 2e-2, torch.float32: 1e-4}
+NAMES = ("Y", "dX", "dW1", "db1", "dW2", "db2")
+
+
+def run_gpu(lib, inp, k, dtype):
+    """One forward + backward through the C ABI; returns dict of CPU fp64 numpy outputs."""
+    T, h = inp.X.shape
+    f = inp.W1.shape[1]
+    d = inp.to("cuda")
+    op = lib.SplitMlp(T, h, f, dtype, k)
+    Y = op.forward(d.X, d.W1, d.b1, d.W2, d.b2)
+    g = op.backward(d.X, d.W1, d.b1, d.W2, d.dY)
+    torch.cuda.synchronize()
+    out = {"Y": Y}
+    out.update(g)
+    return {n: out[n].to(torch.float64).cpu().numpy() for n in NAMES}
+
+
+def rel_err(got, ref):
+    scale = float(np.max(np.abs(ref)))
+    return float(np.max(np.abs(got - ref))) / (scale if scale > 0 else 1.0)
+
+
+def check(got, ref, tol, what=""):
+    errs = {n: rel_err(got[n], ref[n]) for n in NAMES}
+    bad = {n: e for n, e in errs.items() if not (e <= tol)}
+    assert not bad, f"{what}: rel err over tol {tol}: {bad} (all: {errs})"
+    return errs
+
+
+# ------------------------------------------------------------------ C1: fp32 config, full oracle
+def test_c1_fp32_k4_matches_oracle_and_is_split_invariant(lib):
+    c = I.CONFIGS["C1"]
+    inp = I.mlp_inputs(c["tokens"], c["hidden"], c["ffn"], torch.float32, seed=c["seed"])
+    ref = O.mlp_forward_backward(**inp.as_f64())
+    outs = {k: run_gpu(lib, inp, k, torch.float32) for k in (1, 2, 4, 8, 3)}
+    for k, got in outs.items():
+        check(got, ref, 1e-4, f"C1 k={k}")
+    for k, got in outs.items():
+        for n in NAMES:
+            assert rel_err(got[n], outs[1][n]) <= 1e-5, (k, n)
+    for k in (2, 4, 8):                      # same per-row arithmetic for every k
+        assert np.array_equal(outs[k]["Y"], outs[1]["Y"]) and np.array_equal(outs[k]["dX"], outs[1]["dX"])
+
+
+# ------------------------------------------------------------------ small bf16 cases: several tiles + ragged tails
+@pytest.mark.parametrize("T,h,f,k", [
+    (256, 256, 512, 1),       # exact tiles
+    (384, 128, 512, 2),
+    (333, 136, 520, 3),       # ragged everywhere: T % k != 0, h, f not multiples of 64/128/256
+    (130, 72, 264, 1),
+    (1000, 320, 1032, 4),
+    (64, 8, 8, 4),            # minimum hidden/ffn
+    (5, 64, 128, 5),          # one token per slice (k = T)
+    (1, 16, 24, 1),           # a single token
+])
+def test_bf16_small_shapes_match_oracle(lib, T, h, f, k):
+    inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=7)
+    ref = O.mlp_forward_backward(**inp.as_f64())
+    check(run_gpu(lib, inp, k, torch.bfloat16), ref, 2e-2, f"bf16 {T}x{h}x{f} k={k}")
+
+
+@pytest.mark.parametrize("T,h,f,k", [(333, 136, 520, 3), (64, 8, 12, 4), (7, 4, 4, 7)])
+def test_fp32_small_shapes_match_oracle(lib, T, h, f, k):
+    inp = I.mlp_inputs(T, h, f, torch.float32, seed=8)
+    ref = O.mlp_forward_backward(**inp.as_f64())
+    check(run_gpu(lib, inp, k, torch.float32), ref, 1e-4, f"f32 {T}x{h}x{f} k={k}")
+
+
+def test_bf16_large_weights_stress_gelu_range(lib):
+    """W std 0.2 instead of 0.02 pushes |Z| to ~10: both GeLU tails and the steep middle are exercised."""
+    inp = I.mlp_inputs(512, 256, 1024, torch.bfloat16, seed=11, w_std=0.2)
+    ref = O.mlp_forward_backward(**inp.as_f64())
+    check(run_gpu(lib, inp, 2, torch.bfloat16), ref, 2e-2, "bf16 wide")
+
+
+# ------------------------------------------------------------------ C2: full oracle at every k
+@pytest.fixture(scope="module")
+def c2():
+    c = I.CONFIGS["C2"]
+    inp = I.mlp_inputs(c["tokens"], c["hidden"], c["ffn"], torch.bfloat16, seed=c["seed"])
+    return inp, O.mlp_forward_backward(**inp.as_f64())
+
+
+@pytest.mark.parametrize("k", [1, 2, 4, 8])
+def test_c2_bf16_matches_oracle(lib, c2, k):
+    inp, ref = c2
+    check(run_gpu(lib, inp, k, torch.bfloat16), ref, 2e-2, f"C2 k={k}")
+
+
+def test_c2_rows_are_bit_identical_across_k_and_runs(lib, c2):
+    inp, _ = c2
+    a, b, c = run_gpu(lib, inp, 1, torch.bfloat16), run_gpu(lib, inp, 8, torch.bfloat16), run_gpu(lib, inp, 8, torch.bfloat16)
+    assert np.array_equal(a["Y"], b["Y"]) and np.array_equal(a["dX"], b["dX"])      # reading S12
+    for n in NAMES:
+        assert np.array_equal(b[n], c[n]), n                                          # deterministic run to run
+
+
+# ------------------------------------------------------------------ errors and edge cases of the boundary
+def test_error_codes(lib):
+    T, h, f = 64, 64, 128
+    inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=1).to("cuda")
+    desc = lib.make_desc(T, h, f, torch.bfloat16, 2)
+    ws = torch.empty(lib.osdp_split_mlp_workspace_bytes(desc, lib.OSDP_BWD), dtype=torch.uint8, device="cuda")
+    Y = torch.full_like(inp.X, 3.0)
+    args = (inp.X, inp.W1, inp.b1, inp.W2, inp.b2, Y, ws)
+    assert lib.osdp_split_mlp_forward(desc, *args, check=False) == lib.OSDP_OK
+    assert lib.osdp_split_mlp_forward(desc, None, *args[1:], check=False) == lib.OSDP_ERR_NULL
+    assert lib.osdp_split_mlp_forward(lib.make_desc(T, h, f, torch.bfloat16, 0), *args, check=False) == lib.OSDP_ERR_K
+    assert lib.osdp_split_mlp_forward(lib.make_desc(T, h, f, torch.bfloat16, T + 1), *args, check=False) == lib.OSDP_ERR_K
+    assert lib.osdp_split_mlp_forward(lib.make_desc(T, h + 4, f, torch.bfloat16, 1), *args, check=False) == lib.OSDP_ERR_SHAPE
+    assert lib.osdp_split_mlp_forward(lib.make_desc(T, h, f, 5, 1), *args, check=False) == lib.OSDP_ERR_DTYPE
+    Y.fill_(3.0)
+    torch.cuda.synchronize()
+    assert lib.osdp_split_mlp_forward(desc, *args[:6], ws, workspace_bytes=16, check=False) == lib.OSDP_ERR_WORKSPACE
+    assert lib.osdp_split_mlp_forward(desc, *args[:6], ws.data_ptr() + 16, workspace_bytes=ws.numel() - 16,
+                                      check=False) == lib.OSDP_ERR_WORKSPACE
+    assert lib.osdp_split_mlp_forward(desc, inp.X.data_ptr() + 2, *args[1:], check=False) == lib.OSDP_ERR_ALIGN
+    torch.cuda.synchronize()
+    assert bool((Y == 3.0).all())                      # outputs untouched on error
+    with pytest.raises(lib.OsdpError):
+        lib.osdp_split_mlp_backward(desc, inp.X, inp.W1, inp.b1, inp.W2, None, None, Y, None, None, None, None, ws)
+    assert lib.osdp_last_launch_count() == 0
+
+
+def test_backward_overwrites_and_accepts_null_b2(lib):
+    """Reading S11 (overwrite, not accumulate) and S4 (b2 unused)."""
+    T, h, f = 200, 64, 256
+    inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=2)
+    ref = O.mlp_forward_backward(**inp.as_f64())
+    d = inp.to("cuda")
+    op = lib.SplitMlp(T, h, f, torch.bfloat16, 3)
+    out = dict(dX=torch.full_like(d.X, 9.0), dW1=torch.full((h, f), 9.0, device="cuda"),
+               db1=torch.full((f,), 9.0, device="cuda"), dW2=torch.full((f, h), 9.0, device="cuda"),
+               db2=torch.full((h,), 9.0, device="cuda"))
+    op.backward(d.X, d.W1, d.b1, d.W2, d.dY, out=out)
+    op.backward(d.X, d.W1, d.b1, d.W2, d.dY, out=out)      # second call must not accumulate into the first
+    torch.cuda.synchronize()
+    for n in ("dX", "dW1", "db1", "dW2", "db2"):
+        assert rel_err(out[n].double().cpu().numpy(), ref[n]) <= 2e-2, n
+    assert lib.osdp_last_launch_count() == 3 * 9          # k slices x (5 GEMMs + 2 x 2 reduction kernels)
+
+
+def test_runs_on_a_side_stream(lib):
+    T, h, f = 256, 128, 512
+    inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=4)
+    ref = O.mlp_forward_backward(**inp.as_f64())
+    d = inp.to("cuda")
+    op = lib.SplitMlp(T, h, f, torch.bfloat16, 2)
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        Y = op.forward(d.X, d.W1, d.b1, d.W2, d.b2, stream=s)
+    s.synchronize()
+    assert rel_err(Y.double().cpu().numpy(), ref["Y"]) <= 2e-2
