@@ -105,33 +105,14 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "reasons": sorted(reasons), "samples": len(sm)}
 
 
-def dist_setup(n_gpus):
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if world > 1:
-        import torch.distributed as dist
-        torch.cuda.set_device(local)
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    else:
-        torch.cuda.set_device(0)
-    return world, rank, local
-
-
 def barrier(world):
-    if world > 1:
-        import torch.distributed as dist
-        dist.barrier()
-    torch.cuda.synchronize()
+    from paper_2305_09940_b200 import dist as D
+    D.barrier()
 
 
 def max_over_ranks(x, world):
-    if world > 1:
-        import torch.distributed as dist
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
-    return x
+    from paper_2305_09940_b200 import dist as D
+    return D.max_over_ranks(x)
 
 
 # --------------------------------------------------------------------------------------------- reference arm
@@ -162,7 +143,7 @@ def time_oracle(cfg, steps, warmup, sample_tokens=None):
         if i >= warmup:
             times.append(dtm)
     sec = sum(times) / len(times)
-    cores = torch.get_num_threads() if False else (os.cpu_count() or 1)
+    cores = os.cpu_count() or 1
     try:
         import threadpoolctl
         infos = [i for i in threadpoolctl.threadpool_info() if i.get("user_api") == "blas"]
@@ -335,10 +316,11 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the osdp-b200 hot path has no CPU fallback")
     from paper_2305_09940_b200 import binding as lib     # raises if the library was not built
-    world, rank, local = dist_setup(args.gpus)
+    from paper_2305_09940_b200 import dist as D
+    world, rank, local = D.init("nccl")
     peaks = load_peaks()
     T, h, f = cfg["tokens"], cfg["hidden"], cfg["ffn"]
-    wl = Workload(lib, cfg, args.k, seed=cfg["seed"] + rank)
+    wl = Workload(lib, cfg, args.k, seed=D.rank_seed(cfg["seed"], rank))
     flops = executed_flops(T, h, f)
     small = wl.resident_bytes() < 2 * L2_BYTES
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda") if small else None
@@ -440,9 +422,7 @@ def main():
                 "roofline": roofline, "kernels": kernels, "per_k": per_k, "cpu_baseline": cpu,
                 "wall_ms_timed_region": wall_ms}
         print(json.dumps(line), flush=True)
-    if world > 1:
-        import torch.distributed as dist
-        dist.destroy_process_group()
+    D.finalize()
     return 0
 
 
