@@ -12,7 +12,7 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libosdp_b200.so")
+LIB_PATH = os.environ.get("OSDP_B200_LIB") or os.path.join(_HERE, "libosdp_b200.so")   # override: A/B builds
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(

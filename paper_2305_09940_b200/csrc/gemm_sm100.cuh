@@ -8,8 +8,10 @@
 //               descriptors into one of two 256-column TMEM accumulator stages; tcgen05.commit frees
 //               smem slots and publishes finished accumulators
 //   warp 2      TMEM allocator (512 columns) / deallocator
-//   warps 4..7  epilogue: tcgen05.ld (32 lanes x 32 columns per warp), bias / GeLU / GeLU' / fp32
-//               accumulate, 16-byte global stores; overlaps the next tile's main loop through the second
+//   warps 4..7  epilogue: tcgen05.ld (32 lanes x 32 columns per warp), bias / GeLU / GeLU' in fp32, then the
+//               warp's 32 rows x 128 B output segment goes to a 128B-swizzled smem staging buffer and out
+//               through TMA (cp.async.bulk.tensor store; cp.reduce.async.bulk.tensor .add for the fp32
+//               cross-slice accumulation of dW); overlaps the next tile's main loop through the second
 //               accumulator stage
 // Three mbarrier pipelines: smem full/empty (TMA <-> MMA), TMEM full/empty (MMA <-> epilogue).
 //
@@ -42,7 +44,10 @@ constexpr uint32_t kAStageBytes = BLOCK_M * BLOCK_K * 2;   // 16 KiB
 constexpr uint32_t kBStageBytes = BLOCK_N * BLOCK_K * 2;   // 32 KiB
 constexpr uint32_t kStageBytes = kAStageBytes + kBStageBytes;
 constexpr uint32_t kSmemTiles = kStages * kStageBytes;     // 192 KiB
-constexpr uint32_t kSmemBytes = kSmemTiles + 1024 /*align slack*/ + 256 /*barriers*/;
+constexpr uint32_t kStoreBufBytes = 32 * 128;              // one warp's 32 rows x 128 B output segment
+constexpr uint32_t kStoreBufsPerWarp = 2;
+constexpr uint32_t kSmemStore = kNumEpiWarps * kStoreBufsPerWarp * kStoreBufBytes;   // 32 KiB
+constexpr uint32_t kSmemBytes = kSmemTiles + kSmemStore + 1024 /*align slack*/ + 256 /*barriers*/;
 constexpr int kGroupM = 16;   // tile rasterisation: bands of 16 m-tiles, n walks across the band
 
 // ---------------------------------------------------------------------------------------------- PTX wrappers
@@ -96,6 +101,26 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map
       "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
       ::"r"(dst), "l"((uint64_t)map), "r"(bar), "r"(c_inner), "r"(c_outer)
       : "memory");
+}
+// smem -> global tile store / fp32 reduce-add (bulk async-group completion).
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, uint32_t src, int c_inner, int c_outer) {
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];"
+               ::"l"((uint64_t)map), "r"(src), "r"(c_inner), "r"(c_outer)
+               : "memory");
+}
+__device__ __forceinline__ void tma_reduce_add_2d(const CUtensorMap* map, uint32_t src, int c_inner, int c_outer) {
+  asm volatile("cp.reduce.async.bulk.tensor.2d.global.shared::cta.add.bulk_group [%0, {%2, %3}], [%1];"
+               ::"l"((uint64_t)map), "r"(src), "r"(c_inner), "r"(c_outer)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait() { asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory"); }
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void st_shared_v4(uint32_t addr, const uint4& v) {
+  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
   asm volatile("prefetch.tensormap [%0];" ::"l"((uint64_t)map) : "memory");
@@ -177,72 +202,36 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
 __device__ __forceinline__ float bf16_lo(uint32_t w) { return __uint_as_float(w << 16); }
 __device__ __forceinline__ float bf16_hi(uint32_t w) { return __uint_as_float(w & 0xFFFF0000u); }
 
-// One thread's 32 consecutive columns [n, n+32) of row `row` (valid when row_ok); groups of 8 columns are
-// written only while n + 8 g < N (N is a multiple of 8).
+// Output columns per 128-byte row segment (one staged TMA store): 64 bf16 or 32 fp32.
 template <int EPI>
-__device__ __forceinline__ void epilogue_chunk(const uint32_t (&acc)[32], int64_t row, bool row_ok, int n, int N,
-                                               const EpiParams& ep) {
-#pragma unroll
-  for (int g = 0; g < 4; ++g) {
-    const int ng = n + 8 * g;
-    if (ng >= N) break;   // warp-uniform
-    float v[8];
-#pragma unroll
-    for (int j = 0; j < 8; ++j) v[j] = __uint_as_float(acc[8 * g + j]);
+struct EpiTraits {
+  static constexpr bool kF32Out = (EPI == EPI_ACCUM_F32);
+  static constexpr int kChunkCols = kF32Out ? 32 : 64;
+};
 
-    if constexpr (EPI == EPI_BIAS_GELU || EPI == EPI_BIAS || EPI == EPI_BIAS_GELU_DUAL) {
-      const uint4 b = __ldg(reinterpret_cast<const uint4*>((const __nv_bfloat16*)ep.bias + ng));
-      const uint32_t bw[4] = {b.x, b.y, b.z, b.w};
+// Per-warp store pipeline: 2 staging buffers of 32 rows x 128 B (128B swizzle: 16-byte chunk j of row r sits at
+// chunk j ^ (r & 7), which is also what makes the 16-byte st.shared of 8 consecutive rows conflict-free).
+struct StorePipe {
+  uint32_t base;    // smem address of this warp's two buffers
+  uint32_t count;   // stores issued so far
+  int lane;
+  __device__ __forceinline__ void stage(const uint4 (&o)[8], const CUtensorMap* map, int c_inner, int c_outer, bool reduce_add) {
+    if (lane == 0) bulk_wait_read<kStoreBufsPerWarp - 1>();   // the buffer used two stores ago has been read out
+    __syncwarp();
+    const uint32_t buf = base + (count & 1u) * kStoreBufBytes;
+    const uint32_t rowaddr = buf + lane * 128;
 #pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        v[2 * j] += bf16_lo(bw[j]);
-        v[2 * j + 1] += bf16_hi(bw[j]);
-      }
+    for (int j = 0; j < 8; ++j) st_shared_v4(rowaddr + ((j ^ (lane & 7)) << 4), o[j]);
+    fence_proxy_async_smem();   // generic-proxy writes -> visible to the async proxy (TMA)
+    __syncwarp();
+    if (lane == 0) {
+      if (reduce_add) tma_reduce_add_2d(map, buf, c_inner, c_outer);
+      else            tma_store_2d(map, buf, c_inner, c_outer);
+      bulk_commit();
     }
-    if constexpr (EPI == EPI_ACCUM_F32) {
-      if (row_ok) {
-        float4* p = reinterpret_cast<float4*>((float*)ep.out0 + row * ep.ldo + ng);
-        float4 lo = make_float4(v[0], v[1], v[2], v[3]), hi = make_float4(v[4], v[5], v[6], v[7]);
-        if (ep.beta) {
-          const float4 a = p[0], c = p[1];
-          lo.x += a.x; lo.y += a.y; lo.z += a.z; lo.w += a.w;
-          hi.x += c.x; hi.y += c.y; hi.z += c.z; hi.w += c.w;
-        }
-        p[0] = lo;
-        p[1] = hi;
-      }
-    } else if constexpr (EPI == EPI_DGELU) {
-      if (row_ok) {
-        const int64_t o = row * ep.ldo + ng;
-        const uint4 z = *reinterpret_cast<const uint4*>((const __nv_bfloat16*)ep.aux + o);
-        const uint32_t zw[4] = {z.x, z.y, z.z, z.w};
-        uint32_t w[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j)
-          w[j] = pack_bf16x2(v[2 * j] * gelu_bwd<false>(bf16_lo(zw[j])), v[2 * j + 1] * gelu_bwd<false>(bf16_hi(zw[j])));
-        *reinterpret_cast<uint4*>((__nv_bfloat16*)ep.out0 + o) = make_uint4(w[0], w[1], w[2], w[3]);
-      }
-    } else {
-      if (row_ok) {
-        const int64_t o = row * ep.ldo + ng;
-        uint32_t w[4];
-        if constexpr (EPI == EPI_BIAS_GELU_DUAL) {
-#pragma unroll
-          for (int j = 0; j < 4; ++j) w[j] = pack_bf16x2(v[2 * j], v[2 * j + 1]);
-          *reinterpret_cast<uint4*>((__nv_bfloat16*)ep.out0 + o) = make_uint4(w[0], w[1], w[2], w[3]);
-        }
-        if constexpr (EPI == EPI_BIAS_GELU || EPI == EPI_BIAS_GELU_DUAL) {
-#pragma unroll
-          for (int j = 0; j < 8; ++j) v[j] = gelu_fwd<false>(v[j]);
-        }
-#pragma unroll
-        for (int j = 0; j < 4; ++j) w[j] = pack_bf16x2(v[2 * j], v[2 * j + 1]);
-        __nv_bfloat16* dst = (EPI == EPI_BIAS_GELU_DUAL) ? (__nv_bfloat16*)ep.out1 : (__nv_bfloat16*)ep.out0;
-        *reinterpret_cast<uint4*>(dst + o) = make_uint4(w[0], w[1], w[2], w[3]);
-      }
-    }
+    ++count;
   }
-}
+};
 
 // ------------------------------------------------------------------------------------------------- the kernel
 struct TileCoord {
@@ -260,12 +249,14 @@ __device__ __forceinline__ TileCoord tile_coord(int t, int num_m, int num_n) {
 template <int A_MAJOR, int B_MAJOR, int EPI>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
+                       const __grid_constant__ CUtensorMap tmap_out0, const __grid_constant__ CUtensorMap tmap_out1,
                        const GemmShape shape, const EpiParams ep) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;   // 128B swizzle atoms need 1024 B alignment
   const uint32_t smem_a = smem_base;
   const uint32_t smem_b = smem_base + kStages * kAStageBytes;
-  const uint32_t bars = smem_base + kSmemTiles;
+  const uint32_t smem_store = smem_base + kSmemTiles;
+  const uint32_t bars = smem_store + kSmemStore;
   const uint32_t full_bar = bars;                                  // [kStages]
   const uint32_t empty_bar = bars + 8 * kStages;                   // [kStages]
   const uint32_t tfull_bar = bars + 16 * kStages;                  // [kAccStages]
@@ -281,6 +272,8 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmap_a);
     tma_prefetch_desc(&tmap_b);
+    tma_prefetch_desc(&tmap_out0);
+    if constexpr (EPI == EPI_BIAS_GELU_DUAL) tma_prefetch_desc(&tmap_out1);
   }
   if (warp == 1 && lane == 0) {
     for (int i = 0; i < kStages; ++i) {
@@ -362,30 +355,88 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
     }
   } else if (warp >= kEpiWarp0) {
     // ================================================================== epilogue
+    using Tr = EpiTraits<EPI>;
+    constexpr int kChunk = Tr::kChunkCols;
     const int q = warp % 4;   // TMEM lane quarter this warp may access
+    StorePipe pipe{smem_store + q * (kStoreBufsPerWarp * kStoreBufBytes), 0u, lane};
     int it = 0;
     for (int t = blockIdx.x; t < num_tiles; t += gridDim.x, ++it) {
       const TileCoord tc = tile_coord(t, num_m, num_n);
       const int as = it & 1;
       const uint32_t aphase = (it >> 1) & 1;
-      const int64_t row = (int64_t)tc.m_blk * BLOCK_M + q * 32 + lane;
+      const int row0 = tc.m_blk * BLOCK_M + q * 32;     // first row of this warp's 32-row band
+      const int64_t row = row0 + lane;
       const bool row_ok = row < shape.M;
       const int n0 = tc.n_blk * BLOCK_N;
       mbar_wait(tfull_bar + 8 * as, aphase);
       tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * BLOCK_N;
+      const int n_end = min(n0 + BLOCK_N, shape.N);
 #pragma unroll 1
-      for (int c = 0; c < BLOCK_N / 32; ++c) {
-        if (n0 + c * 32 >= shape.N) break;   // warp-uniform
-        uint32_t acc[32];
-        tmem_ld_32x32(taddr + c * 32, acc);
+      for (int n = n0; n < n_end; n += kChunk) {
+        uint32_t acc[kChunk];
+#pragma unroll
+        for (int i = 0; i < kChunk / 32; ++i)
+          tmem_ld_32x32(taddr + (n - n0) + 32 * i, *reinterpret_cast<uint32_t(*)[32]>(&acc[32 * i]));
         tmem_ld_wait();
-        epilogue_chunk<EPI>(acc, row, row_ok, n0 + c * 32, shape.N, ep);
+        if (n + kChunk >= n_end) {   // last read of this accumulator stage: hand it back to the MMA warp early
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(tempty_bar + 8 * as);
+        }
+        uint4 o[8];
+        if constexpr (Tr::kF32Out) {
+#pragma unroll
+          for (int j = 0; j < 8; ++j) o[j] = make_uint4(acc[4 * j], acc[4 * j + 1], acc[4 * j + 2], acc[4 * j + 3]);
+          pipe.stage(o, &tmap_out0, n, row0, ep.beta != 0);
+        } else {
+          uint4 oz[8];   // EPI_BIAS_GELU_DUAL: Z_s (first output)
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            const int ng = n + 8 * j;
+            float v[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(acc[8 * j + i]);
+            if constexpr (EPI == EPI_BIAS_GELU || EPI == EPI_BIAS || EPI == EPI_BIAS_GELU_DUAL) {
+              if (ng < shape.N) {   // warp-uniform
+                const uint4 b = __ldg(reinterpret_cast<const uint4*>((const __nv_bfloat16*)ep.bias + ng));
+                const uint32_t bw[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                  v[2 * i] += bf16_lo(bw[i]);
+                  v[2 * i + 1] += bf16_hi(bw[i]);
+                }
+              }
+            }
+            if constexpr (EPI == EPI_BIAS_GELU_DUAL)
+              oz[j] = make_uint4(pack_bf16x2(v[0], v[1]), pack_bf16x2(v[2], v[3]), pack_bf16x2(v[4], v[5]), pack_bf16x2(v[6], v[7]));
+            if constexpr (EPI == EPI_BIAS_GELU || EPI == EPI_BIAS_GELU_DUAL) {
+#pragma unroll
+              for (int i = 0; i < 8; ++i) v[i] = gelu_fwd<false>(v[i]);
+            }
+            if constexpr (EPI == EPI_DGELU) {
+              uint4 z = make_uint4(0, 0, 0, 0);
+              if (row_ok && ng < shape.N) z = *reinterpret_cast<const uint4*>((const __nv_bfloat16*)ep.aux + row * ep.ldo + ng);
+              const uint32_t zw[4] = {z.x, z.y, z.z, z.w};
+#pragma unroll
+              for (int i = 0; i < 4; ++i) {
+                v[2 * i] *= gelu_bwd<false>(bf16_lo(zw[i]));
+                v[2 * i + 1] *= gelu_bwd<false>(bf16_hi(zw[i]));
+              }
+            }
+            o[j] = make_uint4(pack_bf16x2(v[0], v[1]), pack_bf16x2(v[2], v[3]), pack_bf16x2(v[4], v[5]), pack_bf16x2(v[6], v[7]));
+          }
+          if constexpr (EPI == EPI_BIAS_GELU_DUAL) {
+            pipe.stage(oz, &tmap_out0, n, row0, false);
+            pipe.stage(o, &tmap_out1, n, row0, false);
+          } else {
+            pipe.stage(o, &tmap_out0, n, row0, false);
+          }
+        }
       }
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(tempty_bar + 8 * as);
     }
+    if (lane == 0) bulk_wait<0>();   // all of this warp's stores have completed before the CTA's smem goes away
+    __syncwarp();
   }
 
   tc_fence_before();
@@ -404,18 +455,18 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 EncodeTiledFn encode_tiled_fn();   // osdp_api.cu: resolved through cudaGetDriverEntryPoint (no libcuda link)
 int num_sms();                     // osdp_api.cu
 
-// bf16 matrix stored row-major [outer x inner] with `ld` elements between rows; 128B-swizzled box.
+// Matrix stored row-major [outer x inner] with `ld` elements between rows; 128B-swizzled box.
 inline int make_tmap(CUtensorMap* map, const void* ptr, int64_t inner, int64_t outer, int64_t ld, int box_inner,
-                     int box_outer) {
+                     int box_outer, bool f32 = false) {
   EncodeTiledFn fn = encode_tiled_fn();
   if (!fn) return OSDP_ERR_CUDA;
   const cuuint64_t dims[2] = {(cuuint64_t)inner, (cuuint64_t)outer};
-  const cuuint64_t strides[1] = {(cuuint64_t)ld * 2};
+  const cuuint64_t strides[1] = {(cuuint64_t)ld * (f32 ? 4 : 2)};
   const cuuint32_t box[2] = {(cuuint32_t)box_inner, (cuuint32_t)box_outer};
   const cuuint32_t estr[2] = {1, 1};
-  const CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, estr,
-                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  const CUresult r = fn(map, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2,
+                        const_cast<void*>(ptr), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) {
     note_cuda_error(cudaErrorInvalidValue, "cuTensorMapEncodeTiled");
     return OSDP_ERR_CUDA;
@@ -427,7 +478,7 @@ inline int make_tmap(CUtensorMap* map, const void* ptr, int64_t inner, int64_t o
 template <int A_MAJOR, int B_MAJOR, int EPI>
 inline int launch_gemm_bf16(const void* A, int64_t lda, const void* B, int64_t ldb, const GemmShape& s,
                             const EpiParams& ep, cudaStream_t st) {
-  CUtensorMap ta, tb;
+  CUtensorMap ta, tb, to0, to1;
   int rc;
   if (A_MAJOR == MAJOR_K) rc = make_tmap(&ta, A, s.K, s.M, lda, BLOCK_K, BLOCK_M);
   else                    rc = make_tmap(&ta, A, s.M, s.K, lda, 64, BLOCK_K);
@@ -435,6 +486,15 @@ inline int launch_gemm_bf16(const void* A, int64_t lda, const void* B, int64_t l
   if (B_MAJOR == MAJOR_K) rc = make_tmap(&tb, B, s.K, s.N, ldb, BLOCK_K, BLOCK_N);
   else                    rc = make_tmap(&tb, B, s.N, s.K, ldb, 64, BLOCK_K);
   if (rc != OSDP_OK) return rc;
+  // outputs: [M x N] row-major, leading dimension ldo; one store = 32 rows x 128 bytes
+  constexpr bool f32out = EpiTraits<EPI>::kF32Out;
+  rc = make_tmap(&to0, ep.out0, s.N, s.M, ep.ldo, EpiTraits<EPI>::kChunkCols, 32, f32out);
+  if (rc != OSDP_OK) return rc;
+  to1 = to0;
+  if (EPI == EPI_BIAS_GELU_DUAL) {
+    rc = make_tmap(&to1, ep.out1, s.N, s.M, ep.ldo, EpiTraits<EPI>::kChunkCols, 32, false);
+    if (rc != OSDP_OK) return rc;
+  }
 
   auto kernel = gemm_bf16_sm100_kernel<A_MAJOR, B_MAJOR, EPI>;
   static bool attr_set = false;   // one process per GPU: the attribute is per function per device
@@ -448,7 +508,7 @@ inline int launch_gemm_bf16(const void* A, int64_t lda, const void* B, int64_t l
   const int grid = tiles < sms ? tiles : sms;
   {
     LaunchTrace tr(st);
-    kernel<<<grid, kThreads, kSmemBytes, st>>>(ta, tb, s, ep);
+    kernel<<<grid, kThreads, kSmemBytes, st>>>(ta, tb, to0, to1, s, ep);
   }
   OSDP_CUDA_TRY(cudaGetLastError());
   return OSDP_OK;
