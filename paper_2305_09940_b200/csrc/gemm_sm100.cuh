@@ -2,12 +2,16 @@
 //
 //   C[M x N] = A[M x K] * B[K x N]   (bf16 x bf16 -> fp32 in TMEM), then a fused epilogue (common.cuh Epi).
 //
-// Structure (one persistent CTA per SM, 256 threads, warp-specialised):
-//   warp 0      TMA producer: cp.async.bulk.tensor (128B-swizzled boxes) into a kStages-deep smem ring
-//   warp 1      MMA issuer: one lane issues tcgen05.mma.cta_group::1.kind::f16 (128 x 256 x 16) from smem
-//               descriptors into one of two 256-column TMEM accumulator stages; tcgen05.commit frees
-//               smem slots and publishes finished accumulators
-//   warp 2      TMEM allocator (512 columns) / deallocator
+// Structure: persistent CTA PAIRS (cluster of 2 = one TPC, one CTA per SM, 256 threads each, warp-specialised).
+// A pair computes one 256 x 256 output tile with tcgen05.mma.cta_group::2 (UMMA 256 x 256 x 16): CTA r of the
+// pair owns rows [128 r, 128 r + 128) of the tile (its TMEM lanes) and stages its own 128 A-rows plus ONE HALF
+// (128 columns) of the B tile, so every B byte is fetched from L2 and written to shared memory once per pair.
+//   warp 0      TMA producer (both CTAs): cp.async.bulk.tensor.cta_group::2 (128B-swizzled boxes) into a
+//               kStages-deep smem ring; both CTAs' loads complete_tx on the LEADER's full barrier
+//   warp 1      MMA issuer (leader CTA only): one lane issues the UMMAs from smem descriptors into one of two
+//               256-column TMEM accumulator stages; tcgen05.commit (multicast to both CTAs) frees the smem
+//               slots and publishes finished accumulators
+//   warp 2      TMEM allocator (512 columns, cta_group::2) / deallocator
 //   warps 4..7  epilogue: tcgen05.ld (32 lanes x 32 columns per warp), bias / GeLU / GeLU' in fp32, then the
 //               warp's 32 rows x 128 B output segment goes to a 128B-swizzled smem staging buffer and out
 //               through TMA (cp.async.bulk.tensor store; cp.reduce.async.bulk.tensor .add for the fp32
@@ -30,25 +34,27 @@
 namespace osdp {
 namespace sm100 {
 
-constexpr int BLOCK_M = 128;
-constexpr int BLOCK_N = 256;
+constexpr int BLOCK_M = 128;       // rows per CTA (TMEM lanes)
+constexpr int PAIR_M = 2 * BLOCK_M;   // rows per CTA pair = UMMA M
+constexpr int BLOCK_N = 256;       // columns per pair tile = UMMA N
+constexpr int HALF_N = BLOCK_N / 2;   // B columns staged by each CTA
 constexpr int BLOCK_K = 64;
 constexpr int UMMA_K = 16;
-constexpr int kStages = 4;
+constexpr int kStages = 6;
 constexpr int kAccStages = 2;
 constexpr int kTmemCols = 512;
 constexpr int kThreads = 256;
 constexpr int kEpiWarp0 = 4;
 constexpr int kNumEpiWarps = 4;
 constexpr uint32_t kAStageBytes = BLOCK_M * BLOCK_K * 2;   // 16 KiB
-constexpr uint32_t kBStageBytes = BLOCK_N * BLOCK_K * 2;   // 32 KiB
-constexpr uint32_t kStageBytes = kAStageBytes + kBStageBytes;
+constexpr uint32_t kBStageBytes = HALF_N * BLOCK_K * 2;    // 16 KiB (this CTA's half of the B tile)
+constexpr uint32_t kStageBytes = kAStageBytes + kBStageBytes;   // per CTA; the leader's barrier expects 2x
 constexpr uint32_t kSmemTiles = kStages * kStageBytes;     // 192 KiB
 constexpr uint32_t kStoreBufBytes = 32 * 128;              // one warp's 32 rows x 128 B output segment
 constexpr uint32_t kStoreBufsPerWarp = 2;
 constexpr uint32_t kSmemStore = kNumEpiWarps * kStoreBufsPerWarp * kStoreBufBytes;   // 32 KiB
 constexpr uint32_t kSmemBytes = kSmemTiles + kSmemStore + 1024 /*align slack*/ + 256 /*barriers*/;
-constexpr int kGroupM = 16;   // tile rasterisation: bands of 16 m-tiles, n walks across the band
+constexpr int kGroupM = 8;    // tile rasterisation: bands of 8 pair-tiles (2048 rows), n walks across the band
 
 // ---------------------------------------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -94,11 +100,30 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     }
   }
 }
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+// shared::cluster address of the same smem offset in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t mapa(uint32_t addr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+__device__ __forceinline__ void cluster_sync() {
+  asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+  asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
+// dst: this CTA's smem; bar: shared::cluster address of the mbarrier that receives complete_tx (the leader's).
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c_inner, int c_outer) {
   asm volatile(
-      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
       ::"r"(dst), "l"((uint64_t)map), "r"(bar), "r"(c_inner), "r"(c_outer)
       : "memory");
 }
@@ -127,13 +152,13 @@ __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
 }
 
 __device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols) {
-  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
+  asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
 }
 __device__ __forceinline__ void tmem_relinquish() {
-  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
 }
 __device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
-  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+  asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -144,14 +169,16 @@ __device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t adesc, uint6
       "{\n"
       ".reg .pred p;\n"
       "setp.ne.b32 p, %4, 0;\n"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
+      "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n"
       "}\n" ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
       : "memory");
 }
-// Arrive on an mbarrier when all tcgen05.mma issued so far by this thread have completed
-// (implies tcgen05.fence::before_thread_sync).
+// Arrive on the mbarrier at this smem offset in BOTH CTAs of the pair when all tcgen05.mma issued so far by this
+// thread have completed (implies tcgen05.fence::before_thread_sync).
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+  asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+               ::"r"(bar), "h"((uint16_t)3)
+               : "memory");
 }
 
 // 32 lanes x 32 consecutive fp32 columns: thread i of the warp gets row (lane base + i), v[j] = column j.
@@ -191,7 +218,7 @@ __device__ __forceinline__ uint64_t operand_desc(uint32_t tile_addr, int k16) {
 template <int A_MAJOR, int B_MAJOR>
 __host__ __device__ constexpr uint32_t make_idesc() {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)A_MAJOR << 15) | ((uint32_t)B_MAJOR << 16) |
-         ((uint32_t)(BLOCK_N >> 3) << 17) | ((uint32_t)(BLOCK_M >> 4) << 24);
+         ((uint32_t)(BLOCK_N >> 3) << 17) | ((uint32_t)(PAIR_M >> 4) << 24);
 }
 
 // --------------------------------------------------------------------------------------------------- epilogue
@@ -235,7 +262,7 @@ struct StorePipe {
 
 // ------------------------------------------------------------------------------------------------- the kernel
 struct TileCoord {
-  int m_blk, n_blk;
+  int m_blk, n_blk;   // pair-tile coordinates: rows m_blk * 256, columns n_blk * 256
 };
 __device__ __forceinline__ TileCoord tile_coord(int t, int num_m, int num_n) {
   const int per_group = kGroupM * num_n;
@@ -257,15 +284,18 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
   const uint32_t smem_b = smem_base + kStages * kAStageBytes;
   const uint32_t smem_store = smem_base + kSmemTiles;
   const uint32_t bars = smem_store + kSmemStore;
-  const uint32_t full_bar = bars;                                  // [kStages]
-  const uint32_t empty_bar = bars + 8 * kStages;                   // [kStages]
-  const uint32_t tfull_bar = bars + 16 * kStages;                  // [kAccStages]
-  const uint32_t tempty_bar = bars + 16 * kStages + 8 * kAccStages;   // [kAccStages]
+  const uint32_t full_bar = bars;                                  // [kStages]   (used in the leader CTA)
+  const uint32_t empty_bar = bars + 8 * kStages;                   // [kStages]   (one per CTA, multicast arrive)
+  const uint32_t tfull_bar = bars + 16 * kStages;                  // [kAccStages] (one per CTA, multicast arrive)
+  const uint32_t tempty_bar = bars + 16 * kStages + 8 * kAccStages;   // [kAccStages] (used in the leader CTA)
   const uint32_t tmem_slot = bars + 16 * kStages + 16 * kAccStages;   // uint32
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
-  const int num_m = (shape.M + BLOCK_M - 1) / BLOCK_M, num_n = (shape.N + BLOCK_N - 1) / BLOCK_N;
+  const uint32_t rank = cluster_ctarank();          // 0 = leader of the pair
+  const bool leader = rank == 0;
+  const int pair = blockIdx.x / 2, num_pairs = gridDim.x / 2;
+  const int num_m = (shape.M + PAIR_M - 1) / PAIR_M, num_n = (shape.N + BLOCK_N - 1) / BLOCK_N;
   const int num_tiles = num_m * num_n;
   const int num_kb = (shape.K + BLOCK_K - 1) / BLOCK_K;
 
@@ -277,12 +307,12 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
   }
   if (warp == 1 && lane == 0) {
     for (int i = 0; i < kStages; ++i) {
-      mbar_init(full_bar + 8 * i, 1);
-      mbar_init(empty_bar + 8 * i, 1);
+      mbar_init(full_bar + 8 * i, 1);                      // the leader's producer arrives (+ expect_tx of both CTAs' bytes)
+      mbar_init(empty_bar + 8 * i, 1);                     // one multicast tcgen05.commit
     }
     for (int i = 0; i < kAccStages; ++i) {
-      mbar_init(tfull_bar + 8 * i, 1);
-      mbar_init(tempty_bar + 8 * i, kNumEpiWarps);
+      mbar_init(tfull_bar + 8 * i, 1);                     // one multicast tcgen05.commit
+      mbar_init(tempty_bar + 8 * i, 2 * kNumEpiWarps);     // the epilogue warps of both CTAs
     }
     fence_barrier_init();
   }
@@ -291,24 +321,26 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
     tmem_relinquish();
   }
   tc_fence_before();
-  __syncthreads();
+  cluster_sync();            // both CTAs' barriers are initialised and TMEM is allocated before anyone proceeds
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
 
   if (warp == 0) {
-    // ================================================================== TMA producer
+    // ================================================================== TMA producer (both CTAs)
     int stage = 0;
     uint32_t phase = 0;
-    for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
+    for (int t = pair; t < num_tiles; t += num_pairs) {
       const TileCoord tc = tile_coord(t, num_m, num_n);
-      const int m0 = tc.m_blk * BLOCK_M, n0 = tc.n_blk * BLOCK_N;
+      const int m0 = tc.m_blk * PAIR_M + (int)rank * BLOCK_M;     // this CTA's rows of A
+      const int n0 = tc.n_blk * BLOCK_N + (int)rank * HALF_N;     // this CTA's half of the B tile
       for (int kb = 0; kb < num_kb; ++kb) {
         mbar_wait(empty_bar + 8 * stage, phase ^ 1);
         if (lane == 0) {
-          const uint32_t fb = full_bar + 8 * stage;
+          const uint32_t fb_local = full_bar + 8 * stage;
+          const uint32_t fb = mapa(fb_local, 0);     // the leader's barrier receives both CTAs' bytes
           const uint32_t sa = smem_a + stage * kAStageBytes, sb = smem_b + stage * kBStageBytes;
           const int k0 = kb * BLOCK_K;
-          mbar_expect_tx(fb, kStageBytes);
+          if (leader) mbar_expect_tx(fb_local, 2 * kStageBytes);
           if constexpr (A_MAJOR == MAJOR_K) {
             tma_load_2d(sa, &tmap_a, fb, k0, m0);
           } else {
@@ -319,52 +351,53 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
             tma_load_2d(sb, &tmap_b, fb, k0, n0);
           } else {
 #pragma unroll
-            for (int c = 0; c < BLOCK_N / 64; ++c) tma_load_2d(sb + c * (BLOCK_K * 128), &tmap_b, fb, n0 + 64 * c, k0);
+            for (int c = 0; c < HALF_N / 64; ++c) tma_load_2d(sb + c * (BLOCK_K * 128), &tmap_b, fb, n0 + 64 * c, k0);
           }
         }
         __syncwarp();
         if (++stage == kStages) { stage = 0; phase ^= 1; }
       }
     }
-  } else if (warp == 1) {
-    // ================================================================== MMA issuer
+  } else if (warp == 1 && leader) {
+    // ================================================================== MMA issuer (leader CTA only)
     constexpr uint32_t idesc = make_idesc<A_MAJOR, B_MAJOR>();
     int stage = 0;
     uint32_t phase = 0;
     int it = 0;
-    for (int t = blockIdx.x; t < num_tiles; t += gridDim.x, ++it) {
+    for (int t = pair; t < num_tiles; t += num_pairs, ++it) {
       const int as = it & 1;
       const uint32_t aphase = (it >> 1) & 1;
-      mbar_wait(tempty_bar + 8 * as, aphase ^ 1);   // epilogue has drained this accumulator stage
+      mbar_wait(tempty_bar + 8 * as, aphase ^ 1);   // both CTAs' epilogues have drained this accumulator stage
       tc_fence_after();
       const uint32_t tmem_d = tmem_base + as * BLOCK_N;
       for (int kb = 0; kb < num_kb; ++kb) {
-        mbar_wait(full_bar + 8 * stage, phase);      // TMA bytes have landed
+        mbar_wait(full_bar + 8 * stage, phase);      // both CTAs' TMA bytes have landed
         tc_fence_after();
         if (lane == 0) {
           const uint32_t sa = smem_a + stage * kAStageBytes, sb = smem_b + stage * kBStageBytes;
 #pragma unroll
           for (int k = 0; k < BLOCK_K / UMMA_K; ++k)
             umma_bf16(tmem_d, operand_desc<A_MAJOR>(sa, k), operand_desc<B_MAJOR>(sb, k), idesc, (kb | k) != 0);
-          umma_commit(empty_bar + 8 * stage);        // smem slot free once these MMAs have read it
-          if (kb == num_kb - 1) umma_commit(tfull_bar + 8 * as);   // accumulator complete
+          umma_commit(empty_bar + 8 * stage);        // smem slot free in both CTAs once these MMAs have read it
+          if (kb == num_kb - 1) umma_commit(tfull_bar + 8 * as);   // accumulator complete (both CTAs)
         }
         __syncwarp();
         if (++stage == kStages) { stage = 0; phase ^= 1; }
       }
     }
   } else if (warp >= kEpiWarp0) {
-    // ================================================================== epilogue
+    // ================================================================== epilogue (both CTAs, own 128 rows)
     using Tr = EpiTraits<EPI>;
     constexpr int kChunk = Tr::kChunkCols;
     const int q = warp % 4;   // TMEM lane quarter this warp may access
     StorePipe pipe{smem_store + q * (kStoreBufsPerWarp * kStoreBufBytes), 0u, lane};
+    const uint32_t tempty_leader = mapa(tempty_bar, 0);
     int it = 0;
-    for (int t = blockIdx.x; t < num_tiles; t += gridDim.x, ++it) {
+    for (int t = pair; t < num_tiles; t += num_pairs, ++it) {
       const TileCoord tc = tile_coord(t, num_m, num_n);
       const int as = it & 1;
       const uint32_t aphase = (it >> 1) & 1;
-      const int row0 = tc.m_blk * BLOCK_M + q * 32;     // first row of this warp's 32-row band
+      const int row0 = tc.m_blk * PAIR_M + (int)rank * BLOCK_M + q * 32;     // first row of this warp's 32-row band
       const int64_t row = row0 + lane;
       const bool row_ok = row < shape.M;
       const int n0 = tc.n_blk * BLOCK_N;
@@ -382,7 +415,7 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
         if (n + kChunk >= n_end) {   // last read of this accumulator stage: hand it back to the MMA warp early
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive(tempty_bar + 8 * as);
+          if (lane == 0) mbar_arrive_cluster(tempty_leader + 8 * as);
         }
         uint4 o[8];
         if constexpr (Tr::kF32Out) {
@@ -439,8 +472,9 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
     __syncwarp();
   }
 
+  // Neither CTA may exit (or free TMEM) while its peer can still signal its barriers or run UMMAs on its TMEM.
   tc_fence_before();
-  __syncthreads();
+  cluster_sync();
   if (warp == 2) {
     tc_fence_after();
     tmem_dealloc(tmem_base, kTmemCols);
@@ -483,7 +517,7 @@ inline int launch_gemm_bf16(const void* A, int64_t lda, const void* B, int64_t l
   if (A_MAJOR == MAJOR_K) rc = make_tmap(&ta, A, s.K, s.M, lda, BLOCK_K, BLOCK_M);
   else                    rc = make_tmap(&ta, A, s.M, s.K, lda, 64, BLOCK_K);
   if (rc != OSDP_OK) return rc;
-  if (B_MAJOR == MAJOR_K) rc = make_tmap(&tb, B, s.K, s.N, ldb, BLOCK_K, BLOCK_N);
+  if (B_MAJOR == MAJOR_K) rc = make_tmap(&tb, B, s.K, s.N, ldb, BLOCK_K, HALF_N);
   else                    rc = make_tmap(&tb, B, s.N, s.K, ldb, 64, BLOCK_K);
   if (rc != OSDP_OK) return rc;
   // outputs: [M x N] row-major, leading dimension ldo; one store = 32 rows x 128 bytes
@@ -502,14 +536,27 @@ inline int launch_gemm_bf16(const void* A, int64_t lda, const void* B, int64_t l
     OSDP_CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
     attr_set = true;
   }
-  const int num_m = (s.M + BLOCK_M - 1) / BLOCK_M, num_n = (s.N + BLOCK_N - 1) / BLOCK_N;
-  const int tiles = num_m * num_n;
-  const int sms = num_sms();
-  const int grid = tiles < sms ? tiles : sms;
+  const int num_m = (s.M + PAIR_M - 1) / PAIR_M, num_n = (s.N + BLOCK_N - 1) / BLOCK_N;
+  const int tiles = num_m * num_n;          // 256 x 256 pair tiles
+  const int pairs = num_sms() / 2;          // one CTA pair per TPC
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(2 * (tiles < pairs ? tiles : pairs));
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = kSmemBytes;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = 2;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  cudaError_t err;
   {
     LaunchTrace tr(st);
-    kernel<<<grid, kThreads, kSmemBytes, st>>>(ta, tb, to0, to1, s, ep);
+    err = cudaLaunchKernelEx(&cfg, kernel, ta, tb, to0, to1, s, ep);
   }
+  OSDP_CUDA_TRY(err);
   OSDP_CUDA_TRY(cudaGetLastError());
   return OSDP_OK;
 }
