@@ -40,7 +40,16 @@ constexpr int BLOCK_N = 256;       // columns per pair tile = UMMA N
 constexpr int HALF_N = BLOCK_N / 2;   // B columns staged by each CTA
 constexpr int BLOCK_K = 64;
 constexpr int UMMA_K = 16;
-constexpr int kStages = 6;
+#ifndef OSDP_STAGES
+#define OSDP_STAGES 6
+#endif
+#ifndef OSDP_GROUP_M
+#define OSDP_GROUP_M 8
+#endif
+#ifndef OSDP_WAIT_SLEEP_NS
+#define OSDP_WAIT_SLEEP_NS 0      // > 0: nanosleep between failed mbarrier polls of the long (epilogue) waits
+#endif
+constexpr int kStages = OSDP_STAGES;
 constexpr int kAccStages = 2;
 constexpr int kTmemCols = 512;
 constexpr int kThreads = 256;
@@ -54,7 +63,7 @@ constexpr uint32_t kStoreBufBytes = 32 * 128;              // one warp's 32 rows
 constexpr uint32_t kStoreBufsPerWarp = 2;
 constexpr uint32_t kSmemStore = kNumEpiWarps * kStoreBufsPerWarp * kStoreBufBytes;   // 32 KiB
 constexpr uint32_t kSmemBytes = kSmemTiles + kSmemStore + 1024 /*align slack*/ + 256 /*barriers*/;
-constexpr int kGroupM = 8;    // tile rasterisation: bands of 8 pair-tiles (2048 rows), n walks across the band
+constexpr int kGroupM = OSDP_GROUP_M;    // tile rasterisation: bands of 8 pair-tiles (2048 rows), n walks across the band
 
 // ---------------------------------------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -117,6 +126,24 @@ __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
 __device__ __forceinline__ void cluster_sync() {
   asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
   asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// Long waits (an epilogue warp waiting a whole main loop for its accumulator): optionally back off between polls.
+__device__ __forceinline__ void mbar_wait_long(uint32_t bar, uint32_t parity) {
+#if OSDP_WAIT_SLEEP_NS > 0
+  if (mbar_try_wait(bar, parity)) return;
+  uint64_t t0 = 0;
+  uint32_t spins = 0;
+  while (!mbar_try_wait(bar, parity)) {
+    __nanosleep(OSDP_WAIT_SLEEP_NS);
+    if ((++spins & 0xFFFu) == 0) {
+      const uint64_t now = global_timer_ns();
+      if (t0 == 0) t0 = now;
+      else if (now - t0 > 20ull * 1000 * 1000 * 1000) __trap();
+    }
+  }
+#else
+  mbar_wait(bar, parity);
+#endif
 }
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
@@ -401,7 +428,7 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
       const int64_t row = row0 + lane;
       const bool row_ok = row < shape.M;
       const int n0 = tc.n_blk * BLOCK_N;
-      mbar_wait(tfull_bar + 8 * as, aphase);
+      mbar_wait_long(tfull_bar + 8 * as, aphase);
       tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * BLOCK_N;
       const int n_end = min(n0 + BLOCK_N, shape.N);

@@ -167,3 +167,40 @@ def test_runs_on_a_side_stream(lib):
         Y = op.forward(d.X, d.W1, d.b1, d.W2, d.b2, stream=s)
     s.synchronize()
     assert rel_err(Y.double().cpu().numpy(), ref["Y"]) <= 2e-2
+
+
+@pytest.mark.parametrize("dtype,T,h,f,k", [(torch.bfloat16, 333, 136, 520, 3), (torch.bfloat16, 260, 72, 264, 2),
+                                           (torch.float32, 100, 36, 68, 4)])
+def test_no_out_of_bounds_writes_guard_bands(lib, dtype, T, h, f, k):
+    """compute-sanitizer is closed on this pool, so out-of-bounds stores are caught with guard bands: every
+    output and the workspace sit between 4 KiB bands of 0xA5 that must come back untouched (ragged shapes, so
+    partial tiles clip on every edge)."""
+    G = 4096
+    e = 2 if dtype == torch.bfloat16 else 4
+    desc = lib.make_desc(T, h, f, dtype, k)
+    sizes = {"Y": T * h * e, "dX": T * h * e, "dW1": h * f * 4, "db1": f * 4, "dW2": f * h * 4, "db2": h * 4,
+             "ws": lib.osdp_split_mlp_workspace_bytes(desc, lib.OSDP_BWD)}
+    offs, total = {}, G
+    for n, sz in sizes.items():
+        offs[n] = total
+        total += (sz + 255) // 256 * 256 + G
+    arena = torch.full((total,), 0xA5, dtype=torch.uint8, device="cuda")
+    view = lambda n, dt, shape: arena[offs[n]: offs[n] + sizes[n]].view(dt).view(*shape)
+    inp = I.mlp_inputs(T, h, f, dtype, seed=5)
+    ref = O.mlp_forward_backward(**inp.as_f64())
+    d = inp.to("cuda")
+    Y, dX = view("Y", dtype, (T, h)), view("dX", dtype, (T, h))
+    dW1, db1 = view("dW1", torch.float32, (h, f)), view("db1", torch.float32, (f,))
+    dW2, db2 = view("dW2", torch.float32, (f, h)), view("db2", torch.float32, (h,))
+    ws = arena[offs["ws"]: offs["ws"] + sizes["ws"]]
+    lib.osdp_split_mlp_forward(desc, d.X, d.W1, d.b1, d.W2, d.b2, Y, ws)
+    lib.osdp_split_mlp_backward(desc, d.X, d.W1, d.b1, d.W2, d.b2, d.dY, dX, dW1, db1, dW2, db2, ws)
+    torch.cuda.synchronize()
+    mask = torch.ones(total, dtype=torch.bool, device="cuda")
+    for n, sz in sizes.items():
+        mask[offs[n]: offs[n] + sz] = False
+    assert bool((arena[mask] == 0xA5).all()), "a kernel wrote outside its output/workspace"
+    got = dict(Y=Y, dX=dX, dW1=dW1, db1=db1, dW2=dW2, db2=db2)
+    tol = TOL[dtype]
+    for n in NAMES:
+        assert rel_err(got[n].double().cpu().numpy(), ref[n]) <= tol, n
