@@ -34,36 +34,57 @@
 namespace osdp {
 namespace sm100 {
 
-constexpr int BLOCK_M = 128;       // rows per CTA (TMEM lanes)
-constexpr int PAIR_M = 2 * BLOCK_M;   // rows per CTA pair = UMMA M
+constexpr int BLOCK_M = 128;       // rows per UMMA per CTA (TMEM lanes)
+constexpr int UMMA_M = 2 * BLOCK_M;   // UMMA M of a CTA pair (cta_group::2)
 constexpr int BLOCK_N = 256;       // columns per pair tile = UMMA N
 constexpr int HALF_N = BLOCK_N / 2;   // B columns staged by each CTA
 constexpr int BLOCK_K = 64;
 constexpr int UMMA_K = 16;
-#ifndef OSDP_STAGES
-#define OSDP_STAGES 6
-#endif
-#ifndef OSDP_GROUP_M
-#define OSDP_GROUP_M 8
+#ifndef OSDP_BAND_MIB
+#define OSDP_BAND_MIB 32          // L2 budget for the A rows of one raster band (see launch_gemm_bf16_cluster)
 #endif
 #ifndef OSDP_WAIT_SLEEP_NS
 #define OSDP_WAIT_SLEEP_NS 0      // > 0: nanosleep between failed mbarrier polls of the long (epilogue) waits
 #endif
-constexpr int kStages = OSDP_STAGES;
-constexpr int kAccStages = 2;
 constexpr int kTmemCols = 512;
 constexpr int kThreads = 256;
 constexpr int kEpiWarp0 = 4;
 constexpr int kNumEpiWarps = 4;
-constexpr uint32_t kAStageBytes = BLOCK_M * BLOCK_K * 2;   // 16 KiB
 constexpr uint32_t kBStageBytes = HALF_N * BLOCK_K * 2;    // 16 KiB (this CTA's half of the B tile)
-constexpr uint32_t kStageBytes = kAStageBytes + kBStageBytes;   // per CTA; the leader's barrier expects 2x
-constexpr uint32_t kSmemTiles = kStages * kStageBytes;     // 192 KiB
 constexpr uint32_t kStoreBufBytes = 32 * 128;              // one warp's 32 rows x 128 B output segment
 constexpr uint32_t kStoreBufsPerWarp = 2;
 constexpr uint32_t kSmemStore = kNumEpiWarps * kStoreBufsPerWarp * kStoreBufBytes;   // 32 KiB
-constexpr uint32_t kSmemBytes = kSmemTiles + kSmemStore + 1024 /*align slack*/ + 256 /*barriers*/;
-constexpr int kGroupM = OSDP_GROUP_M;    // tile rasterisation: bands of 8 pair-tiles (2048 rows), n walks across the band
+
+// Two tile shapes share the kernel.  MT = M-halves (UMMAs of 128 rows) per CTA:
+//   MT = 1: CTA 128 x 256, pair 256 x 256; TMEM holds TWO accumulator stages, so the epilogue of tile i overlaps
+//           the main loop of tile i + 1; 6 smem stages of 32 KiB; 64 KiB of operands per 8.4 MFLOP k-block.
+//   MT = 2: CTA 256 x 256, pair 512 x 256; the accumulator fills all 512 TMEM columns (one stage, epilogue
+//           exposed); 4 smem stages of 48 KiB; 96 KiB of operands per 16.8 MFLOP k-block, i.e. 25 % less
+//           L2 -> SM -> smem traffic per flop.  Large GEMMs run power-limited, where that traffic is what
+//           decides the clock, so long-K GEMMs take MT = 2.
+template <int MT>
+struct TileCfg {
+  static constexpr int kCtaM = MT * BLOCK_M;       // rows per CTA
+  static constexpr int kPairM = 2 * kCtaM;         // rows per pair tile
+  static constexpr int kStages = MT == 1 ? 6 : 4;
+  static constexpr int kAccStages = 2 / MT;
+  static constexpr uint32_t kAStageBytes = kCtaM * BLOCK_K * 2;          // 16 / 32 KiB
+  static constexpr uint32_t kStageBytes = kAStageBytes + kBStageBytes;   // per CTA; the leader's barrier expects 2x
+  static constexpr uint32_t kSmemTiles = kStages * kStageBytes;          // 192 KiB
+  static constexpr uint32_t kSmemBytes = kSmemTiles + kSmemStore + 1024 /*align slack*/ + 256 /*barriers*/;
+};
+
+// L2 cache-hint descriptors (what createpolicy.fractional.L2::evict_*.b64 with fraction 1.0 produces).
+constexpr uint64_t kEvictNormal = 0x1000000000000000ull;
+constexpr uint64_t kEvictFirst = 0x12F0000000000000ull;
+constexpr uint64_t kEvictLast = 0x14F0000000000000ull;
+#ifndef OSDP_HINT_A
+#define OSDP_HINT_A 0     // 0 normal, 1 evict_first, 2 evict_last (both hints measured worse: DESIGN.md section 7)
+#endif
+#ifndef OSDP_HINT_B
+#define OSDP_HINT_B 0
+#endif
+__host__ __device__ constexpr uint64_t hint_policy(int h) { return h == 1 ? kEvictFirst : h == 2 ? kEvictLast : kEvictNormal; }
 
 // ---------------------------------------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -148,10 +169,23 @@ __device__ __forceinline__ void mbar_wait_long(uint32_t bar, uint32_t parity) {
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
 // dst: this CTA's smem; bar: shared::cluster address of the mbarrier that receives complete_tx (the leader's).
-__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c_inner, int c_outer) {
+// policy: an L2 cache-hint descriptor (kEvictFirst / kEvictNormal / kEvictLast below).
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c_inner, int c_outer,
+                                            uint64_t policy) {
   asm volatile(
-      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
-      ::"r"(dst), "l"((uint64_t)map), "r"(bar), "r"(c_inner), "r"(c_outer)
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint "
+      "[%0], [%1, {%3, %4}], [%2], %5;"
+      ::"r"(dst), "l"((uint64_t)map), "r"(bar), "r"(c_inner), "r"(c_outer), "l"(policy)
+      : "memory");
+}
+// Same, delivered to the same smem offset of every CTA in `mask` (cluster ranks); each destination's bytes are
+// signalled on the barrier at `bar`'s offset in the leader of that destination's pair.
+__device__ __forceinline__ void tma_load_2d_mc(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c_inner, int c_outer,
+                                               uint16_t mask, uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster.L2::cache_hint "
+      "[%0], [%1, {%3, %4}], [%2], %5, %6;"
+      ::"r"(dst), "l"((uint64_t)map), "r"(bar), "r"(c_inner), "r"(c_outer), "h"(mask), "l"(policy)
       : "memory");
 }
 // smem -> global tile store / fp32 reduce-add (bulk async-group completion).
@@ -200,11 +234,11 @@ __device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t adesc, uint6
       "}\n" ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
       : "memory");
 }
-// Arrive on the mbarrier at this smem offset in BOTH CTAs of the pair when all tcgen05.mma issued so far by this
-// thread have completed (implies tcgen05.fence::before_thread_sync).
-__device__ __forceinline__ void umma_commit(uint32_t bar) {
+// Arrive on the mbarrier at this smem offset in every CTA of `mask` (cluster ranks) when all tcgen05.mma issued so
+// far by this thread have completed (implies tcgen05.fence::before_thread_sync).
+__device__ __forceinline__ void umma_commit(uint32_t bar, uint16_t mask) {
   asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
-               ::"r"(bar), "h"((uint16_t)3)
+               ::"r"(bar), "h"(mask)
                : "memory");
 }
 
@@ -245,7 +279,7 @@ __device__ __forceinline__ uint64_t operand_desc(uint32_t tile_addr, int k16) {
 template <int A_MAJOR, int B_MAJOR>
 __host__ __device__ constexpr uint32_t make_idesc() {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)A_MAJOR << 15) | ((uint32_t)B_MAJOR << 16) |
-         ((uint32_t)(BLOCK_N >> 3) << 17) | ((uint32_t)(PAIR_M >> 4) << 24);
+         ((uint32_t)(BLOCK_N >> 3) << 17) | ((uint32_t)(UMMA_M >> 4) << 24);
 }
 
 // --------------------------------------------------------------------------------------------------- epilogue
@@ -289,41 +323,57 @@ struct StorePipe {
 
 // ------------------------------------------------------------------------------------------------- the kernel
 struct TileCoord {
-  int m_blk, n_blk;   // pair-tile coordinates: rows m_blk * 256, columns n_blk * 256
+  int m_blk, n_blk;   // cluster-tile coordinates: rows m_blk * CM * 256, columns n_blk * CN * 256
 };
-__device__ __forceinline__ TileCoord tile_coord(int t, int num_m, int num_n) {
-  const int per_group = kGroupM * num_n;
+__device__ __forceinline__ TileCoord tile_coord(int t, int num_m, int num_n, int group_m) {
+  const int per_group = group_m * num_n;
   const int g = t / per_group;
-  const int first_m = g * kGroupM;
-  const int gsize = min(kGroupM, num_m - first_m);
+  const int first_m = g * group_m;
+  const int gsize = min(group_m, num_m - first_m);
   const int local = t - g * per_group;
   return {first_m + local % gsize, local / gsize};
 }
 
-template <int A_MAJOR, int B_MAJOR, int EPI>
+// CM x CN CTA pairs form one cluster (2 * CM * CN CTAs) and compute a (CM * 256) x (CN * 256) block of C.  Pairs in
+// the same cluster row need the same A rows, pairs in the same cluster column the same B columns: each CTA fetches
+// 1/CN of its A tile and 1/CM of its B half-tile and TMA-multicasts it to the CTAs that share it, so L2 -> SM
+// traffic per flop falls by (1/CN + 1/CM) / 2.  CM = CN = 1 is the plain pair kernel.
+template <int A_MAJOR, int B_MAJOR, int EPI, int MT, int CM, int CN>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
                        const __grid_constant__ CUtensorMap tmap_out0, const __grid_constant__ CUtensorMap tmap_out1,
-                       const GemmShape shape, const EpiParams ep) {
+                       const GemmShape shape, const EpiParams ep, const int group_m) {
+  using Cfg = TileCfg<MT>;
+  constexpr int kStages = Cfg::kStages, kAccStages = Cfg::kAccStages;
+  constexpr int kCtaM = Cfg::kCtaM, kPairM = Cfg::kPairM;
+  constexpr uint32_t kAStageBytes = Cfg::kAStageBytes, kStageBytes = Cfg::kStageBytes, kSmemTiles = Cfg::kSmemTiles;
+  constexpr int kPairs = CM * CN;
+  constexpr int kCluster = 2 * kPairs;
+  static_assert(CM == 1 || CM == 2, "CM");
+  static_assert(CN == 1 || CN == 2, "CN");
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;   // 128B swizzle atoms need 1024 B alignment
   const uint32_t smem_a = smem_base;
   const uint32_t smem_b = smem_base + kStages * kAStageBytes;
   const uint32_t smem_store = smem_base + kSmemTiles;
   const uint32_t bars = smem_store + kSmemStore;
-  const uint32_t full_bar = bars;                                  // [kStages]   (used in the leader CTA)
+  const uint32_t full_bar = bars;                                  // [kStages]   (used in each pair's leader CTA)
   const uint32_t empty_bar = bars + 8 * kStages;                   // [kStages]   (one per CTA, multicast arrive)
   const uint32_t tfull_bar = bars + 16 * kStages;                  // [kAccStages] (one per CTA, multicast arrive)
-  const uint32_t tempty_bar = bars + 16 * kStages + 8 * kAccStages;   // [kAccStages] (used in the leader CTA)
+  const uint32_t tempty_bar = bars + 16 * kStages + 8 * kAccStages;   // [kAccStages] (used in each pair's leader CTA)
   const uint32_t tmem_slot = bars + 16 * kStages + 16 * kAccStages;   // uint32
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
-  const uint32_t rank = cluster_ctarank();          // 0 = leader of the pair
+  const uint32_t crank = cluster_ctarank();
+  const uint32_t rank = crank & 1u;                 // 0 = leader of its pair
   const bool leader = rank == 0;
-  const int pair = blockIdx.x / 2, num_pairs = gridDim.x / 2;
-  const int num_m = (shape.M + PAIR_M - 1) / PAIR_M, num_n = (shape.N + BLOCK_N - 1) / BLOCK_N;
-  const int num_tiles = num_m * num_n;
+  const uint32_t leader_crank = crank & ~1u;
+  const int pi = (int)(crank >> 1) / CN, pj = (int)(crank >> 1) % CN;   // this pair's position in the cluster
+  const int cluster_id = blockIdx.x / kCluster, num_clusters = gridDim.x / kCluster;
+  const int num_m = (shape.M + kPairM - 1) / kPairM, num_n = (shape.N + BLOCK_N - 1) / BLOCK_N;   // pair tiles
+  const int num_cm = (num_m + CM - 1) / CM, num_cn = (num_n + CN - 1) / CN;                         // cluster tiles
+  const int num_tiles = num_cm * num_cn;
   const int num_kb = (shape.K + BLOCK_K - 1) / BLOCK_K;
 
   if (warp == 0 && lane == 0) {
@@ -335,7 +385,7 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
   if (warp == 1 && lane == 0) {
     for (int i = 0; i < kStages; ++i) {
       mbar_init(full_bar + 8 * i, 1);                      // the leader's producer arrives (+ expect_tx of both CTAs' bytes)
-      mbar_init(empty_bar + 8 * i, 1);                     // one multicast tcgen05.commit
+      mbar_init(empty_bar + 8 * i, kPairs);                // one multicast tcgen05.commit per pair of the cluster
     }
     for (int i = 0; i < kAccStages; ++i) {
       mbar_init(tfull_bar + 8 * i, 1);                     // one multicast tcgen05.commit
@@ -348,37 +398,89 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
     tmem_relinquish();
   }
   tc_fence_before();
-  cluster_sync();            // both CTAs' barriers are initialised and TMEM is allocated before anyone proceeds
+  cluster_sync();            // every CTA's barriers are initialised and TMEM is allocated before anyone proceeds
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
 
   if (warp == 0) {
-    // ================================================================== TMA producer (both CTAs)
+    // ================================================================== TMA producer (every CTA)
+    // multicast destinations: the CTAs of equal pair-rank in this cluster row (A) / cluster column (B)
+    uint16_t mask_a = 0, mask_b = 0;
+#pragma unroll
+    for (int j = 0; j < CN; ++j) mask_a |= (uint16_t)(1u << (2 * (pi * CN + j) + (int)rank));
+#pragma unroll
+    for (int i = 0; i < CM; ++i) mask_b |= (uint16_t)(1u << (2 * (i * CN + pj) + (int)rank));
+    // Tiles walk along n inside a band of group_m cluster-tile rows: the band's A rows are re-used by every wave
+    // of the band (keep them in L2), B streams through once per band (let it go first).
+    constexpr uint64_t pol_a = hint_policy(OSDP_HINT_A), pol_b = hint_policy(OSDP_HINT_B);
+    constexpr int kARows = kCtaM / CN;     // A rows (K-major) this CTA fetches; it is part pj of the tile
+    constexpr int kBRows = HALF_N / CM;    // B columns this CTA fetches; it is part pi of the half-tile
     int stage = 0;
     uint32_t phase = 0;
-    for (int t = pair; t < num_tiles; t += num_pairs) {
-      const TileCoord tc = tile_coord(t, num_m, num_n);
-      const int m0 = tc.m_blk * PAIR_M + (int)rank * BLOCK_M;     // this CTA's rows of A
-      const int n0 = tc.n_blk * BLOCK_N + (int)rank * HALF_N;     // this CTA's half of the B tile
+#ifdef OSDP_DBG_NOLOAD
+    int dbg_filled = 0;
+#endif
+    for (int t = cluster_id; t < num_tiles; t += num_clusters) {
+      const TileCoord tc = tile_coord(t, num_cm, num_cn, group_m);
+      int m0 = (tc.m_blk * CM + pi) * kPairM + (int)rank * kCtaM;       // this CTA's rows of A
+      int n0 = (tc.n_blk * CN + pj) * BLOCK_N + (int)rank * HALF_N;     // this CTA's half of the B tile
+#ifdef OSDP_DBG_PRIVTILE   // probe: every pair re-reads its own private operand tiles (all L2 hits, nothing shared)
+      m0 = (cluster_id * kPairM) % (num_m * kPairM) + (int)rank * kCtaM;
+      n0 = (cluster_id * BLOCK_N) % (num_n * BLOCK_N) + (int)rank * HALF_N;
+#endif
+#ifdef OSDP_DBG_SAMETILE   // probe: every pair re-reads tile (0, 0)
+      m0 = (int)rank * kCtaM;
+      n0 = (int)rank * HALF_N;
+#endif
       for (int kb = 0; kb < num_kb; ++kb) {
-        mbar_wait(empty_bar + 8 * stage, phase ^ 1);
+        mbar_wait(empty_bar + 8 * stage, phase ^ 1);   // the slot is free in every CTA of the cluster
+#ifdef OSDP_DBG_NOLOAD   // probe: after the ring has been filled once, re-use its contents (no L2->SM traffic)
+        if (dbg_filled >= kStages) {
+          if (lane == 0 && leader) mbar_arrive(full_bar + 8 * stage);
+          __syncwarp();
+          if (++stage == kStages) { stage = 0; phase ^= 1; }
+          continue;
+        }
+        ++dbg_filled;
+#endif
         if (lane == 0) {
           const uint32_t fb_local = full_bar + 8 * stage;
-          const uint32_t fb = mapa(fb_local, 0);     // the leader's barrier receives both CTAs' bytes
+          const uint32_t fb = mapa(fb_local, leader_crank);     // the pair leader's barrier receives both CTAs' bytes
           const uint32_t sa = smem_a + stage * kAStageBytes, sb = smem_b + stage * kBStageBytes;
+#ifdef OSDP_DBG_KWRAP
+          const int k0 = (kb % OSDP_DBG_KWRAP) * BLOCK_K;
+#else
           const int k0 = kb * BLOCK_K;
+#endif
           if (leader) mbar_expect_tx(fb_local, 2 * kStageBytes);
-          if constexpr (A_MAJOR == MAJOR_K) {
-            tma_load_2d(sa, &tmap_a, fb, k0, m0);
-          } else {
+          if constexpr (kPairs == 1) {
+            if constexpr (A_MAJOR == MAJOR_K) {
+              tma_load_2d(sa, &tmap_a, fb, k0, m0, pol_a);
+            } else {
 #pragma unroll
-            for (int c = 0; c < BLOCK_M / 64; ++c) tma_load_2d(sa + c * (BLOCK_K * 128), &tmap_a, fb, m0 + 64 * c, k0);
-          }
-          if constexpr (B_MAJOR == MAJOR_K) {
-            tma_load_2d(sb, &tmap_b, fb, k0, n0);
-          } else {
+              for (int c = 0; c < kCtaM / 64; ++c) tma_load_2d(sa + c * (BLOCK_K * 128), &tmap_a, fb, m0 + 64 * c, k0, pol_a);
+            }
+            if constexpr (B_MAJOR == MAJOR_K) {
+              tma_load_2d(sb, &tmap_b, fb, k0, n0, pol_b);
+            } else {
 #pragma unroll
-            for (int c = 0; c < HALF_N / 64; ++c) tma_load_2d(sb + c * (BLOCK_K * 128), &tmap_b, fb, n0 + 64 * c, k0);
+              for (int c = 0; c < HALF_N / 64; ++c) tma_load_2d(sb + c * (BLOCK_K * 128), &tmap_b, fb, n0 + 64 * c, k0, pol_b);
+            }
+          } else {
+            if constexpr (A_MAJOR == MAJOR_K) {
+              tma_load_2d_mc(sa + pj * (kARows * 128), &tmap_a, fb, k0, m0 + pj * kARows, mask_a, pol_a);
+            } else {
+#pragma unroll
+              for (int c = pj * (kARows / 64); c < (pj + 1) * (kARows / 64); ++c)
+                tma_load_2d_mc(sa + c * (BLOCK_K * 128), &tmap_a, fb, m0 + 64 * c, k0, mask_a, pol_a);
+            }
+            if constexpr (B_MAJOR == MAJOR_K) {
+              tma_load_2d_mc(sb + pi * (kBRows * 128), &tmap_b, fb, k0, n0 + pi * kBRows, mask_b, pol_b);
+            } else {
+#pragma unroll
+              for (int c = pi * (kBRows / 64); c < (pi + 1) * (kBRows / 64); ++c)
+                tma_load_2d_mc(sb + c * (BLOCK_K * 128), &tmap_b, fb, n0 + 64 * c, k0, mask_b, pol_b);
+            }
           }
         }
         __syncwarp();
@@ -386,52 +488,72 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
       }
     }
   } else if (warp == 1 && leader) {
-    // ================================================================== MMA issuer (leader CTA only)
+    // ================================================================== MMA issuer (each pair's leader CTA)
     constexpr uint32_t idesc = make_idesc<A_MAJOR, B_MAJOR>();
+    constexpr uint16_t mask_cluster = (uint16_t)((1u << kCluster) - 1u);
+    const uint16_t mask_pair = (uint16_t)(3u << leader_crank);
     int stage = 0;
     uint32_t phase = 0;
     int it = 0;
-    for (int t = pair; t < num_tiles; t += num_pairs, ++it) {
-      const int as = it & 1;
-      const uint32_t aphase = (it >> 1) & 1;
+    for (int t = cluster_id; t < num_tiles; t += num_clusters, ++it) {
+      const TileCoord tc = tile_coord(t, num_cm, num_cn, group_m);
+      // a pair whose tile lies outside C (odd tile counts) still takes part in the loads, but skips the math
+      const bool valid = (tc.m_blk * CM + pi) < num_m && (tc.n_blk * CN + pj) < num_n;
+      const int as = it % kAccStages;
+      const uint32_t aphase = (it / kAccStages) & 1;
       mbar_wait(tempty_bar + 8 * as, aphase ^ 1);   // both CTAs' epilogues have drained this accumulator stage
       tc_fence_after();
-      const uint32_t tmem_d = tmem_base + as * BLOCK_N;
+      const uint32_t tmem_d = tmem_base + as * (MT * BLOCK_N);   // M-half h accumulates in columns [256 h, 256 h + 256)
       for (int kb = 0; kb < num_kb; ++kb) {
         mbar_wait(full_bar + 8 * stage, phase);      // both CTAs' TMA bytes have landed
         tc_fence_after();
         if (lane == 0) {
           const uint32_t sa = smem_a + stage * kAStageBytes, sb = smem_b + stage * kBStageBytes;
+          if (valid) {
 #pragma unroll
-          for (int k = 0; k < BLOCK_K / UMMA_K; ++k)
-            umma_bf16(tmem_d, operand_desc<A_MAJOR>(sa, k), operand_desc<B_MAJOR>(sb, k), idesc, (kb | k) != 0);
-          umma_commit(empty_bar + 8 * stage);        // smem slot free in both CTAs once these MMAs have read it
-          if (kb == num_kb - 1) umma_commit(tfull_bar + 8 * as);   // accumulator complete (both CTAs)
+            for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
+              const uint64_t bdesc = operand_desc<B_MAJOR>(sb, k);
+#pragma unroll
+              for (int h = 0; h < MT; ++h)
+                umma_bf16(tmem_d + h * BLOCK_N, operand_desc<A_MAJOR>(sa + h * (BLOCK_M * BLOCK_K * 2), k), bdesc, idesc,
+                          (kb | k) != 0);
+            }
+          }
+          umma_commit(empty_bar + 8 * stage, mask_cluster);   // slot free (for this pair) in every CTA that may refill it
+          if (kb == num_kb - 1) umma_commit(tfull_bar + 8 * as, mask_pair);   // accumulator complete (both CTAs)
         }
         __syncwarp();
         if (++stage == kStages) { stage = 0; phase ^= 1; }
       }
     }
   } else if (warp >= kEpiWarp0) {
-    // ================================================================== epilogue (both CTAs, own 128 rows)
+    // ================================================================== epilogue (both CTAs, own rows)
     using Tr = EpiTraits<EPI>;
     constexpr int kChunk = Tr::kChunkCols;
     const int q = warp % 4;   // TMEM lane quarter this warp may access
     StorePipe pipe{smem_store + q * (kStoreBufsPerWarp * kStoreBufBytes), 0u, lane};
-    const uint32_t tempty_leader = mapa(tempty_bar, 0);
+    const uint32_t tempty_leader = mapa(tempty_bar, leader_crank);
     int it = 0;
-    for (int t = pair; t < num_tiles; t += num_pairs, ++it) {
-      const TileCoord tc = tile_coord(t, num_m, num_n);
-      const int as = it & 1;
-      const uint32_t aphase = (it >> 1) & 1;
-      const int row0 = tc.m_blk * PAIR_M + (int)rank * BLOCK_M + q * 32;     // first row of this warp's 32-row band
-      const int64_t row = row0 + lane;
-      const bool row_ok = row < shape.M;
-      const int n0 = tc.n_blk * BLOCK_N;
+    for (int t = cluster_id; t < num_tiles; t += num_clusters, ++it) {
+      const TileCoord tc = tile_coord(t, num_cm, num_cn, group_m);
+      const int as = it % kAccStages;
+      const uint32_t aphase = (it / kAccStages) & 1;
+      const int n0 = (tc.n_blk * CN + pj) * BLOCK_N;
+      const int n_end = min(n0 + BLOCK_N, shape.N);
       mbar_wait_long(tfull_bar + 8 * as, aphase);
       tc_fence_after();
-      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * BLOCK_N;
-      const int n_end = min(n0 + BLOCK_N, shape.N);
+      bool released = false;   // the accumulator stage goes back to the MMA warp right after its last tcgen05.ld
+#pragma unroll 1
+      for (int h = 0; h < MT; ++h) {
+      const int row0 = (tc.m_blk * CM + pi) * kPairM + (int)rank * kCtaM + h * BLOCK_M + q * 32;   // this warp's 32-row band
+      const int64_t row = row0 + lane;
+      const bool row_ok = row < shape.M;
+      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * (MT * BLOCK_N) + h * BLOCK_N;
+      bool skip = row0 >= shape.M || n0 >= shape.N;   // nothing of this warp's band lies inside C (warp-uniform)
+#ifdef OSDP_DBG_NOEPI   // probe: drain nothing, hand the accumulator straight back (no tcgen05.ld, no stores)
+      skip = true;
+#endif
+      if (skip) continue;
 #pragma unroll 1
       for (int n = n0; n < n_end; n += kChunk) {
         uint32_t acc[kChunk];
@@ -439,10 +561,11 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
         for (int i = 0; i < kChunk / 32; ++i)
           tmem_ld_32x32(taddr + (n - n0) + 32 * i, *reinterpret_cast<uint32_t(*)[32]>(&acc[32 * i]));
         tmem_ld_wait();
-        if (n + kChunk >= n_end) {   // last read of this accumulator stage: hand it back to the MMA warp early
+        if (h == MT - 1 && n + kChunk >= n_end) {   // last read of this accumulator stage
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive_cluster(tempty_leader + 8 * as);
+          released = true;
         }
         uint4 o[8];
         if constexpr (Tr::kF32Out) {
@@ -494,12 +617,18 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
           }
         }
       }
+      }   // h
+      if (!released) {
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(tempty_leader + 8 * as);
+      }
     }
     if (lane == 0) bulk_wait<0>();   // all of this warp's stores have completed before the CTA's smem goes away
     __syncwarp();
   }
 
-  // Neither CTA may exit (or free TMEM) while its peer can still signal its barriers or run UMMAs on its TMEM.
+  // No CTA may exit (or free TMEM) while a peer can still signal its barriers, write its smem or run UMMAs on its TMEM.
   tc_fence_before();
   cluster_sync();
   if (warp == 2) {
@@ -536,15 +665,17 @@ inline int make_tmap(CUtensorMap* map, const void* ptr, int64_t inner, int64_t o
 }
 
 // A, B: bf16 device pointers stored as common.cuh describes for the given majorness.
-template <int A_MAJOR, int B_MAJOR, int EPI>
-inline int launch_gemm_bf16(const void* A, int64_t lda, const void* B, int64_t ldb, const GemmShape& s,
-                            const EpiParams& ep, cudaStream_t st) {
+template <int A_MAJOR, int B_MAJOR, int EPI, int MT, int CM, int CN>
+inline int launch_gemm_bf16_cluster(const void* A, int64_t lda, const void* B, int64_t ldb, const GemmShape& s,
+                                    const EpiParams& ep, cudaStream_t st) {
+  using Cfg = TileCfg<MT>;
   CUtensorMap ta, tb, to0, to1;
   int rc;
-  if (A_MAJOR == MAJOR_K) rc = make_tmap(&ta, A, s.K, s.M, lda, BLOCK_K, BLOCK_M);
+  // one TMA box = what ONE CTA fetches per k-block: 1/CN of its A rows, 1/CM of its B half (MN-major: 64-wide boxes)
+  if (A_MAJOR == MAJOR_K) rc = make_tmap(&ta, A, s.K, s.M, lda, BLOCK_K, Cfg::kCtaM / CN);
   else                    rc = make_tmap(&ta, A, s.M, s.K, lda, 64, BLOCK_K);
   if (rc != OSDP_OK) return rc;
-  if (B_MAJOR == MAJOR_K) rc = make_tmap(&tb, B, s.K, s.N, ldb, BLOCK_K, HALF_N);
+  if (B_MAJOR == MAJOR_K) rc = make_tmap(&tb, B, s.K, s.N, ldb, BLOCK_K, HALF_N / CM);
   else                    rc = make_tmap(&tb, B, s.N, s.K, ldb, 64, BLOCK_K);
   if (rc != OSDP_OK) return rc;
   // outputs: [M x N] row-major, leading dimension ldo; one store = 32 rows x 128 bytes
@@ -557,35 +688,89 @@ inline int launch_gemm_bf16(const void* A, int64_t lda, const void* B, int64_t l
     if (rc != OSDP_OK) return rc;
   }
 
-  auto kernel = gemm_bf16_sm100_kernel<A_MAJOR, B_MAJOR, EPI>;
-  static bool attr_set = false;   // one process per GPU: the attribute is per function per device
-  if (!attr_set) {
-    OSDP_CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
-    attr_set = true;
-  }
-  const int num_m = (s.M + PAIR_M - 1) / PAIR_M, num_n = (s.N + BLOCK_N - 1) / BLOCK_N;
-  const int tiles = num_m * num_n;          // 256 x 256 pair tiles
-  const int pairs = num_sms() / 2;          // one CTA pair per TPC
+  constexpr int kCluster = 2 * CM * CN;
+  auto kernel = gemm_bf16_sm100_kernel<A_MAJOR, B_MAJOR, EPI, MT, CM, CN>;
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(2 * (tiles < pairs ? tiles : pairs));
   cfg.blockDim = dim3(kThreads);
-  cfg.dynamicSmemBytes = kSmemBytes;
+  cfg.dynamicSmemBytes = Cfg::kSmemBytes;
   cfg.stream = st;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;
-  attr[0].val.clusterDim.x = 2;
+  attr[0].val.clusterDim.x = kCluster;
   attr[0].val.clusterDim.y = 1;
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
+  static int max_clusters = 0;   // one process per GPU: attribute and occupancy are per function per device
+  if (max_clusters == 0) {
+    OSDP_CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmemBytes));
+    int n = 0;
+    cfg.gridDim = dim3(kCluster * 64);
+    if (kCluster == 2) n = num_sms() / 2;   // one CTA pair per TPC
+    else OSDP_CUDA_TRY(cudaOccupancyMaxActiveClusters(&n, kernel, &cfg));
+    if (n < 1) {
+      note_cuda_error(cudaErrorInvalidConfiguration, "cudaOccupancyMaxActiveClusters");
+      return OSDP_ERR_CUDA;
+    }
+    max_clusters = n;
+  }
+  const int num_m = (s.M + Cfg::kPairM - 1) / Cfg::kPairM, num_n = (s.N + BLOCK_N - 1) / BLOCK_N;   // pair tiles
+  const int tiles = ((num_m + CM - 1) / CM) * ((num_n + CN - 1) / CN);                      // cluster tiles
+  cfg.gridDim = dim3(kCluster * (tiles < max_clusters ? tiles : max_clusters));
+  // Raster band: as many cluster-tile rows as keep the band's A rows (band rows x K bf16) inside the L2 budget;
+  // DRAM reads are about |A| + |B| * (row bands), so taller is better while A stays resident.
+#ifdef OSDP_GROUP_M
+  int group_m = OSDP_GROUP_M / (CM * MT);
+#else
+  const int64_t row_bytes = (int64_t)CM * Cfg::kPairM * s.K * 2;
+  int group_m = (int)(((int64_t)OSDP_BAND_MIB << 20) / row_bytes);
+#endif
+  if (group_m < 1) group_m = 1;
   cudaError_t err;
   {
     LaunchTrace tr(st);
-    err = cudaLaunchKernelEx(&cfg, kernel, ta, tb, to0, to1, s, ep);
+    err = cudaLaunchKernelEx(&cfg, kernel, ta, tb, to0, to1, s, ep, group_m);
   }
   OSDP_CUDA_TRY(err);
   OSDP_CUDA_TRY(cudaGetLastError());
   return OSDP_OK;
+}
+
+// Tile shape and cluster shape per launch.
+//  * MT = 2 (512 x 256 pair tiles, 25 % less operand traffic, exposed epilogue) for long contractions, where the
+//    main loop of a tile dwarfs its epilogue; MT = 1 (256 x 256, overlapped epilogue) otherwise.
+//  * Multicast clusters (CM x CN pairs) are compiled only on request (-DOSDP_CM / -DOSDP_CN): clusters of more than
+//    2 CTAs can use at most 132 of the 148 SMs, which costs more than the saved L2 -> SM traffic returns.
+#ifndef OSDP_CM
+#define OSDP_CM 1
+#endif
+#ifndef OSDP_CN
+#define OSDP_CN 1
+#endif
+#ifndef OSDP_CLUSTER_MIN_TILES
+#define OSDP_CLUSTER_MIN_TILES 148
+#endif
+#ifndef OSDP_MT2_MIN_K
+#define OSDP_MT2_MIN_K 4096
+#endif
+#ifndef OSDP_MT2_MIN_TILES
+#define OSDP_MT2_MIN_TILES (num_sms() / 2)      // at least one 512 x 256 tile per CTA pair
+#endif
+template <int A_MAJOR, int B_MAJOR, int EPI, int MT>
+inline int launch_gemm_bf16_mt(const void* A, int64_t lda, const void* B, int64_t ldb, const GemmShape& s,
+                               const EpiParams& ep, cudaStream_t st) {
+  const int64_t num_m = (s.M + TileCfg<MT>::kPairM - 1) / TileCfg<MT>::kPairM, num_n = (s.N + BLOCK_N - 1) / BLOCK_N;
+  if (OSDP_CM * OSDP_CN > 1 && num_m * num_n >= OSDP_CLUSTER_MIN_TILES)
+    return launch_gemm_bf16_cluster<A_MAJOR, B_MAJOR, EPI, MT, OSDP_CM, OSDP_CN>(A, lda, B, ldb, s, ep, st);
+  return launch_gemm_bf16_cluster<A_MAJOR, B_MAJOR, EPI, MT, 1, 1>(A, lda, B, ldb, s, ep, st);
+}
+template <int A_MAJOR, int B_MAJOR, int EPI>
+inline int launch_gemm_bf16(const void* A, int64_t lda, const void* B, int64_t ldb, const GemmShape& s,
+                            const EpiParams& ep, cudaStream_t st) {
+  const int64_t tiles2 = ((s.M + 511) / 512) * ((s.N + BLOCK_N - 1) / BLOCK_N);
+  if (s.K >= OSDP_MT2_MIN_K && tiles2 >= OSDP_MT2_MIN_TILES)
+    return launch_gemm_bf16_mt<A_MAJOR, B_MAJOR, EPI, 2>(A, lda, B, ldb, s, ep, st);
+  return launch_gemm_bf16_mt<A_MAJOR, B_MAJOR, EPI, 1>(A, lda, B, ldb, s, ep, st);
 }
 
 }  // namespace sm100
