@@ -28,6 +28,8 @@
 #pragma once
 #include <cuda.h>
 
+#include <atomic>
+
 #include "common.cuh"
 #include "epilogue_math.cuh"
 
@@ -47,13 +49,12 @@ constexpr int UMMA_K = 16;
 #define OSDP_WAIT_SLEEP_NS 0      // > 0: nanosleep between failed mbarrier polls of the long (epilogue) waits
 #endif
 constexpr int kTmemCols = 512;
-constexpr int kThreads = 256;
+constexpr int kThreads = 384;      // warps 0-3: TMA, MMA, TMEM alloc, (idle); warps 4-11: epilogue
 constexpr int kEpiWarp0 = 4;
-constexpr int kNumEpiWarps = 4;
+constexpr int kNumEpiWarps = 8;    // two per TMEM lane quarter (warp % 4), taking alternate column chunks
 constexpr uint32_t kBStageBytes = HALF_N * BLOCK_K * 2;    // 16 KiB (this CTA's half of the B tile)
 constexpr uint32_t kStoreBufBytes = 32 * 128;              // one warp's 32 rows x 128 B output segment
-constexpr uint32_t kStoreBufsPerWarp = 2;
-constexpr uint32_t kSmemStore = kNumEpiWarps * kStoreBufsPerWarp * kStoreBufBytes;   // 32 KiB
+constexpr uint32_t kSmemStore = kNumEpiWarps * kStoreBufBytes;   // 32 KiB
 
 // Two tile shapes share the kernel.  MT = M-halves (UMMAs of 128 rows) per CTA:
 //   MT = 1: CTA 128 x 256, pair 256 x 256; TMEM holds TWO accumulator stages, so the epilogue of tile i overlaps
@@ -297,19 +298,21 @@ struct EpiTraits {
   static constexpr int kChunkCols = kF32Out ? 32 : 64;
 };
 
-// Per-warp store pipeline: 2 staging buffers of 32 rows x 128 B (128B swizzle: 16-byte chunk j of row r sits at
-// chunk j ^ (r & 7), which is also what makes the 16-byte st.shared of 8 consecutive rows conflict-free).
+// Per-warp output staging: one buffer of 32 rows x 128 B (128B swizzle: 16-byte chunk j of row r sits at chunk
+// j ^ (r & 7), which is also what makes the 16-byte st.shared of 8 consecutive rows conflict-free).  A warp fills
+// it, hands it to TMA and meanwhile loads and computes its next chunk; the second warp of the same lane quarter
+// covers the remaining latency.
 struct StorePipe {
-  uint32_t base;    // smem address of this warp's two buffers
-  uint32_t count;   // stores issued so far
+  uint32_t buf;     // smem address of this warp's buffer
   int lane;
-  __device__ __forceinline__ void stage(const uint4 (&o)[8], const CUtensorMap* map, int c_inner, int c_outer, bool reduce_add) {
-    if (lane == 0) bulk_wait_read<kStoreBufsPerWarp - 1>();   // the buffer used two stores ago has been read out
+  __device__ __forceinline__ void begin() const {
+    if (lane == 0) bulk_wait_read<0>();   // the previous store has read the buffer out
     __syncwarp();
-    const uint32_t buf = base + (count & 1u) * kStoreBufBytes;
-    const uint32_t rowaddr = buf + lane * 128;
-#pragma unroll
-    for (int j = 0; j < 8; ++j) st_shared_v4(rowaddr + ((j ^ (lane & 7)) << 4), o[j]);
+  }
+  __device__ __forceinline__ void put(int j, const uint4& v) const {
+    st_shared_v4(buf + lane * 128 + ((j ^ (lane & 7)) << 4), v);
+  }
+  __device__ __forceinline__ void commit(const CUtensorMap* map, int c_inner, int c_outer, bool reduce_add) const {
     fence_proxy_async_smem();   // generic-proxy writes -> visible to the async proxy (TMA)
     __syncwarp();
     if (lane == 0) {
@@ -317,9 +320,43 @@ struct StorePipe {
       else            tma_store_2d(map, buf, c_inner, c_outer);
       bulk_commit();
     }
-    ++count;
   }
 };
+
+// ------------------------------------------------------------------------------------------------- wave sync
+// Persistent CTA pairs drift apart over a long launch; the pairs that share an A or B panel then fetch it at
+// different times, the panel has to survive in L2 for the whole skew, and DRAM reads grow to several times the
+// unique bytes (measured: 4.5 GB instead of 2-3 GB per C4 GEMM).  So the producers of all
+// clusters line up at every tile boundary: a cluster announces that the loads of its tile i are issued, and starts
+// the loads of tile i + 1 only when every cluster has announced tile i.  Tiles are equal work, so the wait is short,
+// and with MT = 2 it falls under the exposed epilogue.  In step, sharers hit L2 together (near-simultaneous
+// requests for a line are merged there) and DRAM reads fall to the unique bytes of a wave.
+// One counter per launch in flight; the cluster that makes the last announcement of a launch resets it to zero.
+constexpr int kWaveSyncSlots = 256;
+__device__ unsigned int g_wave_sync[kWaveSyncSlots];
+
+__device__ __forceinline__ unsigned int ld_acquire_gpu(const unsigned int* p) {
+  unsigned int v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ unsigned int atom_add_release_gpu(unsigned int* p, unsigned int x) {
+  unsigned int old;
+  asm volatile("atom.add.release.gpu.global.u32 %0, [%1], %2;" : "=r"(old) : "l"(p), "r"(x) : "memory");
+  return old;
+}
+__device__ __forceinline__ void wave_wait(const unsigned int* ctr, unsigned int target) {
+  uint64_t t0 = 0;
+  uint32_t spins = 0;
+  while (ld_acquire_gpu(ctr) < target) {
+    __nanosleep(64);
+    if ((++spins & 0x3FFu) == 0) {
+      const uint64_t now = global_timer_ns();
+      if (t0 == 0) t0 = now;
+      else if (now - t0 > 20ull * 1000 * 1000 * 1000) __trap();
+    }
+  }
+}
 
 // ------------------------------------------------------------------------------------------------- the kernel
 struct TileCoord {
@@ -342,7 +379,7 @@ template <int A_MAJOR, int B_MAJOR, int EPI, int MT, int CM, int CN>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
                        const __grid_constant__ CUtensorMap tmap_out0, const __grid_constant__ CUtensorMap tmap_out1,
-                       const GemmShape shape, const EpiParams ep, const int group_m) {
+                       const GemmShape shape, const EpiParams ep, const int group_m, unsigned int* wave_sync) {
   using Cfg = TileCfg<MT>;
   constexpr int kStages = Cfg::kStages, kAccStages = Cfg::kAccStages;
   constexpr int kCtaM = Cfg::kCtaM, kPairM = Cfg::kPairM;
@@ -420,7 +457,12 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
 #ifdef OSDP_DBG_NOLOAD
     int dbg_filled = 0;
 #endif
-    for (int t = cluster_id; t < num_tiles; t += num_clusters) {
+    int it = 0;
+    for (int t = cluster_id; t < num_tiles; t += num_clusters, ++it) {
+      if (wave_sync != nullptr && it > 0) {   // every cluster has issued the loads of its previous tile
+        if (lane == 0) wave_wait(wave_sync, (unsigned int)it * (unsigned int)num_clusters);
+        __syncwarp();
+      }
       const TileCoord tc = tile_coord(t, num_cm, num_cn, group_m);
       int m0 = (tc.m_blk * CM + pi) * kPairM + (int)rank * kCtaM;       // this CTA's rows of A
       int n0 = (tc.n_blk * CN + pj) * BLOCK_N + (int)rank * HALF_N;     // this CTA's half of the B tile
@@ -486,6 +528,10 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
         __syncwarp();
         if (++stage == kStages) { stage = 0; phase ^= 1; }
       }
+      if (wave_sync != nullptr && crank == 0 && lane == 0) {
+        if (atom_add_release_gpu(wave_sync, 1u) == (unsigned int)num_tiles - 1u)
+          *reinterpret_cast<volatile unsigned int*>(wave_sync) = 0u;   // last announcement of the launch: nobody waits any more
+      }
     }
   } else if (warp == 1 && leader) {
     // ================================================================== MMA issuer (each pair's leader CTA)
@@ -530,9 +576,30 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
     // ================================================================== epilogue (both CTAs, own rows)
     using Tr = EpiTraits<EPI>;
     constexpr int kChunk = Tr::kChunkCols;
-    const int q = warp % 4;   // TMEM lane quarter this warp may access
-    StorePipe pipe{smem_store + q * (kStoreBufsPerWarp * kStoreBufBytes), 0u, lane};
+    const int q = warp % 4;                    // TMEM lane quarter this warp may access
+    const int cg = (warp - kEpiWarp0) / 4;     // which of the two warps of that quarter: takes chunks cg, cg + 2, ...
+    const StorePipe pipe{smem_store + (uint32_t)(warp - kEpiWarp0) * kStoreBufBytes, lane};
     const uint32_t tempty_leader = mapa(tempty_bar, leader_crank);
+    const __nv_bfloat16* bias = reinterpret_cast<const __nv_bfloat16*>(ep.bias);
+    // 8 consecutive accumulator columns (+ bias) -> fp32 values
+    auto load8 = [&](const uint32_t* a, int ng, float (&v)[8]) {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(a[i]);
+      if constexpr (EPI == EPI_BIAS_GELU || EPI == EPI_BIAS || EPI == EPI_BIAS_GELU_DUAL) {
+        if (ng < shape.N) {   // warp-uniform
+          const uint4 b = __ldg(reinterpret_cast<const uint4*>(bias + ng));
+          const uint32_t bw[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            v[2 * i] += bf16_lo(bw[i]);
+            v[2 * i + 1] += bf16_hi(bw[i]);
+          }
+        }
+      }
+    };
+    auto pack8 = [](const float (&v)[8]) {
+      return make_uint4(pack_bf16x2(v[0], v[1]), pack_bf16x2(v[2], v[3]), pack_bf16x2(v[4], v[5]), pack_bf16x2(v[6], v[7]));
+    };
     int it = 0;
     for (int t = cluster_id; t < num_tiles; t += num_clusters, ++it) {
       const TileCoord tc = tile_coord(t, num_cm, num_cn, group_m);
@@ -542,81 +609,78 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
       const int n_end = min(n0 + BLOCK_N, shape.N);
       mbar_wait_long(tfull_bar + 8 * as, aphase);
       tc_fence_after();
-      bool released = false;   // the accumulator stage goes back to the MMA warp right after its last tcgen05.ld
+      bool released = false;   // the accumulator stage goes back to the MMA warp right after this warp's last tcgen05.ld
 #pragma unroll 1
       for (int h = 0; h < MT; ++h) {
-      const int row0 = (tc.m_blk * CM + pi) * kPairM + (int)rank * kCtaM + h * BLOCK_M + q * 32;   // this warp's 32-row band
-      const int64_t row = row0 + lane;
-      const bool row_ok = row < shape.M;
-      const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * (MT * BLOCK_N) + h * BLOCK_N;
-      bool skip = row0 >= shape.M || n0 >= shape.N;   // nothing of this warp's band lies inside C (warp-uniform)
+        const int row0 = (tc.m_blk * CM + pi) * kPairM + (int)rank * kCtaM + h * BLOCK_M + q * 32;   // this warp's 32-row band
+        const int64_t row = row0 + lane;
+        const bool row_ok = row < shape.M;
+        const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * (MT * BLOCK_N) + h * BLOCK_N;
+        bool skip = row0 >= shape.M;   // nothing of this warp's band lies inside C (warp-uniform)
 #ifdef OSDP_DBG_NOEPI   // probe: drain nothing, hand the accumulator straight back (no tcgen05.ld, no stores)
-      skip = true;
+        skip = true;
 #endif
-      if (skip) continue;
+        if (skip) continue;
 #pragma unroll 1
-      for (int n = n0; n < n_end; n += kChunk) {
-        uint32_t acc[kChunk];
+        for (int n = n0 + cg * kChunk; n < n_end; n += 2 * kChunk) {
+          uint32_t acc[kChunk];
+          [[maybe_unused]] uint4 zraw[8];
+          if constexpr (EPI == EPI_DGELU) {   // stored Z_s of this chunk: issue the loads before waiting on TMEM
 #pragma unroll
-        for (int i = 0; i < kChunk / 32; ++i)
-          tmem_ld_32x32(taddr + (n - n0) + 32 * i, *reinterpret_cast<uint32_t(*)[32]>(&acc[32 * i]));
-        tmem_ld_wait();
-        if (h == MT - 1 && n + kChunk >= n_end) {   // last read of this accumulator stage
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive_cluster(tempty_leader + 8 * as);
-          released = true;
-        }
-        uint4 o[8];
-        if constexpr (Tr::kF32Out) {
+            for (int j = 0; j < 8; ++j) {
+              zraw[j] = make_uint4(0, 0, 0, 0);
+              if (row_ok && n + 8 * j < shape.N)
+                zraw[j] = *reinterpret_cast<const uint4*>((const __nv_bfloat16*)ep.aux + row * ep.ldo + n + 8 * j);
+            }
+          }
 #pragma unroll
-          for (int j = 0; j < 8; ++j) o[j] = make_uint4(acc[4 * j], acc[4 * j + 1], acc[4 * j + 2], acc[4 * j + 3]);
-          pipe.stage(o, &tmap_out0, n, row0, ep.beta != 0);
-        } else {
-          uint4 oz[8];   // EPI_BIAS_GELU_DUAL: Z_s (first output)
+          for (int i = 0; i < kChunk / 32; ++i)
+            tmem_ld_32x32(taddr + (n - n0) + 32 * i, *reinterpret_cast<uint32_t(*)[32]>(&acc[32 * i]));
+          tmem_ld_wait();
+          if (h == MT - 1 && n + 2 * kChunk >= n_end) {   // this warp's last read of the accumulator stage
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(tempty_leader + 8 * as);
+            released = true;
+          }
+          if constexpr (Tr::kF32Out) {
+            pipe.begin();
 #pragma unroll
-          for (int j = 0; j < 8; ++j) {
-            const int ng = n + 8 * j;
-            float v[8];
+            for (int j = 0; j < 8; ++j) pipe.put(j, make_uint4(acc[4 * j], acc[4 * j + 1], acc[4 * j + 2], acc[4 * j + 3]));
+            pipe.commit(&tmap_out0, n, row0, ep.beta != 0);
+          } else {
+            if constexpr (EPI == EPI_BIAS_GELU_DUAL) {   // first pass: Z_s = acc + bias
+              pipe.begin();
 #pragma unroll
-            for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(acc[8 * j + i]);
-            if constexpr (EPI == EPI_BIAS_GELU || EPI == EPI_BIAS || EPI == EPI_BIAS_GELU_DUAL) {
-              if (ng < shape.N) {   // warp-uniform
-                const uint4 b = __ldg(reinterpret_cast<const uint4*>((const __nv_bfloat16*)ep.bias + ng));
-                const uint32_t bw[4] = {b.x, b.y, b.z, b.w};
+              for (int j = 0; j < 8; ++j) {
+                float v[8];
+                load8(&acc[8 * j], n + 8 * j, v);
+                pipe.put(j, pack8(v));
+              }
+              pipe.commit(&tmap_out0, n, row0, false);
+            }
+            pipe.begin();
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              float v[8];
+              load8(&acc[8 * j], n + 8 * j, v);
+              if constexpr (EPI == EPI_BIAS_GELU || EPI == EPI_BIAS_GELU_DUAL) {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) v[i] = gelu_fwd<false>(v[i]);
+              }
+              if constexpr (EPI == EPI_DGELU) {
+                const uint32_t zw[4] = {zraw[j].x, zraw[j].y, zraw[j].z, zraw[j].w};
 #pragma unroll
                 for (int i = 0; i < 4; ++i) {
-                  v[2 * i] += bf16_lo(bw[i]);
-                  v[2 * i + 1] += bf16_hi(bw[i]);
+                  v[2 * i] *= gelu_bwd<false>(bf16_lo(zw[i]));
+                  v[2 * i + 1] *= gelu_bwd<false>(bf16_hi(zw[i]));
                 }
               }
+              pipe.put(j, pack8(v));
             }
-            if constexpr (EPI == EPI_BIAS_GELU_DUAL)
-              oz[j] = make_uint4(pack_bf16x2(v[0], v[1]), pack_bf16x2(v[2], v[3]), pack_bf16x2(v[4], v[5]), pack_bf16x2(v[6], v[7]));
-            if constexpr (EPI == EPI_BIAS_GELU || EPI == EPI_BIAS_GELU_DUAL) {
-#pragma unroll
-              for (int i = 0; i < 8; ++i) v[i] = gelu_fwd<false>(v[i]);
-            }
-            if constexpr (EPI == EPI_DGELU) {
-              uint4 z = make_uint4(0, 0, 0, 0);
-              if (row_ok && ng < shape.N) z = *reinterpret_cast<const uint4*>((const __nv_bfloat16*)ep.aux + row * ep.ldo + ng);
-              const uint32_t zw[4] = {z.x, z.y, z.z, z.w};
-#pragma unroll
-              for (int i = 0; i < 4; ++i) {
-                v[2 * i] *= gelu_bwd<false>(bf16_lo(zw[i]));
-                v[2 * i + 1] *= gelu_bwd<false>(bf16_hi(zw[i]));
-              }
-            }
-            o[j] = make_uint4(pack_bf16x2(v[0], v[1]), pack_bf16x2(v[2], v[3]), pack_bf16x2(v[4], v[5]), pack_bf16x2(v[6], v[7]));
-          }
-          if constexpr (EPI == EPI_BIAS_GELU_DUAL) {
-            pipe.stage(oz, &tmap_out0, n, row0, false);
-            pipe.stage(o, &tmap_out1, n, row0, false);
-          } else {
-            pipe.stage(o, &tmap_out0, n, row0, false);
+            pipe.commit(EPI == EPI_BIAS_GELU_DUAL ? &tmap_out1 : &tmap_out0, n, row0, false);
           }
         }
-      }
       }   // h
       if (!released) {
         tc_fence_before();
@@ -726,10 +790,20 @@ inline int launch_gemm_bf16_cluster(const void* A, int64_t lda, const void* B, i
   int group_m = (int)(((int64_t)OSDP_BAND_MIB << 20) / row_bytes);
 #endif
   if (group_m < 1) group_m = 1;
+  // wave sync only when there is more than one wave, and only with a fully resident grid
+  unsigned int* wave_sync = nullptr;
+#ifndef OSDP_NO_WAVE_SYNC
+  if (MT == 2 && tiles > max_clusters) {   // MT = 1 overlaps its epilogue, so a wait at the tile boundary would be exposed
+    static unsigned int* base = nullptr;
+    static std::atomic<unsigned int> seq{0};
+    if (!base) OSDP_CUDA_TRY(cudaGetSymbolAddress(reinterpret_cast<void**>(&base), g_wave_sync));
+    wave_sync = base + (seq.fetch_add(1) % kWaveSyncSlots);
+  }
+#endif
   cudaError_t err;
   {
     LaunchTrace tr(st);
-    err = cudaLaunchKernelEx(&cfg, kernel, ta, tb, to0, to1, s, ep, group_m);
+    err = cudaLaunchKernelEx(&cfg, kernel, ta, tb, to0, to1, s, ep, group_m, wave_sync);
   }
   OSDP_CUDA_TRY(err);
   OSDP_CUDA_TRY(cudaGetLastError());
