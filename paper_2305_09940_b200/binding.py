@@ -32,6 +32,7 @@ EXPORTS = (
     "osdp_status_string", "osdp_last_cuda_error", "osdp_version", "osdp_split_mlp_workspace_bytes",
     "osdp_split_mlp_forward", "osdp_split_mlp_backward", "osdp_last_launch_count", "osdp_cost_eval",
     "osdp_mlp_op_cost", "osdp_plan", "osdp_plan_batch", "osdp_trace_enable", "osdp_trace_read", "osdp_step_name",
+    "osdp_set_tuning", "osdp_get_tuning",
 )
 
 
@@ -78,6 +79,11 @@ _lib.osdp_plan_batch.argtypes = [C.POINTER(osdp_op_cost), C.c_int32, C.POINTER(o
 
 _lib.osdp_trace_enable.restype = C.c_int
 _lib.osdp_trace_enable.argtypes = [C.c_int]
+_lib.osdp_set_tuning.restype = C.c_int
+_lib.osdp_set_tuning.argtypes = [C.c_int, C.c_int64]
+_lib.osdp_get_tuning.restype = C.c_int64
+_lib.osdp_get_tuning.argtypes = [C.c_int]
+OSDP_TUNE_MT2_MIN_K, OSDP_TUNE_MT2_MIN_TILES, OSDP_TUNE_WAVE_SYNC, OSDP_TUNE_BAND_MIB = 0, 1, 2, 3
 _lib.osdp_trace_read.restype = C.c_int64
 _lib.osdp_trace_read.argtypes = [C.c_int64, C.POINTER(C.c_int32), C.POINTER(C.c_float)]
 _lib.osdp_step_name.restype = C.c_char_p
@@ -107,6 +113,17 @@ def osdp_version() -> str:
 
 def osdp_last_launch_count() -> int:
     return int(_lib.osdp_last_launch_count())
+
+
+def osdp_set_tuning(key: int, value: int, check: bool = True) -> int:
+    rc = int(_lib.osdp_set_tuning(key, value))
+    if check and rc != OSDP_OK:
+        raise OsdpError(rc, "osdp_set_tuning")
+    return rc
+
+
+def osdp_get_tuning(key: int) -> int:
+    return int(_lib.osdp_get_tuning(key))
 
 
 def osdp_trace_enable(on: bool) -> None:

@@ -42,9 +42,17 @@ constexpr int BLOCK_N = 256;       // columns per pair tile = UMMA N
 constexpr int HALF_N = BLOCK_N / 2;   // B columns staged by each CTA
 constexpr int BLOCK_K = 64;
 constexpr int UMMA_K = 16;
-#ifndef OSDP_BAND_MIB
-#define OSDP_BAND_MIB 32          // L2 budget for the A rows of one raster band (see launch_gemm_bf16_cluster)
-#endif
+// Kernel selection knobs (osdp_set_tuning): defaults are the measured best on C3/C4.
+struct Tuning {
+  std::atomic<int64_t> mt2_min_k{4096};     // MT = 2 from this contraction length on
+  std::atomic<int64_t> mt2_min_tiles{0};    // ... and at least this many 512 x 256 tiles (0 = SMs / 2)
+  std::atomic<int64_t> wave_sync{1};        // line the producers up at tile boundaries (MT = 2 launches)
+  std::atomic<int64_t> band_mib{32};        // L2 budget for the A rows of one raster band
+};
+inline Tuning& tuning() {
+  static Tuning t;
+  return t;
+}
 #ifndef OSDP_WAIT_SLEEP_NS
 #define OSDP_WAIT_SLEEP_NS 0      // > 0: nanosleep between failed mbarrier polls of the long (epilogue) waits
 #endif
@@ -783,27 +791,23 @@ inline int launch_gemm_bf16_cluster(const void* A, int64_t lda, const void* B, i
   cfg.gridDim = dim3(kCluster * (tiles < max_clusters ? tiles : max_clusters));
   // Raster band: as many cluster-tile rows as keep the band's A rows (band rows x K bf16) inside the L2 budget;
   // DRAM reads are about |A| + |B| * (row bands), so taller is better while A stays resident.
-#ifdef OSDP_GROUP_M
-  int group_m = OSDP_GROUP_M / (CM * MT);
-#else
   const int64_t row_bytes = (int64_t)CM * Cfg::kPairM * s.K * 2;
-  int group_m = (int)(((int64_t)OSDP_BAND_MIB << 20) / row_bytes);
-#endif
+  int64_t group_m = (tuning().band_mib.load() << 20) / row_bytes;
   if (group_m < 1) group_m = 1;
+  if (group_m > (1 << 20)) group_m = 1 << 20;
   // wave sync only when there is more than one wave, and only with a fully resident grid
   unsigned int* wave_sync = nullptr;
-#ifndef OSDP_NO_WAVE_SYNC
-  if (MT == 2 && tiles > max_clusters) {   // MT = 1 overlaps its epilogue, so a wait at the tile boundary would be exposed
+  // (MT = 1 overlaps its epilogue with the next main loop, so a wait at the tile boundary would be exposed)
+  if (MT == 2 && tiles > max_clusters && tuning().wave_sync.load() != 0) {
     static unsigned int* base = nullptr;
     static std::atomic<unsigned int> seq{0};
     if (!base) OSDP_CUDA_TRY(cudaGetSymbolAddress(reinterpret_cast<void**>(&base), g_wave_sync));
     wave_sync = base + (seq.fetch_add(1) % kWaveSyncSlots);
   }
-#endif
   cudaError_t err;
   {
     LaunchTrace tr(st);
-    err = cudaLaunchKernelEx(&cfg, kernel, ta, tb, to0, to1, s, ep, group_m, wave_sync);
+    err = cudaLaunchKernelEx(&cfg, kernel, ta, tb, to0, to1, s, ep, (int)group_m, wave_sync);
   }
   OSDP_CUDA_TRY(err);
   OSDP_CUDA_TRY(cudaGetLastError());
@@ -824,12 +828,6 @@ inline int launch_gemm_bf16_cluster(const void* A, int64_t lda, const void* B, i
 #ifndef OSDP_CLUSTER_MIN_TILES
 #define OSDP_CLUSTER_MIN_TILES 148
 #endif
-#ifndef OSDP_MT2_MIN_K
-#define OSDP_MT2_MIN_K 4096
-#endif
-#ifndef OSDP_MT2_MIN_TILES
-#define OSDP_MT2_MIN_TILES (num_sms() / 2)      // at least one 512 x 256 tile per CTA pair
-#endif
 template <int A_MAJOR, int B_MAJOR, int EPI, int MT>
 inline int launch_gemm_bf16_mt(const void* A, int64_t lda, const void* B, int64_t ldb, const GemmShape& s,
                                const EpiParams& ep, cudaStream_t st) {
@@ -838,11 +836,26 @@ inline int launch_gemm_bf16_mt(const void* A, int64_t lda, const void* B, int64_
     return launch_gemm_bf16_cluster<A_MAJOR, B_MAJOR, EPI, MT, OSDP_CM, OSDP_CN>(A, lda, B, ldb, s, ep, st);
   return launch_gemm_bf16_cluster<A_MAJOR, B_MAJOR, EPI, MT, 1, 1>(A, lda, B, ldb, s, ep, st);
 }
+// Fraction of the machine's MMA slots that do useful work for pair tiles of pair_m rows: padding of M to whole
+// tiles (N is a multiple of 256 in every workload; its padding is the same for both shapes) times the fill of
+// the last wave.
+inline double tile_efficiency(const GemmShape& s, int pair_m) {
+  const int64_t num_m = (s.M + pair_m - 1) / pair_m, num_n = (s.N + BLOCK_N - 1) / BLOCK_N;
+  const int64_t tiles = num_m * num_n, pairs = num_sms() / 2;
+  const int64_t waves = (tiles + pairs - 1) / pairs;
+  return ((double)s.M / (double)(num_m * pair_m)) * ((double)tiles / (double)(waves * pairs));
+}
+
 template <int A_MAJOR, int B_MAJOR, int EPI>
 inline int launch_gemm_bf16(const void* A, int64_t lda, const void* B, int64_t ldb, const GemmShape& s,
                             const EpiParams& ep, cudaStream_t st) {
   const int64_t tiles2 = ((s.M + 511) / 512) * ((s.N + BLOCK_N - 1) / BLOCK_N);
-  if (s.K >= OSDP_MT2_MIN_K && tiles2 >= OSDP_MT2_MIN_TILES)
+  int64_t min_tiles = tuning().mt2_min_tiles.load();
+  const bool forced = min_tiles > 0;               // tests force MT = 2 on small shapes
+  if (min_tiles <= 0) min_tiles = num_sms() / 2;   // at least one 512 x 256 tile per CTA pair
+  // MT = 2 saves a quarter of the operand traffic; it is not worth more than ~10 % of idle MMA slots
+  const bool fits = forced || tile_efficiency(s, 512) >= 0.9 * tile_efficiency(s, 256);
+  if (s.K >= tuning().mt2_min_k.load() && tiles2 >= min_tiles && fits)
     return launch_gemm_bf16_mt<A_MAJOR, B_MAJOR, EPI, 2>(A, lda, B, ldb, s, ep, st);
   return launch_gemm_bf16_mt<A_MAJOR, B_MAJOR, EPI, 1>(A, lda, B, ldb, s, ep, st);
 }

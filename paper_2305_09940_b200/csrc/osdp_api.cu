@@ -177,6 +177,40 @@ const char* osdp_last_cuda_error(void) { return g_last_error.c_str(); }
 const char* osdp_version(void) { return "osdp-b200 0.1.0 (sm_100a)"; }
 int64_t osdp_last_launch_count(void) { return g_launches; }
 
+int osdp_set_tuning(int key, int64_t value) {
+  sm100::Tuning& t = sm100::tuning();
+  switch (key) {
+    case OSDP_TUNE_MT2_MIN_K:
+      if (value < 1) return OSDP_ERR_ARG;
+      t.mt2_min_k = value;
+      return OSDP_OK;
+    case OSDP_TUNE_MT2_MIN_TILES:
+      if (value < 0) return OSDP_ERR_ARG;
+      t.mt2_min_tiles = value;
+      return OSDP_OK;
+    case OSDP_TUNE_WAVE_SYNC:
+      if (value != 0 && value != 1) return OSDP_ERR_ARG;
+      t.wave_sync = value;
+      return OSDP_OK;
+    case OSDP_TUNE_BAND_MIB:
+      if (value < 1 || value > 1024) return OSDP_ERR_ARG;
+      t.band_mib = value;
+      return OSDP_OK;
+    default: return OSDP_ERR_ARG;
+  }
+}
+
+int64_t osdp_get_tuning(int key) {
+  sm100::Tuning& t = sm100::tuning();
+  switch (key) {
+    case OSDP_TUNE_MT2_MIN_K: return t.mt2_min_k;
+    case OSDP_TUNE_MT2_MIN_TILES: return t.mt2_min_tiles;
+    case OSDP_TUNE_WAVE_SYNC: return t.wave_sync;
+    case OSDP_TUNE_BAND_MIB: return t.band_mib;
+    default: return -1;
+  }
+}
+
 int osdp_trace_enable(int on) {
   g_trace.on = on != 0;
   if (!g_trace.on) g_trace.steps.clear();

@@ -88,6 +88,60 @@ def test_bf16_large_weights_stress_gelu_range(lib):
     check(run_gpu(lib, inp, 2, torch.bfloat16), ref, 2e-2, "bf16 wide")
 
 
+# ------------------------------------------------------------------ every tile shape of the bf16 GEMM on small shapes
+@pytest.fixture
+def force_big_tiles(lib):
+    """512 x 256 pair tiles (MT = 2) for every launch, whatever K and the tile count: the default build takes them
+    only for long-K GEMMs that fill the machine (full-size tests), so the ragged small shapes would never see them."""
+    keys = (lib.OSDP_TUNE_MT2_MIN_K, lib.OSDP_TUNE_MT2_MIN_TILES, lib.OSDP_TUNE_WAVE_SYNC, lib.OSDP_TUNE_BAND_MIB)
+    old = {k: lib.osdp_get_tuning(k) for k in keys}
+    lib.osdp_set_tuning(lib.OSDP_TUNE_MT2_MIN_K, 1)
+    lib.osdp_set_tuning(lib.OSDP_TUNE_MT2_MIN_TILES, 1)
+    yield
+    for k, v in old.items():
+        lib.osdp_set_tuning(k, v)
+
+
+@pytest.mark.parametrize("T,h,f,k", [
+    (512, 256, 512, 1),       # exact 512 x 256 tiles
+    (333, 136, 520, 3),       # ragged everywhere
+    (1000, 320, 1032, 2),     # partial second M-half, partial last tile
+    (130, 72, 264, 1),        # less than one M-half
+    (5, 64, 128, 5),
+])
+def test_bf16_big_tiles_match_oracle(lib, force_big_tiles, T, h, f, k):
+    inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=9)
+    ref = O.mlp_forward_backward(**inp.as_f64())
+    check(run_gpu(lib, inp, k, torch.bfloat16), ref, 2e-2, f"bf16 MT=2 {T}x{h}x{f} k={k}")
+
+
+def test_bf16_tile_shapes_and_wave_sync_agree_bitwise(lib, force_big_tiles):
+    """One owner CTA per output element and ascending-k accumulation in every configuration: tile shape, raster
+    band and wave sync change the schedule, not a single bit of the result.  Shape: more 512 x 256 tiles than CTA
+    pairs in the big GEMMs (several waves, so the wave sync really waits), ragged edges."""
+    T, h, f = 5200, 1288, 5144
+    inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=10)
+    outs = []
+    for min_k, sync, band in ((1, 1, 32), (1, 0, 32), (1, 1, 1), (1 << 40, 1, 32)):
+        lib.osdp_set_tuning(lib.OSDP_TUNE_MT2_MIN_K, min_k)
+        lib.osdp_set_tuning(lib.OSDP_TUNE_WAVE_SYNC, sync)
+        lib.osdp_set_tuning(lib.OSDP_TUNE_BAND_MIB, band)
+        outs.append(run_gpu(lib, inp, 2, torch.bfloat16))
+    for o in outs[1:]:
+        for n in NAMES:
+            assert np.array_equal(o[n], outs[0][n]), n
+    check(outs[0], O.mlp_forward_backward(**inp.as_f64()), 2e-2, "bf16 MT=2 several waves")
+
+
+def test_tuning_rejects_bad_arguments(lib):
+    assert lib.osdp_set_tuning(99, 1, check=False) == lib.OSDP_ERR_ARG
+    assert lib.osdp_set_tuning(lib.OSDP_TUNE_WAVE_SYNC, 2, check=False) == lib.OSDP_ERR_ARG
+    assert lib.osdp_set_tuning(lib.OSDP_TUNE_MT2_MIN_K, 0, check=False) == lib.OSDP_ERR_ARG
+    assert lib.osdp_set_tuning(lib.OSDP_TUNE_BAND_MIB, 0, check=False) == lib.OSDP_ERR_ARG
+    assert lib.osdp_get_tuning(99) == -1
+    assert lib.osdp_get_tuning(lib.OSDP_TUNE_MT2_MIN_K) == 4096 and lib.osdp_get_tuning(lib.OSDP_TUNE_WAVE_SYNC) == 1
+
+
 # ------------------------------------------------------------------ C2: full oracle at every k
 @pytest.fixture(scope="module")
 def c2():
