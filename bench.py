@@ -404,7 +404,7 @@ def main():
                "share": sum(v) / total_traced}
         if sid <= 7:
             ent["tflops"] = gemm_flops / (avg * 1e-3) / 1e12
-        kernels[f"A{sid}" if sid <= 8 else "db1"] = ent
+        kernels[f"A{sid}"] = ent
     dom = max((s for s in per if s <= 7), key=lambda s: sum(per[s]))
     dom_avg = sum(per[dom]) / len(per[dom])
     achieved = gemm_flops / (dom_avg * 1e-3) / 1e12

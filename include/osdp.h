@@ -69,7 +69,8 @@ const char* osdp_version(void);
 
 /* ---- A10: workspace accounting (PAPER.md:84-86 M_extra; PAPER.md:167 size/slice_granularity) ----------
  * Bytes of caller workspace one forward (OSDP_FWD) or backward (OSDP_BWD) call needs.  Pure host function.
- *   FWD: one [T_s x f] tensor (H_s);  BWD: two (Z_s, overwritten by dZ_s; H_s) + fixed fp32 column-sum scratch;
+ *   FWD: one [T_s x f] tensor (H_s);  BWD: two (Z_s, overwritten by dZ_s; H_s) + fixed fp32 column-sum scratch
+ *   (32 x (hidden + ffn) floats);
  *   T_s = ceil(T/k); each tensor rounded up to 256 B.  Returns 0 on an invalid descriptor. */
 size_t osdp_split_mlp_workspace_bytes(const osdp_mlp_desc* desc, int pass);
 
@@ -105,8 +106,8 @@ int64_t osdp_last_launch_count(void);
  * overlapped (MT = 1) and of 512 x 256 with 25 % less operand traffic and an exposed epilogue (MT = 2), the
  * latter with the producers of all CTA pairs lined up at every tile boundary ("wave sync").  A launch takes
  * MT = 2 when K >= OSDP_TUNE_MT2_MIN_K and it has at least OSDP_TUNE_MT2_MIN_TILES 512 x 256 tiles
- * (0 = one per CTA pair of the device).  OSDP_TUNE_WAVE_SYNC: 0 off, 1 on for MT = 2 launches of more than
- * one wave.  OSDP_TUNE_BAND_MIB: L2 budget (MiB) for the A rows of one raster band.  Results do not depend on
+ * (0 = one per CTA pair of the device).  OSDP_TUNE_WAVE_SYNC (MT = 2 launches of more than one wave): 0 off,
+ * 1 at tile boundaries, q > 1 also every q k-blocks (64 contraction elements each) inside a tile.  OSDP_TUNE_BAND_MIB: L2 budget (MiB) for the A rows of one raster band.  Results do not depend on
  * any knob beyond fp32 summation order inside a tile (there is none: one owner per output tile).
  * Returns OSDP_ERR_ARG for an unknown key or a value out of range.  osdp_get_tuning returns -1 for an unknown key. */
 typedef enum osdp_tune_key {
@@ -123,8 +124,8 @@ int64_t osdp_get_tuning(int key);
  * bracketed by two CUDA events recorded on the call's stream (nothing else changes; no synchronisation).
  * osdp_trace_read: waits for the recorded events, writes up to max_entries (step id, milliseconds) pairs in
  * launch order, clears the trace and returns the number of launches recorded since the last read (which may
- * exceed max_entries), or -1 on a CUDA error.  Step ids: 1..7 = A1..A7 GEMMs, 8 = A8 db2 column sum, 9 = db1
- * column sum (each column sum is two launches).  osdp_step_name(id) returns a static string. */
+ * exceed max_entries), or -1 on a CUDA error.  Step ids: 1..7 = A1..A7 GEMMs, 8 = the db2 and db1
+ * column sums (A8; two launches serve both).  osdp_step_name(id) returns a static string. */
 int osdp_trace_enable(int on);
 int64_t osdp_trace_read(int64_t max_entries, int32_t* step_ids, float* ms);
 const char* osdp_step_name(int step_id);

@@ -142,8 +142,8 @@ REDUCE_ROW_CHUNKS = 32
 
 
 def mlp_reduce_scratch_bytes(h: int, f: int) -> int:
-    """fp32 partial column sums for db1/db2: REDUCE_ROW_CHUNKS x max(h, f) floats, 256 B aligned."""
-    return ceil_div(REDUCE_ROW_CHUNKS * max(h, f) * 4, 256) * 256
+    """fp32 partial column sums for db2 and db1: REDUCE_ROW_CHUNKS x (h + f) floats, 256 B aligned."""
+    return ceil_div(REDUCE_ROW_CHUNKS * (h + f) * 4, 256) * 256
 
 
 def mlp_persistent_bytes(T: int, h: int, f: int, e: int, backward: bool) -> int:

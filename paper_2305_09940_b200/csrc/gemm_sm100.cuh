@@ -387,7 +387,8 @@ template <int A_MAJOR, int B_MAJOR, int EPI, int MT, int CM, int CN>
 __global__ void __launch_bounds__(kThreads, 1)
 gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
                        const __grid_constant__ CUtensorMap tmap_out0, const __grid_constant__ CUtensorMap tmap_out1,
-                       const GemmShape shape, const EpiParams ep, const int group_m, unsigned int* wave_sync) {
+                       const GemmShape shape, const EpiParams ep, const int group_m, unsigned int* wave_sync,
+                       const int sync_kb) {
   using Cfg = TileCfg<MT>;
   constexpr int kStages = Cfg::kStages, kAccStages = Cfg::kAccStages;
   constexpr int kCtaM = Cfg::kCtaM, kPairM = Cfg::kPairM;
@@ -446,6 +447,11 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
   cluster_sync();            // every CTA's barriers are initialised and TMEM is allocated before anyone proceeds
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
+  // Programmatic dependent launch: everything above overlapped the tail of the previous kernel of the stream; from
+  // here on this kernel reads and writes memory that kernel may still be using.  The next kernel may start its own
+  // set-up as soon as SMs free up.
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
   if (warp == 0) {
     // ================================================================== TMA producer (every CTA)
@@ -467,8 +473,12 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
 #endif
     int it = 0;
     for (int t = cluster_id; t < num_tiles; t += num_clusters, ++it) {
+      // Sync points of a tile: before k-blocks sync_kb, 2 sync_kb, ... (if sync_kb > 0) and after the last one.
+      const unsigned int syncs_per_tile = 1u + (sync_kb > 0 ? (unsigned int)((num_kb - 1) / sync_kb) : 0u);
+      const unsigned int sync_base = (unsigned int)it * syncs_per_tile * (unsigned int)num_clusters;   // earlier waves were full
+      const unsigned int active = (unsigned int)min(num_clusters, num_tiles - it * num_clusters);       // clusters in this wave
       if (wave_sync != nullptr && it > 0) {   // every cluster has issued the loads of its previous tile
-        if (lane == 0) wave_wait(wave_sync, (unsigned int)it * (unsigned int)num_clusters);
+        if (lane == 0) wave_wait(wave_sync, sync_base);
         __syncwarp();
       }
       const TileCoord tc = tile_coord(t, num_cm, num_cn, group_m);
@@ -483,6 +493,13 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
       n0 = (int)rank * HALF_N;
 #endif
       for (int kb = 0; kb < num_kb; ++kb) {
+        if (wave_sync != nullptr && sync_kb > 0 && kb > 0 && kb % sync_kb == 0) {   // stay in step inside the tile too
+          if (lane == 0) {
+            if (crank == 0) atom_add_release_gpu(wave_sync, 1u);
+            wave_wait(wave_sync, sync_base + (unsigned int)(kb / sync_kb) * active);
+          }
+          __syncwarp();
+        }
         mbar_wait(empty_bar + 8 * stage, phase ^ 1);   // the slot is free in every CTA of the cluster
 #ifdef OSDP_DBG_NOLOAD   // probe: after the ring has been filled once, re-use its contents (no L2->SM traffic)
         if (dbg_filled >= kStages) {
@@ -537,7 +554,7 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
         if (++stage == kStages) { stage = 0; phase ^= 1; }
       }
       if (wave_sync != nullptr && crank == 0 && lane == 0) {
-        if (atom_add_release_gpu(wave_sync, 1u) == (unsigned int)num_tiles - 1u)
+        if (atom_add_release_gpu(wave_sync, 1u) == (unsigned int)num_tiles * syncs_per_tile - 1u)
           *reinterpret_cast<volatile unsigned int*>(wave_sync) = 0u;   // last announcement of the launch: nobody waits any more
       }
     }
@@ -766,13 +783,15 @@ inline int launch_gemm_bf16_cluster(const void* A, int64_t lda, const void* B, i
   cfg.blockDim = dim3(kThreads);
   cfg.dynamicSmemBytes = Cfg::kSmemBytes;
   cfg.stream = st;
-  cudaLaunchAttribute attr[1];
+  cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = kCluster;
   attr[0].val.clusterDim.y = 1;
   attr[0].val.clusterDim.z = 1;
+  attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // see griddepcontrol in the kernel
+  attr[1].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
-  cfg.numAttrs = 1;
+  cfg.numAttrs = 2;
   static int max_clusters = 0;   // one process per GPU: attribute and occupancy are per function per device
   if (max_clusters == 0) {
     OSDP_CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmemBytes));
@@ -797,8 +816,9 @@ inline int launch_gemm_bf16_cluster(const void* A, int64_t lda, const void* B, i
   if (group_m > (1 << 20)) group_m = 1 << 20;
   // wave sync only when there is more than one wave, and only with a fully resident grid
   unsigned int* wave_sync = nullptr;
+  const int64_t sync_mode = tuning().wave_sync.load();   // 0 off, 1 tile boundaries, q > 1: also every q k-blocks
   // (MT = 1 overlaps its epilogue with the next main loop, so a wait at the tile boundary would be exposed)
-  if (MT == 2 && tiles > max_clusters && tuning().wave_sync.load() != 0) {
+  if (MT == 2 && tiles > max_clusters && sync_mode != 0) {
     static unsigned int* base = nullptr;
     static std::atomic<unsigned int> seq{0};
     if (!base) OSDP_CUDA_TRY(cudaGetSymbolAddress(reinterpret_cast<void**>(&base), g_wave_sync));
@@ -807,7 +827,8 @@ inline int launch_gemm_bf16_cluster(const void* A, int64_t lda, const void* B, i
   cudaError_t err;
   {
     LaunchTrace tr(st);
-    err = cudaLaunchKernelEx(&cfg, kernel, ta, tb, to0, to1, s, ep, (int)group_m, wave_sync);
+    err = cudaLaunchKernelEx(&cfg, kernel, ta, tb, to0, to1, s, ep, (int)group_m, wave_sync,
+                             sync_mode > 1 ? (int)sync_mode : 0);
   }
   OSDP_CUDA_TRY(err);
   OSDP_CUDA_TRY(cudaGetLastError());

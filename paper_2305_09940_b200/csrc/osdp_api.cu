@@ -103,8 +103,7 @@ inline size_t slice_buf_bytes(const osdp_mlp_desc* d) {
   return align_up((size_t)ts * (size_t)d->ffn * elem_size(d->dtype), 256);
 }
 inline size_t reduce_scratch_bytes(const osdp_mlp_desc* d) {
-  const int64_t c = d->hidden > d->ffn ? d->hidden : d->ffn;
-  return align_up((size_t)kReduceRowChunks * (size_t)c * 4, 256);
+  return align_up((size_t)kReduceRowChunks * (size_t)(d->hidden + d->ffn) * 4, 256);
 }
 size_t workspace_bytes(const osdp_mlp_desc* d, int pass) {
   if (pass == OSDP_FWD) return slice_buf_bytes(d);
@@ -136,10 +135,13 @@ int gemm(int dtype, const void* A, int64_t lda, const void* B, int64_t ldb, cons
   return launch_gemm_f32<EPI>(op, s, ep, st);
 }
 
-int colsum(int dtype, const void* src, int rows, int cols, int64_t ld, float* scratch, float* out, int beta,
-           cudaStream_t st) {
-  if (dtype == OSDP_BF16) return launch_colsum<__nv_bfloat16>((const __nv_bfloat16*)src, rows, cols, ld, scratch, out, beta, st);
-  return launch_colsum<float>((const float*)src, rows, cols, ld, scratch, out, beta, st);
+// db2 (+)= colsum(dY_s [rows x h]), db1 (+)= colsum(dZ_s [rows x f])
+int colsum2(int dtype, const void* dYs, int h, float* db2, const void* dZs, int f, float* db1, int rows, float* scratch,
+            int beta, cudaStream_t st) {
+  if (dtype == OSDP_BF16)
+    return launch_colsum2<__nv_bfloat16>((const __nv_bfloat16*)dYs, h, h, db2, (const __nv_bfloat16*)dZs, f, f, db1, rows,
+                                         scratch, beta, st);
+  return launch_colsum2<float>((const float*)dYs, h, h, db2, (const float*)dZs, f, f, db1, rows, scratch, beta, st);
 }
 
 #define OSDP_TRY(expr)            \
@@ -189,7 +191,7 @@ int osdp_set_tuning(int key, int64_t value) {
       t.mt2_min_tiles = value;
       return OSDP_OK;
     case OSDP_TUNE_WAVE_SYNC:
-      if (value != 0 && value != 1) return OSDP_ERR_ARG;
+      if (value < 0 || value > (1 << 20)) return OSDP_ERR_ARG;
       t.wave_sync = value;
       return OSDP_OK;
     case OSDP_TUNE_BAND_MIB:
@@ -246,8 +248,7 @@ const char* osdp_step_name(int step_id) {
     case 5: return "A5 dW2 += H^T dY";
     case 6: return "A6 dW1 += X^T dZ";
     case 7: return "A7 dX = dZ W1^T";
-    case 8: return "A8 db2 column sum";
-    case 9: return "db1 column sum";
+    case 8: return "A8 db2 and db1 column sums";
     default: return "unknown";
   }
 }
@@ -356,9 +357,7 @@ int osdp_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const void
     OSDP_TRY((gemm<MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32>(dt, Hs, f, dYs, h, GemmShape{(int)f, (int)h, Ts}, e5, st)));
     // A8: db2 (+)= colsum(dY_s);  db1 (+)= colsum(dZ_s)
     trace_set_step(8);
-    OSDP_TRY(colsum(dt, dYs, Ts, (int)h, h, scratch, db2, beta, st));
-    trace_set_step(9);
-    OSDP_TRY(colsum(dt, Zs, Ts, (int)f, f, scratch, db1, beta, st));
+    OSDP_TRY(colsum2(dt, dYs, (int)h, db2, Zs, (int)f, db1, Ts, scratch, beta, st));
     // A6: dW1 (+)= X_s^T dZ_s
     trace_set_step(6);
     EpiParams e6 = {nullptr, dW1, nullptr, nullptr, f, beta};
