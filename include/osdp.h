@@ -97,6 +97,41 @@ int osdp_split_mlp_backward(const osdp_mlp_desc* desc,
                             void* dX, float* dW1, float* db1, float* dW2, float* db2,
                             void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- ffn-axis split: the paper-literal operator splitting applied to the MLP pair -------------------------
+ * PAPER.md:165 (section 3.3): "both the last dimension of the input data and the first dimension of the operator
+ * are partitioned into multiple slices ... the computation of each slice is executed sequentially ... all
+ * computation results are summed as the final output".  For Linear2 (Y = H W2) the contraction axis is ffn, so
+ * slice s owns ffn columns [lo_s, lo_{s+1}) and
+ *     forward : H_s = gelu(X W1[:, lo_s:lo_{s+1}] + b1[lo_s:lo_{s+1}])   [tokens x f_s]  (workspace)
+ *               Y  += H_s W2[lo_s:lo_{s+1}, :]                            summed over slices in fp32, then + b2
+ *     backward: Z_s, H_s recomputed; dZ_s = (dY W2[lo_s:lo_{s+1}, :]^T) (.) gelu'(Z_s)
+ *               dW2[lo_s:lo_{s+1}, :] = H_s^T dY;  dW1[:, lo_s:lo_{s+1}] = X^T dZ_s;  db1[lo_s:lo_{s+1}] = colsum(dZ_s)
+ *               (each written once: slices own disjoint parts of the weight gradients)
+ *               dX += dZ_s W1[:, lo_s:lo_{s+1}]^T                         summed over slices in fp32;  db2 = colsum(dY)
+ * The tokens x ffn intermediate never exists whole (only tokens x ceil(ffn/k)), exactly as in the token split,
+ * but the only tensors that span slices are Y and dX (tokens x hidden) instead of dW1 and dW2 (hidden x ffn):
+ * the cross-slice read-modify-write traffic falls by hidden*ffn / (tokens*hidden) and every weight is read once per pass
+ * (DESIGN.md section 10).
+ * Same arguments, dtypes, layouts, ownership and error behaviour as osdp_split_mlp_forward/backward, except:
+ *   - desc->k = number of ffn slices, 1 <= k <= ffn / (16 / sizeof(dtype));  lo_s = floor(s * units / k) * unit with
+ *     unit = 16 bytes of elements and units = ffn / unit (slices are whole 16-byte column groups);
+ *   - workspace (osdp_ffn_split_mlp_workspace_bytes): FWD one [tokens x f_max] tensor, BWD two, f_max = the widest
+ *     slice; for k > 1 plus one fp32 [tokens x hidden] accumulator (Y or dX); BWD plus the column-sum scratch.
+ *     Each part rounded up to 256 B.
+ *   - results: Y and dX differ across k only by fp32 re-association of the slice sums (then one rounding to the
+ *     storage dtype); dW1, dW2, db1, db2 are bit-identical for every k.
+ * osdp_ffn_split_mlp_op_cost fills the cost-model factors of this variant for osdp_cost_eval / osdp_plan
+ * (extra_fixed includes the fp32 accumulator, i.e. it describes k > 1). */
+size_t osdp_ffn_split_mlp_workspace_bytes(const osdp_mlp_desc* desc, int pass);
+int osdp_ffn_split_mlp_forward(const osdp_mlp_desc* desc,
+                               const void* X, const void* W1, const void* b1, const void* W2, const void* b2,
+                               void* Y, void* workspace, size_t workspace_bytes, void* stream);
+int osdp_ffn_split_mlp_backward(const osdp_mlp_desc* desc,
+                                const void* X, const void* W1, const void* b1, const void* W2, const void* b2,
+                                const void* dY,
+                                void* dX, float* dW1, float* db1, float* dW2, float* db2,
+                                void* workspace, size_t workspace_bytes, void* stream);
+
 /* Number of kernel launches the last forward/backward call of the calling thread enqueued (for bench.py's
  * gpu_launches claim). */
 int64_t osdp_last_launch_count(void);
@@ -167,6 +202,7 @@ int osdp_cost_eval(const osdp_op_cost* op, int mode, int32_t k, int64_t batch, c
  * gradients); extra_transient = workspace at k = 1 minus the fixed scratch; extra_fixed = that scratch;
  * S = (2 h f + f + h) * sizeof(dtype); act_bytes = 0; gamma/delta = 0 (the caller calibrates them). */
 int osdp_mlp_op_cost(const osdp_mlp_desc* desc, int pass, osdp_op_cost* out);
+int osdp_ffn_split_mlp_op_cost(const osdp_mlp_desc* desc, int pass, osdp_op_cost* out);   /* ffn-axis split, see above */
 
 /* Search engine (Algorithm 1 lines 4-11 at a fixed batch; PAPER.md:149 DFS with two prunings).
  * Decision per operator: mode in {DP, ZDP} x k in k_candidates (ascending, each >= 1).  Minimises

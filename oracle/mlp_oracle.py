@@ -127,6 +127,37 @@ def matmul_contraction_split(X, W, granularity: int):
     return out
 
 
+def ffn_slice_bounds(f: int, k: int, unit: int):
+    """Slices of the ffn axis in whole ``unit``-column groups (unit = 16 bytes of storage elements):
+    slice s = columns [floor(s U / k) unit, floor((s + 1) U / k) unit) with U = f / unit."""
+    U = f // unit
+    return [((s * U) // k * unit, ((s + 1) * U) // k * unit) for s in range(k)]
+
+
+def mlp_forward_backward_ffn_split(X, W1, b1, W2, b2, dY, k: int, unit: int = 8):
+    """The paper-literal split applied to the MLP pair, in fp64: Linear2's contraction
+    axis (= Linear1's output axis) is cut into k slices, the slices are computed one after another and
+    the partial products of Y and of dX are summed; each slice writes its own rows of dW2 and columns
+    of dW1 / db1.  Used only to pin "ffn split == unsplit"."""
+    T, f = X.shape[0], W1.shape[1]
+    Y = np.zeros((T, W2.shape[1]))
+    dX = np.zeros_like(X)
+    dW1 = np.empty_like(W1)
+    dW2 = np.empty_like(W2)
+    db1 = np.empty_like(b1)
+    for lo, hi in ffn_slice_bounds(f, k, unit):
+        Zs = X @ W1[:, lo:hi] + b1[None, lo:hi]
+        Hs = gelu(Zs)
+        Y += Hs @ W2[lo:hi, :]
+        dZs = (dY @ W2[lo:hi, :].T) * gelu_prime(Zs)
+        dW2[lo:hi, :] = Hs.T @ dY
+        dW1[:, lo:hi] = X.T @ dZs
+        db1[lo:hi] = dZs.sum(axis=0)
+        dX += dZs @ W1[:, lo:hi].T
+    Y += b2[None, :]
+    return dict(Y=Y, dX=dX, dW1=dW1, db1=db1, dW2=dW2, db2=dY.sum(axis=0))
+
+
 # ----------------------------------------------------------------------------------------------
 # Sampled oracle for the large configs (SURVEY.md §8(c) "GPU vs oracle"): the SAME definition,
 # restricted to a subset of token rows or of ffn columns.  Every output tensor is covered:

@@ -32,7 +32,8 @@ EXPORTS = (
     "osdp_status_string", "osdp_last_cuda_error", "osdp_version", "osdp_split_mlp_workspace_bytes",
     "osdp_split_mlp_forward", "osdp_split_mlp_backward", "osdp_last_launch_count", "osdp_cost_eval",
     "osdp_mlp_op_cost", "osdp_plan", "osdp_plan_batch", "osdp_trace_enable", "osdp_trace_read", "osdp_step_name",
-    "osdp_set_tuning", "osdp_get_tuning",
+    "osdp_set_tuning", "osdp_get_tuning", "osdp_ffn_split_mlp_workspace_bytes", "osdp_ffn_split_mlp_forward",
+    "osdp_ffn_split_mlp_backward", "osdp_ffn_split_mlp_op_cost",
 )
 
 
@@ -62,6 +63,14 @@ _lib.osdp_split_mlp_forward.restype = C.c_int
 _lib.osdp_split_mlp_forward.argtypes = [C.POINTER(osdp_mlp_desc)] + [C.c_void_p] * 7 + [C.c_size_t, C.c_void_p]
 _lib.osdp_split_mlp_backward.restype = C.c_int
 _lib.osdp_split_mlp_backward.argtypes = [C.POINTER(osdp_mlp_desc)] + [C.c_void_p] * 12 + [C.c_size_t, C.c_void_p]
+_lib.osdp_ffn_split_mlp_workspace_bytes.restype = C.c_size_t
+_lib.osdp_ffn_split_mlp_workspace_bytes.argtypes = [C.POINTER(osdp_mlp_desc), C.c_int]
+_lib.osdp_ffn_split_mlp_forward.restype = C.c_int
+_lib.osdp_ffn_split_mlp_forward.argtypes = [C.POINTER(osdp_mlp_desc)] + [C.c_void_p] * 7 + [C.c_size_t, C.c_void_p]
+_lib.osdp_ffn_split_mlp_backward.restype = C.c_int
+_lib.osdp_ffn_split_mlp_backward.argtypes = [C.POINTER(osdp_mlp_desc)] + [C.c_void_p] * 12 + [C.c_size_t, C.c_void_p]
+_lib.osdp_ffn_split_mlp_op_cost.restype = C.c_int
+_lib.osdp_ffn_split_mlp_op_cost.argtypes = [C.POINTER(osdp_mlp_desc), C.c_int, C.POINTER(osdp_op_cost)]
 _lib.osdp_cost_eval.restype = C.c_int
 _lib.osdp_cost_eval.argtypes = [C.POINTER(osdp_op_cost), C.c_int, C.c_int32, C.c_int64, C.POINTER(osdp_device),
                                 C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_double)]
@@ -199,6 +208,40 @@ def osdp_split_mlp_backward(desc, X, W1, b1, W2, b2, dY, dX, dW1, db1, dW2, db2,
     return st
 
 
+def osdp_ffn_split_mlp_workspace_bytes(desc: osdp_mlp_desc, pass_: int) -> int:
+    return int(_lib.osdp_ffn_split_mlp_workspace_bytes(C.byref(desc), int(pass_)))
+
+
+def osdp_ffn_split_mlp_forward(desc, X, W1, b1, W2, b2, Y, workspace, workspace_bytes=None, stream=None, check=True):
+    if workspace_bytes is None:
+        workspace_bytes = workspace.numel() * workspace.element_size()
+    st = _lib.osdp_ffn_split_mlp_forward(C.byref(desc), _ptr(X), _ptr(W1), _ptr(b1), _ptr(W2), _ptr(b2), _ptr(Y),
+                                         _ptr(workspace), int(workspace_bytes), _stream_ptr(stream))
+    if check and st != OSDP_OK:
+        raise OsdpError(st, "osdp_ffn_split_mlp_forward")
+    return st
+
+
+def osdp_ffn_split_mlp_backward(desc, X, W1, b1, W2, b2, dY, dX, dW1, db1, dW2, db2, workspace, workspace_bytes=None,
+                                stream=None, check=True):
+    if workspace_bytes is None:
+        workspace_bytes = workspace.numel() * workspace.element_size()
+    st = _lib.osdp_ffn_split_mlp_backward(C.byref(desc), _ptr(X), _ptr(W1), _ptr(b1), _ptr(W2), _ptr(b2), _ptr(dY),
+                                          _ptr(dX), _ptr(dW1), _ptr(db1), _ptr(dW2), _ptr(db2), _ptr(workspace),
+                                          int(workspace_bytes), _stream_ptr(stream))
+    if check and st != OSDP_OK:
+        raise OsdpError(st, "osdp_ffn_split_mlp_backward")
+    return st
+
+
+def osdp_ffn_split_mlp_op_cost(desc: osdp_mlp_desc, pass_: int) -> osdp_op_cost:
+    out = osdp_op_cost()
+    st = _lib.osdp_ffn_split_mlp_op_cost(C.byref(desc), pass_, C.byref(out))
+    if st != OSDP_OK:
+        raise OsdpError(st, "osdp_ffn_split_mlp_op_cost")
+    return out
+
+
 # ---------------------------------------------------------------------------------------------- planner
 def osdp_cost_eval(op: osdp_op_cost, mode: int, k: int, batch: int, dev: osdp_device):
     p, t, s = C.c_uint64(), C.c_uint64(), C.c_double()
@@ -257,11 +300,17 @@ def osdp_plan_batch(ops, dev: osdp_device, batch_max: int, k_candidates, check=T
 class SplitMlp:
     """Holds a descriptor and caller-owned workspace/outputs for repeated calls on one device."""
 
-    def __init__(self, tokens, hidden, ffn, dtype: torch.dtype, k: int, device="cuda"):
+    def __init__(self, tokens, hidden, ffn, dtype: torch.dtype, k: int, device="cuda", axis="tokens"):
+        """axis = "tokens" (osdp_split_mlp_*) or "ffn" (osdp_ffn_split_mlp_*, the paper-literal contraction split)."""
+        if axis not in ("tokens", "ffn"):
+            raise ValueError("axis must be 'tokens' or 'ffn'")
         self.desc = make_desc(tokens, hidden, ffn, dtype, k)
-        self.dtype, self.device = dtype, torch.device(device)
-        self.ws_fwd_bytes = osdp_split_mlp_workspace_bytes(self.desc, OSDP_FWD)
-        self.ws_bwd_bytes = osdp_split_mlp_workspace_bytes(self.desc, OSDP_BWD)
+        self.dtype, self.device, self.axis = dtype, torch.device(device), axis
+        ws = osdp_split_mlp_workspace_bytes if axis == "tokens" else osdp_ffn_split_mlp_workspace_bytes
+        self._fwd = osdp_split_mlp_forward if axis == "tokens" else osdp_ffn_split_mlp_forward
+        self._bwd = osdp_split_mlp_backward if axis == "tokens" else osdp_ffn_split_mlp_backward
+        self.ws_fwd_bytes = ws(self.desc, OSDP_FWD)
+        self.ws_bwd_bytes = ws(self.desc, OSDP_BWD)
         if self.ws_fwd_bytes == 0:
             raise OsdpError(OSDP_ERR_SHAPE, "SplitMlp: invalid descriptor")
         self.workspace = torch.empty(max(self.ws_fwd_bytes, self.ws_bwd_bytes), dtype=torch.uint8, device=self.device)
@@ -269,7 +318,7 @@ class SplitMlp:
     def forward(self, X, W1, b1, W2, b2, Y=None, stream=None):
         if Y is None:
             Y = torch.empty_like(X)
-        osdp_split_mlp_forward(self.desc, X, W1, b1, W2, b2, Y, self.workspace, stream=stream)
+        self._fwd(self.desc, X, W1, b1, W2, b2, Y, self.workspace, stream=stream)
         return Y
 
     def backward(self, X, W1, b1, W2, dY, out=None, stream=None):
@@ -279,6 +328,6 @@ class SplitMlp:
                        db1=torch.empty(b1.shape, dtype=torch.float32, device=X.device),
                        dW2=torch.empty(W2.shape, dtype=torch.float32, device=X.device),
                        db2=torch.empty(W2.shape[1], dtype=torch.float32, device=X.device))
-        osdp_split_mlp_backward(self.desc, X, W1, b1, W2, None, dY, out["dX"], out["dW1"], out["db1"], out["dW2"],
-                                out["db2"], self.workspace, stream=stream)
+        self._bwd(self.desc, X, W1, b1, W2, None, dY, out["dX"], out["dW1"], out["db1"], out["dW2"],
+                  out["db2"], self.workspace, stream=stream)
         return out

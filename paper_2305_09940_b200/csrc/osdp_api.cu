@@ -7,6 +7,7 @@
 #include <string>
 #include <vector>
 
+#include "cast.cuh"
 #include "common.cuh"
 #include "gemm_f32.cuh"
 #include "gemm_sm100.cuh"
@@ -108,6 +109,37 @@ inline size_t reduce_scratch_bytes(const osdp_mlp_desc* d) {
 size_t workspace_bytes(const osdp_mlp_desc* d, int pass) {
   if (pass == OSDP_FWD) return slice_buf_bytes(d);
   return 2 * slice_buf_bytes(d) + reduce_scratch_bytes(d);
+}
+
+// ---- ffn-axis split: slice s owns ffn columns [ffn_lo(s), ffn_lo(s + 1)), whole 16-byte units
+inline int64_t ffn_unit(const osdp_mlp_desc* d) { return 16 / (int64_t)elem_size(d->dtype); }
+inline int64_t ffn_lo(const osdp_mlp_desc* d, int64_t s) {
+  const int64_t u = ffn_unit(d), units = d->ffn / u;
+  return (s * units / d->k) * u;
+}
+inline int64_t ffn_slice_max(const osdp_mlp_desc* d) {
+  const int64_t u = ffn_unit(d), units = d->ffn / u;
+  return ((units + d->k - 1) / d->k) * u;
+}
+int check_desc_ffn(const osdp_mlp_desc* d) {
+  const int rc = check_desc(d);
+  if (rc == OSDP_ERR_K) {   // check_desc bounds k by tokens; here the bound is the number of 16-byte ffn units
+    if (d->k < 1) return OSDP_ERR_K;
+  } else if (rc != OSDP_OK) {
+    return rc;
+  }
+  if ((int64_t)d->k > d->ffn / ffn_unit(d)) return OSDP_ERR_K;
+  return OSDP_OK;
+}
+inline size_t ffn_slice_buf_bytes(const osdp_mlp_desc* d) {
+  return align_up((size_t)d->tokens * (size_t)ffn_slice_max(d) * elem_size(d->dtype), 256);
+}
+inline size_t ffn_acc_bytes(const osdp_mlp_desc* d) {   // fp32 accumulator of Y / dX across slices; not needed at k = 1
+  return d->k == 1 ? 0 : align_up((size_t)d->tokens * (size_t)d->hidden * 4, 256);
+}
+size_t ffn_workspace_bytes(const osdp_mlp_desc* d, int pass) {
+  if (pass == OSDP_FWD) return ffn_slice_buf_bytes(d) + ffn_acc_bytes(d);
+  return 2 * ffn_slice_buf_bytes(d) + ffn_acc_bytes(d) + reduce_scratch_bytes(d);
 }
 
 inline bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) != 0; }
@@ -249,6 +281,7 @@ const char* osdp_step_name(int step_id) {
     case 6: return "A6 dW1 += X^T dZ";
     case 7: return "A7 dX = dZ W1^T";
     case 8: return "A8 db2 and db1 column sums";
+    case 10: return "fp32 accumulator -> output (ffn-axis split)";
     default: return "unknown";
   }
 }
@@ -366,6 +399,141 @@ int osdp_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const void
     trace_set_step(7);
     EpiParams e7 = {nullptr, dXs, nullptr, nullptr, h, 0};
     OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_PLAIN>(dt, Zs, f, W1, f, GemmShape{Ts, (int)h, (int)f}, e7, st)));
+  }
+  return OSDP_OK;
+}
+
+// ============================================================================================ ffn-axis split
+size_t osdp_ffn_split_mlp_workspace_bytes(const osdp_mlp_desc* desc, int pass) {
+  if (check_desc_ffn(desc) != OSDP_OK || (pass != OSDP_FWD && pass != OSDP_BWD)) return 0;
+  return ffn_workspace_bytes(desc, pass);
+}
+
+int osdp_ffn_split_mlp_op_cost(const osdp_mlp_desc* desc, int pass, osdp_op_cost* out) {
+  if (!out) return OSDP_ERR_NULL;
+  OSDP_TRY(check_desc_ffn(desc));
+  if (pass != OSDP_FWD && pass != OSDP_BWD) return OSDP_ERR_ARG;
+  const uint64_t T = desc->tokens, h = desc->hidden, f = desc->ffn, e = elem_size(desc->dtype);
+  osdp_op_cost c = {};
+  c.S = (double)((2 * h * f + f + h) * e);
+  const uint64_t acc = align_up((size_t)T * h * 4, 256);   // cross-slice fp32 accumulator (any k > 1)
+  if (pass == OSDP_FWD) {
+    c.model_bytes = (2 * T * h + 2 * h * f + f + h) * e;
+    c.extra_transient = T * f * e;
+    c.extra_fixed = acc;
+  } else {
+    c.model_bytes = (3 * T * h + 2 * h * f + f + h) * e + (2 * h * f + f + h) * 4;
+    c.extra_transient = 2 * T * f * e;
+    c.extra_fixed = acc + reduce_scratch_bytes(desc);
+  }
+  *out = c;
+  return OSDP_OK;
+}
+
+int osdp_ffn_split_mlp_forward(const osdp_mlp_desc* desc, const void* X, const void* W1, const void* b1, const void* W2,
+                               const void* b2, void* Y, void* workspace, size_t workspace_bytes_given, void* stream) {
+  g_launches = 0;
+  OSDP_TRY(check_desc_ffn(desc));
+  if (!X || !W1 || !b1 || !W2 || !b2 || !Y || !workspace) return OSDP_ERR_NULL;
+  if (misaligned(X, 16) || misaligned(W1, 16) || misaligned(b1, 16) || misaligned(W2, 16) || misaligned(b2, 16) ||
+      misaligned(Y, 16))
+    return OSDP_ERR_ALIGN;
+  if (misaligned(workspace, 256) || workspace_bytes_given < ffn_workspace_bytes(desc, OSDP_FWD)) return OSDP_ERR_WORKSPACE;
+  if (desc->dtype == OSDP_BF16) OSDP_TRY(check_arch());
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t T = desc->tokens, h = desc->hidden;
+  const size_t e = elem_size(desc->dtype);
+  const int dt = desc->dtype, k = desc->k;
+  void* Hs = workspace;
+  float* Yacc = (float*)((char*)workspace + ffn_slice_buf_bytes(desc));
+
+  for (int s = 0; s < k; ++s) {
+    const int64_t lo = ffn_lo(desc, s), hi = ffn_lo(desc, s + 1);
+    const int fs = (int)(hi - lo);
+    if (fs == 0) continue;   // cannot happen for k <= units; kept for symmetry with the token split
+    // A1: H_s = gelu(X W1[:, lo:hi] + b1[lo:hi])                    [T x fs], compact
+    trace_set_step(1);
+    EpiParams e1 = {(const char*)b1 + (size_t)lo * e, Hs, nullptr, nullptr, fs, 0};
+    OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_BIAS_GELU>(dt, X, h, (const char*)W1 + (size_t)lo * e, desc->ffn,
+                                                     GemmShape{(int)T, fs, (int)h}, e1, st)));
+    // A2: Y (+)= H_s W2[lo:hi, :]   -- the paper's split: contraction axis sliced, partial products summed
+    trace_set_step(2);
+    const char* W2s = (const char*)W2 + (size_t)lo * h * e;
+    if (k == 1) {
+      EpiParams e2 = {b2, Y, nullptr, nullptr, h, 0};
+      OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_BIAS>(dt, Hs, fs, W2s, h, GemmShape{(int)T, (int)h, fs}, e2, st)));
+    } else {
+      EpiParams e2 = {nullptr, Yacc, nullptr, nullptr, h, s == 0 ? 0 : 1};
+      OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_ACCUM_F32>(dt, Hs, fs, W2s, h, GemmShape{(int)T, (int)h, fs}, e2, st)));
+    }
+  }
+  if (k > 1) {   // Y = storage(Yacc + b2)
+    trace_set_step(10);
+    OSDP_TRY(launch_acc_to_out(dt, Yacc, b2, Y, T, (int)h, sm100::num_sms(), st));
+  }
+  return OSDP_OK;
+}
+
+int osdp_ffn_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const void* W1, const void* b1, const void* W2,
+                                const void* b2, const void* dY, void* dX, float* dW1, float* db1, float* dW2, float* db2,
+                                void* workspace, size_t workspace_bytes_given, void* stream) {
+  (void)b2;
+  g_launches = 0;
+  OSDP_TRY(check_desc_ffn(desc));
+  if (!X || !W1 || !b1 || !W2 || !dY || !dX || !dW1 || !db1 || !dW2 || !db2 || !workspace) return OSDP_ERR_NULL;
+  if (misaligned(X, 16) || misaligned(W1, 16) || misaligned(b1, 16) || misaligned(W2, 16) || misaligned(dY, 16) ||
+      misaligned(dX, 16) || misaligned(dW1, 16) || misaligned(db1, 16) || misaligned(dW2, 16) || misaligned(db2, 16))
+    return OSDP_ERR_ALIGN;
+  if (misaligned(workspace, 256) || workspace_bytes_given < ffn_workspace_bytes(desc, OSDP_BWD)) return OSDP_ERR_WORKSPACE;
+  if (desc->dtype == OSDP_BF16) OSDP_TRY(check_arch());
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t T = desc->tokens, h = desc->hidden, f = desc->ffn;
+  const size_t e = elem_size(desc->dtype);
+  const int dt = desc->dtype, k = desc->k;
+  const size_t buf = ffn_slice_buf_bytes(desc);
+  void* Zs = workspace;                                  // Z_s, then dZ_s in place       [T x fs]
+  void* Hs = (char*)workspace + buf;                     // H_s                           [T x fs]
+  float* dXacc = (float*)((char*)workspace + 2 * buf);   // fp32 accumulator of dX        [T x h]   (k > 1)
+  float* scratch = (float*)((char*)workspace + 2 * buf + ffn_acc_bytes(desc));
+
+  for (int s = 0; s < k; ++s) {
+    const int64_t lo = ffn_lo(desc, s), hi = ffn_lo(desc, s + 1);
+    const int fs = (int)(hi - lo);
+    if (fs == 0) continue;
+    const char* W1s = (const char*)W1 + (size_t)lo * e;           // W1[:, lo:hi], leading dimension f
+    const char* W2s = (const char*)W2 + (size_t)lo * h * e;       // W2[lo:hi, :]
+    // A3: Z_s = X W1[:, lo:hi] + b1[lo:hi], H_s = gelu(Z_s)
+    trace_set_step(3);
+    EpiParams e3 = {(const char*)b1 + (size_t)lo * e, Zs, Hs, nullptr, fs, 0};
+    OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_BIAS_GELU_DUAL>(dt, X, h, W1s, f, GemmShape{(int)T, fs, (int)h}, e3, st)));
+    // A4: dZ_s = (dY W2[lo:hi, :]^T) (.) gelu'(Z_s), in place over Z_s
+    trace_set_step(4);
+    EpiParams e4 = {nullptr, Zs, nullptr, Zs, fs, 0};
+    OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_DGELU>(dt, dY, h, W2s, h, GemmShape{(int)T, fs, (int)h}, e4, st)));
+    // A5: dW2[lo:hi, :] = H_s^T dY       -- rows of dW2 belong to exactly one slice: written once, no accumulation
+    trace_set_step(5);
+    EpiParams e5 = {nullptr, dW2 + (size_t)lo * h, nullptr, nullptr, h, 0};
+    OSDP_TRY((gemm<MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32>(dt, Hs, fs, dY, h, GemmShape{fs, (int)h, (int)T}, e5, st)));
+    // A8: db1[lo:hi] = colsum(dZ_s); db2 = colsum(dY) once, with the first slice
+    trace_set_step(8);
+    OSDP_TRY(colsum2(dt, dY, s == 0 ? (int)h : 0, db2, Zs, fs, db1 + lo, (int)T, scratch, 0, st));
+    // A6: dW1[:, lo:hi] = X^T dZ_s       -- columns of dW1 belong to exactly one slice
+    trace_set_step(6);
+    EpiParams e6 = {nullptr, dW1 + lo, nullptr, nullptr, f, 0};
+    OSDP_TRY((gemm<MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32>(dt, X, h, Zs, fs, GemmShape{(int)h, fs, (int)T}, e6, st)));
+    // A7: dX (+)= dZ_s W1[:, lo:hi]^T    -- the only result that spans slices
+    trace_set_step(7);
+    if (k == 1) {
+      EpiParams e7 = {nullptr, dX, nullptr, nullptr, h, 0};
+      OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_PLAIN>(dt, Zs, fs, W1s, f, GemmShape{(int)T, (int)h, fs}, e7, st)));
+    } else {
+      EpiParams e7 = {nullptr, dXacc, nullptr, nullptr, h, s == 0 ? 0 : 1};
+      OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_ACCUM_F32>(dt, Zs, fs, W1s, f, GemmShape{(int)T, (int)h, fs}, e7, st)));
+    }
+  }
+  if (k > 1) {   // dX = storage(dXacc)
+    trace_set_step(10);
+    OSDP_TRY(launch_acc_to_out(dt, dXacc, nullptr, dX, T, (int)h, sm100::num_sms(), st));
   }
   return OSDP_OK;
 }

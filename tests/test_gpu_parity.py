@@ -142,6 +142,86 @@ def test_tuning_rejects_bad_arguments(lib):
     assert lib.osdp_get_tuning(lib.OSDP_TUNE_MT2_MIN_K) == 4096 and lib.osdp_get_tuning(lib.OSDP_TUNE_WAVE_SYNC) == 1
 
 
+# ------------------------------------------------------------------ ffn-axis (paper-literal) split
+def run_gpu_ffn(lib, inp, k, dtype):
+    T, h = inp.X.shape
+    f = inp.W1.shape[1]
+    d = inp.to("cuda")
+    op = lib.SplitMlp(T, h, f, dtype, k, axis="ffn")
+    Y = op.forward(d.X, d.W1, d.b1, d.W2, d.b2)
+    g = op.backward(d.X, d.W1, d.b1, d.W2, d.dY)
+    torch.cuda.synchronize()
+    out = {"Y": Y}
+    out.update(g)
+    return {n: out[n].to(torch.float64).cpu().numpy() for n in NAMES}
+
+
+@pytest.mark.parametrize("T,h,f,k", [
+    (256, 256, 512, 1),
+    (256, 256, 512, 2),
+    (333, 136, 520, 3),       # ragged everywhere; 65 column units over 3 slices (176, 168, 176 columns)
+    (1000, 320, 1032, 4),
+    (130, 72, 264, 33),       # one 8-column unit per slice (k = ffn / 8)
+    (64, 8, 8, 1),
+    (1, 16, 24, 3),
+])
+def test_bf16_ffn_split_matches_oracle(lib, T, h, f, k):
+    inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=13)
+    ref = O.mlp_forward_backward(**inp.as_f64())
+    check(run_gpu_ffn(lib, inp, k, torch.bfloat16), ref, 2e-2, f"bf16 ffn split {T}x{h}x{f} k={k}")
+
+
+def test_bf16_ffn_split_big_tiles_match_oracle(lib, force_big_tiles):
+    inp = I.mlp_inputs(1000, 320, 1032, torch.bfloat16, seed=14)
+    ref = O.mlp_forward_backward(**inp.as_f64())
+    check(run_gpu_ffn(lib, inp, 3, torch.bfloat16), ref, 2e-2, "bf16 ffn split MT=2")
+
+
+def test_fp32_ffn_split_matches_oracle_and_is_split_invariant(lib):
+    c = I.CONFIGS["C1"]
+    inp = I.mlp_inputs(c["tokens"], c["hidden"], c["ffn"], torch.float32, seed=c["seed"])
+    ref = O.mlp_forward_backward(**inp.as_f64())
+    outs = {k: run_gpu_ffn(lib, inp, k, torch.float32) for k in (1, 2, 4, 3, 256)}
+    for k, got in outs.items():
+        check(got, ref, 1e-4, f"C1 ffn split k={k}")
+        for n in NAMES:
+            assert rel_err(got[n], outs[1][n]) <= 1e-5, (k, n)
+        for n in ("dW1", "db1", "dW2", "db2"):          # slices own disjoint parts of the weight gradients
+            assert np.array_equal(got[n], outs[1][n]), (k, n)
+
+
+def test_c2_ffn_split_matches_oracle_and_weight_grads_are_bit_identical_across_k(lib, c2):
+    inp, ref = c2
+    outs = {k: run_gpu_ffn(lib, inp, k, torch.bfloat16) for k in (1, 2, 4, 8)}
+    for k, got in outs.items():
+        check(got, ref, 2e-2, f"C2 ffn split k={k}")
+        for n in ("dW1", "db1", "dW2", "db2"):
+            assert np.array_equal(got[n], outs[1][n]), (k, n)
+    again = run_gpu_ffn(lib, inp, 8, torch.bfloat16)
+    for n in NAMES:
+        assert np.array_equal(again[n], outs[8][n]), n      # deterministic run to run
+
+
+def test_ffn_split_error_codes_and_workspace(lib):
+    T, h, f = 64, 64, 128
+    inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=1).to("cuda")
+    desc = lib.make_desc(T, h, f, torch.bfloat16, 4)
+    fwd, bwd = (lib.osdp_ffn_split_mlp_workspace_bytes(desc, p) for p in (lib.OSDP_FWD, lib.OSDP_BWD))
+    assert fwd == T * 32 * 2 + T * h * 4 and bwd == 2 * T * 32 * 2 + T * h * 4 + 32 * (h + f) * 4
+    assert lib.osdp_ffn_split_mlp_workspace_bytes(lib.make_desc(T, h, f, torch.bfloat16, 1), lib.OSDP_FWD) == T * f * 2
+    assert lib.osdp_ffn_split_mlp_workspace_bytes(lib.make_desc(T, h, f, torch.bfloat16, f // 8 + 1), lib.OSDP_FWD) == 0
+    ws = torch.empty(bwd, dtype=torch.uint8, device="cuda")
+    Y = torch.full_like(inp.X, 3.0)
+    args = (inp.X, inp.W1, inp.b1, inp.W2, inp.b2, Y, ws)
+    assert lib.osdp_ffn_split_mlp_forward(desc, *args, check=False) == lib.OSDP_OK
+    assert lib.osdp_ffn_split_mlp_forward(lib.make_desc(T, h, f, torch.bfloat16, T + 1), *args, check=False) == lib.OSDP_ERR_K
+    assert lib.osdp_ffn_split_mlp_forward(lib.make_desc(T, h, f, torch.bfloat16, 16), *args, check=False) == lib.OSDP_OK
+    assert lib.osdp_ffn_split_mlp_forward(lib.make_desc(T, h, f, torch.bfloat16, 0), *args, check=False) == lib.OSDP_ERR_K
+    assert lib.osdp_ffn_split_mlp_forward(desc, None, *args[1:], check=False) == lib.OSDP_ERR_NULL
+    assert lib.osdp_ffn_split_mlp_forward(desc, *args[:6], ws, workspace_bytes=64, check=False) == lib.OSDP_ERR_WORKSPACE
+    assert lib.osdp_last_launch_count() == 0
+
+
 # ------------------------------------------------------------------ C2: full oracle at every k
 @pytest.fixture(scope="module")
 def c2():

@@ -162,6 +162,25 @@ def test_paper_literal_contraction_split(g):
     assert np.allclose(O.matmul_contraction_split(X, W, g), ref, rtol=1e-13, atol=1e-13)
 
 
+@pytest.mark.parametrize("k,unit", [(1, 8), (2, 8), (3, 8), (5, 8), (6, 8), (4, 4), (12, 4)])
+def test_ffn_split_equals_unsplit(k, unit):
+    """The paper-literal split of the MLP pair along ffn: summed partial products == unsplit."""
+    d = _tiny(T=12, h=8, f=48, seed=12)
+    ref = O.mlp_forward_backward(**d)
+    got = O.mlp_forward_backward_ffn_split(**d, k=k, unit=unit)
+    for name in ref:
+        scale = np.max(np.abs(ref[name]))
+        assert np.max(np.abs(ref[name] - got[name])) <= 1e-13 * scale, name
+
+
+def test_ffn_slice_bounds_partition_in_whole_units():
+    for f, k, unit in ((48, 5, 8), (520, 3, 8), (1032, 4, 8), (68, 4, 4), (8, 1, 8), (64, 8, 8)):
+        b = O.ffn_slice_bounds(f, k, unit)
+        assert b[0][0] == 0 and b[-1][1] == f and all(b[i][1] == b[i + 1][0] for i in range(k - 1))
+        assert all(lo % unit == 0 and hi % unit == 0 and hi > lo for lo, hi in b)
+        assert max(hi - lo for lo, hi in b) == -(-(f // unit) // k) * unit
+
+
 # ---------------------------------------------------------------- sampled oracle == full oracle
 def test_sampled_oracle_is_a_restriction_of_the_full_one():
     d = _tiny(T=20, h=8, f=24, seed=13)
