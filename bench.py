@@ -248,9 +248,11 @@ class Workload:
         self.hY = e((self.T, self.h), dtype=self.dtype, pin_memory=True)
         self.hg = {n: e(t.shape, dtype=t.dtype, pin_memory=True) for n, t in self.g.items()}
 
-    def set_k(self, k):
-        self.k = k
-        self.op = self.lib.SplitMlp(self.T, self.h, self.f, self.dtype, k)
+    def set_k(self, k, axis="tokens"):
+        self.k, self.axis = k, axis
+        self.op = None
+        torch.cuda.empty_cache()
+        self.op = self.lib.SplitMlp(self.T, self.h, self.f, self.dtype, k, axis=axis)
 
     def step(self):
         d = self.dev
@@ -297,7 +299,7 @@ def timed_steps(fn, steps, world, flush=None):
     return sum(a.elapsed_time(b) for a, b in evs), wall
 
 
-def measure_peak_bytes(lib, cfg, k):
+def measure_peak_bytes(lib, cfg, k, axis="tokens"):
     """Peak device bytes of ONE forward call and ONE backward call, each with only its own tensors live,
     against the cost model (osdp_mlp_op_cost + osdp_cost_eval)."""
     from paper_2305_09940_b200 import inputs as I
@@ -312,24 +314,30 @@ def measure_peak_bytes(lib, cfg, k):
         desc = lib.make_desc(T, h, f, dt, k)
         mk = lambda *s, d=dt: torch.empty(s, dtype=d, device="cuda")
         X, W1, b1, W2, b2 = mk(T, h), mk(h, f), mk(f), mk(f, h), mk(h)
-        ws = torch.empty(lib.osdp_split_mlp_workspace_bytes(desc, pass_), dtype=torch.uint8, device="cuda")
+        ffn = axis == "ffn"
+        ws_bytes = (lib.osdp_ffn_split_mlp_workspace_bytes if ffn else lib.osdp_split_mlp_workspace_bytes)(desc, pass_)
+        ws = torch.empty(ws_bytes, dtype=torch.uint8, device="cuda")
         for t in (X, W1, b1, W2, b2):
             t.zero_()
         if pass_ == lib.OSDP_FWD:
             Y = mk(T, h)
-            lib.osdp_split_mlp_forward(desc, X, W1, b1, W2, b2, Y, ws)
+            (lib.osdp_ffn_split_mlp_forward if ffn else lib.osdp_split_mlp_forward)(desc, X, W1, b1, W2, b2, Y, ws)
         else:
             dY, dX = mk(T, h), mk(T, h)
             dY.zero_()
             f32 = torch.float32
             dW1, db1, dW2, db2 = mk(h, f, d=f32), mk(f, d=f32), mk(f, h, d=f32), mk(h, d=f32)
-            lib.osdp_split_mlp_backward(desc, X, W1, b1, W2, b2, dY, dX, dW1, db1, dW2, db2, ws)
+            (lib.osdp_ffn_split_mlp_backward if ffn else lib.osdp_split_mlp_backward)(
+                desc, X, W1, b1, W2, b2, dY, dX, dW1, db1, dW2, db2, ws)
         torch.cuda.synchronize()
         measured = torch.cuda.max_memory_allocated() - base
-        c = lib.osdp_mlp_op_cost(desc, pass_)
+        c = (lib.osdp_ffn_split_mlp_op_cost if ffn else lib.osdp_mlp_op_cost)(desc, pass_)
         dev = lib.osdp_device(1, 0.0, 0.0, 1 << 62)
         p, tr, _ = lib.osdp_cost_eval(c, lib.OSDP_DP, k, 1, dev)
-        out[name] = {"measured": int(measured), "model": int(p + tr), "workspace": int(ws.numel())}
+        model = int(p + tr)
+        if ffn and k == 1:       # the variant's cost factors describe k > 1; at k = 1 there is no fp32 accumulator
+            model -= (T * h * 4 + 255) // 256 * 256
+        out[name] = {"measured": int(measured), "model": model, "workspace": int(ws.numel())}
         del X, W1, b1, W2, b2, ws
         if pass_ == lib.OSDP_FWD:
             del Y
@@ -435,22 +443,26 @@ def main():
                "h2d_bytes_per_step": wl.h2d_bytes(), "d2h_bytes_per_step": wl.d2h_bytes()}
 
     # ---- per-k table: TFLOP/s and peak bytes vs the cost model (rank 0, N = 1 only)
-    per_k = None
+    per_k = per_k_ffn = None
     if not args.no_sweep and world == 1 and cfg.get("ks"):
-        per_k = []
-        for k in cfg["ks"]:
-            wl.set_k(k)
-            for _ in range(2):
-                wl.step()
-            s_ms, _ = timed_steps(wl.step, max(3, args.steps // 2), 1, flush)
-            s_ms /= max(3, args.steps // 2)
-            per_k.append({"k": k, "ms_per_step": s_ms, "tflops": flops / (s_ms * 1e-3) / 1e12,
-                          "frac_of_sustained_peak": flops / (s_ms * 1e-3) / 1e12 / peak if peak else None})
+        tables = {"tokens": [], "ffn": []}       # "ffn": the paper-literal split (osdp_ffn_split_mlp_*), DESIGN.md section 10
+        n_sw = max(3, args.steps // 2)
+        for axis, tab in tables.items():
+            for k in cfg["ks"]:
+                wl.set_k(k, axis)
+                for _ in range(2):
+                    wl.step()
+                s_ms, _ = timed_steps(wl.step, n_sw, 1, flush)
+                s_ms /= n_sw
+                tab.append({"k": k, "ms_per_step": s_ms, "tflops": flops / (s_ms * 1e-3) / 1e12,
+                            "frac_of_sustained_peak": flops / (s_ms * 1e-3) / 1e12 / peak if peak else None})
         wl.set_k(args.k)
         del wl
         torch.cuda.empty_cache()
-        for ent in per_k:
-            ent["peak_bytes"] = measure_peak_bytes(lib, cfg, ent["k"])
+        for axis, tab in tables.items():
+            for ent in tab:
+                ent["peak_bytes"] = measure_peak_bytes(lib, cfg, ent["k"], axis)
+        per_k, per_k_ffn = tables["tokens"], tables["ffn"]
     cpu = None
     if not args.no_cpu_baseline and rank == 0 and world == 1:
         r = time_oracle(cfg, 1, 0)
@@ -467,7 +479,8 @@ def main():
                 "frac_of_sustained_peak": value / world / peak if peak else None,
                 "frac_of_nominal_peak": value / world / NOMINAL_BF16_TFLOPS,
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches) * args.steps,
-                "roofline": roofline, "kernels": kernels, "per_k": per_k, "cpu_baseline": cpu,
+                "roofline": roofline, "kernels": kernels, "per_k": per_k, "per_k_ffn_split": per_k_ffn,
+                "cpu_baseline": cpu,
                 "wall_ms_timed_region": wall_ms}
         print(json.dumps(line), flush=True)
     D.finalize()

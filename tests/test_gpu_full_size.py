@@ -27,20 +27,23 @@ def sample_indices(T, k, f, seed=0):
     return sorted(rows), sorted(cols)
 
 
-def check_sampled(lib, inp, x64, ks, what, refs=None):
+def check_sampled(lib, inp, x64, ks, what, refs=None, axis="tokens"):
     T, h = inp.X.shape
     f = inp.W1.shape[1]
     d = inp.to("cuda")
     cache = {}
     for k in ks:
         rows, cols = sample_indices(T, k, f)
+        if axis == "ffn":      # first/last columns of ffn slices as well
+            fb = O.ffn_slice_bounds(f, k, 8)
+            cols = sorted(set(cols) | {fb[0][1] - 1, fb[-1][0], fb[k // 2][0], fb[k // 2][1] - 1})
         key = (tuple(rows), tuple(cols))
         if key not in cache:
             cache[key] = (O.sampled_rows(x64["X"], x64["W1"], x64["b1"], x64["W2"], x64["b2"], x64["dY"], rows),
                           O.sampled_cols(x64["X"], x64["W1"], x64["b1"], x64["W2"], x64["dY"], cols),
                           O.db2_full(x64["dY"]))
         r, c, db2 = cache[key]
-        op = lib.SplitMlp(T, h, f, torch.bfloat16, k)
+        op = lib.SplitMlp(T, h, f, torch.bfloat16, k, axis=axis)
         Y = op.forward(d.X, d.W1, d.b1, d.W2, d.b2)
         g = op.backward(d.X, d.W1, d.b1, d.W2, d.dY)
         torch.cuda.synchronize()
@@ -68,6 +71,13 @@ def test_c4_sampled_oracle_bench_config_and_extremes(lib):
     c = I.CONFIGS["C4"]
     inp = I.mlp_inputs(c["tokens"], c["hidden"], c["ffn"], torch.bfloat16, seed=c["seed"])
     check_sampled(lib, inp, inp.as_f64(), (4, 1, 32), "C4")          # k = 4 is what bench.py times
+
+
+def test_c4_ffn_split_sampled_oracle(lib):
+    """The ffn-axis (paper-literal) split at the gigantic-operator config, unsplit and at the two extremes bench.py reports."""
+    c = I.CONFIGS["C4"]
+    inp = I.mlp_inputs(c["tokens"], c["hidden"], c["ffn"], torch.bfloat16, seed=c["seed"])
+    check_sampled(lib, inp, inp.as_f64(), (4, 32), "C4 ffn split", axis="ffn")
 
 
 def test_c4_token_downscaled_full_oracle(lib):
@@ -159,3 +169,23 @@ def test_peak_bytes_within_5pct_of_cost_model(lib, cfg, ks):
             assert abs(m - model) <= 0.05 * model, (cfg, k, name, pk)
             e = 4 if c["dtype"] == "f32" else 2
             assert pk[name]["workspace"] == P.mlp_workspace_bytes(c["tokens"], c["hidden"], c["ffn"], e, k, name == "bwd")
+
+
+@pytest.mark.parametrize("cfg,ks", [("C4", (1, 4, 32)), ("C2", (2, 8))])
+def test_ffn_split_peak_bytes_within_5pct_of_cost_model(lib, cfg, ks):
+    """Peak device bytes of the ffn-axis split: caller tensors + [T x ceil(f/k)] slice buffers + the fp32 [T x h]
+    accumulator (k > 1) + scratch, against osdp_ffn_split_mlp_op_cost + osdp_cost_eval."""
+    import bench
+    c = I.CONFIGS[cfg]
+    T, h, f = c["tokens"], c["hidden"], c["ffn"]
+    for k in ks:
+        pk = bench.measure_peak_bytes(lib, c, k, axis="ffn")
+        for name in ("fwd", "bwd"):
+            m, model = pk[name]["measured"], pk[name]["model"]
+            assert abs(m - model) <= 0.05 * model, (cfg, k, name, pk)
+            fs = -(-(f // 8) // k) * 8
+            bufs = (2 if name == "bwd" else 1) * ((T * fs * 2 + 255) // 256 * 256)
+            acc = 0 if k == 1 else (T * h * 4 + 255) // 256 * 256
+            scratch = P.mlp_reduce_scratch_bytes(h, f) if name == "bwd" else 0
+            assert pk[name]["workspace"] == bufs + acc + scratch
+
