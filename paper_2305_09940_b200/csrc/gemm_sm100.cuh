@@ -2,22 +2,24 @@
 //
 //   C[M x N] = A[M x K] * B[K x N]   (bf16 x bf16 -> fp32 in TMEM), then a fused epilogue (common.cuh Epi).
 //
-// Structure: persistent CTA PAIRS (cluster of 2 = one TPC, one CTA per SM, 256 threads each, warp-specialised).
-// A pair computes one 256 x 256 output tile with tcgen05.mma.cta_group::2 (UMMA 256 x 256 x 16): CTA r of the
-// pair owns rows [128 r, 128 r + 128) of the tile (its TMEM lanes) and stages its own 128 A-rows plus ONE HALF
-// (128 columns) of the B tile, so every B byte is fetched from L2 and written to shared memory once per pair.
+// Structure: persistent CTA PAIRS (cluster of 2 = one TPC, one CTA per SM, 384 threads each, warp-specialised).
+// Every MMA is tcgen05.mma.cta_group::2 (UMMA 256 x 256 x 16): CTA r of the pair supplies 128 A-rows (its TMEM
+// lanes) and ONE HALF (128 columns) of the B tile, so every B byte is fetched from L2 and written to shared memory
+// once per pair.  A CTA owns MT such row halves: MT = 1 -> 256 x 256 pair tiles, two TMEM accumulator stages
+// (epilogue overlapped); MT = 2 -> 512 x 256 pair tiles, one stage, 25 % less operand traffic (TileCfg below).
 //   warp 0      TMA producer (both CTAs): cp.async.bulk.tensor.cta_group::2 (128B-swizzled boxes) into a
-//               kStages-deep smem ring; both CTAs' loads complete_tx on the LEADER's full barrier
-//   warp 1      MMA issuer (leader CTA only): one lane issues the UMMAs from smem descriptors into one of two
-//               256-column TMEM accumulator stages; tcgen05.commit (multicast to both CTAs) frees the smem
-//               slots and publishes finished accumulators
+//               kStages-deep smem ring; both CTAs' loads complete_tx on the LEADER's full barrier; lines up with
+//               the other pairs at tile boundaries (wave sync, MT = 2)
+//   warp 1      MMA issuer (leader CTA only): one lane issues the UMMAs from smem descriptors into TMEM;
+//               tcgen05.commit (multicast to both CTAs) frees the smem slots and publishes finished accumulators
 //   warp 2      TMEM allocator (512 columns, cta_group::2) / deallocator
-//   warps 4..7  epilogue: tcgen05.ld (32 lanes x 32 columns per warp), bias / GeLU / GeLU' in fp32, then the
-//               warp's 32 rows x 128 B output segment goes to a 128B-swizzled smem staging buffer and out
-//               through TMA (cp.async.bulk.tensor store; cp.reduce.async.bulk.tensor .add for the fp32
-//               cross-slice accumulation of dW); overlaps the next tile's main loop through the second
-//               accumulator stage
-// Three mbarrier pipelines: smem full/empty (TMA <-> MMA), TMEM full/empty (MMA <-> epilogue).
+//   warps 4..11 epilogue, two per TMEM lane quarter on alternate column chunks: tcgen05.ld (32 lanes x 32 columns),
+//               bias / GeLU / GeLU' in fp32, then the warp's 32 rows x 128 B output segment goes to a 128B-swizzled
+//               smem staging buffer and out through TMA (cp.async.bulk.tensor store; cp.reduce.async.bulk.tensor
+//               .add for fp32 cross-slice accumulation)
+// Three mbarrier pipelines: smem full/empty (TMA <-> MMA), TMEM full/empty (MMA <-> epilogue).  Launched with
+// programmatic stream serialization: the set-up overlaps the previous kernel's tail (griddepcontrol).
+// Optionally CM x CN pairs form one cluster and TMA-multicast the operand tiles they share (off by default).
 //
 // Operand majorness: both K-major and MN-major operands are supported directly by
 // the UMMA shared-memory descriptors, so the dW GEMMs (A = H_s^T, X_s^T; B = dY_s, dZ_s) need no transposes.
