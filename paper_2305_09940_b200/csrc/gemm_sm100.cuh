@@ -355,17 +355,19 @@ __device__ __forceinline__ unsigned int atom_add_release_gpu(unsigned int* p, un
   asm volatile("atom.add.release.gpu.global.u32 %0, [%1], %2;" : "=r"(old) : "l"(p), "r"(x) : "memory");
   return old;
 }
-__device__ __forceinline__ void wave_wait(const unsigned int* ctr, unsigned int target) {
-  uint64_t t0 = 0;
+// The sync is a performance hint, never a correctness requirement, and it must not become a deadlock: two such
+// launches running concurrently on different streams can each hold SMs the other one's missing CTAs need.  So a
+// wait gives up after ~200 us (tiles take 50-120 us; a healthy wait is a few us) and returns false; the caller
+// then stops waiting for the rest of the launch but keeps announcing, so the counter still balances.
+__device__ __forceinline__ bool wave_wait(const unsigned int* ctr, unsigned int target) {
+  if (ld_acquire_gpu(ctr) >= target) return true;
+  const uint64_t t0 = global_timer_ns();
   uint32_t spins = 0;
   while (ld_acquire_gpu(ctr) < target) {
     __nanosleep(64);
-    if ((++spins & 0x3FFu) == 0) {
-      const uint64_t now = global_timer_ns();
-      if (t0 == 0) t0 = now;
-      else if (now - t0 > 20ull * 1000 * 1000 * 1000) __trap();
-    }
+    if ((++spins & 0x3Fu) == 0 && global_timer_ns() - t0 > 200ull * 1000) return false;
   }
+  return true;
 }
 
 // ------------------------------------------------------------------------------------------------- the kernel
@@ -474,14 +476,14 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
     int dbg_filled = 0;
 #endif
     int it = 0;
+    bool waiting = true;   // false once a wait has timed out (see wave_wait)
     for (int t = cluster_id; t < num_tiles; t += num_clusters, ++it) {
       // Sync points of a tile: before k-blocks sync_kb, 2 sync_kb, ... (if sync_kb > 0) and after the last one.
       const unsigned int syncs_per_tile = 1u + (sync_kb > 0 ? (unsigned int)((num_kb - 1) / sync_kb) : 0u);
       const unsigned int sync_base = (unsigned int)it * syncs_per_tile * (unsigned int)num_clusters;   // earlier waves were full
       const unsigned int active = (unsigned int)min(num_clusters, num_tiles - it * num_clusters);       // clusters in this wave
-      if (wave_sync != nullptr && it > 0) {   // every cluster has issued the loads of its previous tile
-        if (lane == 0) wave_wait(wave_sync, sync_base);
-        __syncwarp();
+      if (wave_sync != nullptr && waiting && it > 0) {   // every cluster has issued the loads of its previous tile
+        waiting = __shfl_sync(0xFFFFFFFFu, lane == 0 ? (int)wave_wait(wave_sync, sync_base) : 0, 0) != 0;
       }
       const TileCoord tc = tile_coord(t, num_cm, num_cn, group_m);
       int m0 = (tc.m_blk * CM + pi) * kPairM + (int)rank * kCtaM;       // this CTA's rows of A
@@ -496,11 +498,12 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
 #endif
       for (int kb = 0; kb < num_kb; ++kb) {
         if (wave_sync != nullptr && sync_kb > 0 && kb > 0 && kb % sync_kb == 0) {   // stay in step inside the tile too
+          int ok = 1;
           if (lane == 0) {
             if (crank == 0) atom_add_release_gpu(wave_sync, 1u);
-            wave_wait(wave_sync, sync_base + (unsigned int)(kb / sync_kb) * active);
+            if (waiting) ok = (int)wave_wait(wave_sync, sync_base + (unsigned int)(kb / sync_kb) * active);
           }
-          __syncwarp();
+          waiting = waiting && __shfl_sync(0xFFFFFFFFu, ok, 0) != 0;
         }
         mbar_wait(empty_bar + 8 * stage, phase ^ 1);   // the slot is free in every CTA of the cluster
 #ifdef OSDP_DBG_NOLOAD   // probe: after the ring has been filled once, re-use its contents (no L2->SM traffic)

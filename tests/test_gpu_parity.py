@@ -133,6 +133,29 @@ def test_bf16_tile_shapes_and_wave_sync_agree_bitwise(lib, force_big_tiles):
     check(outs[0], O.mlp_forward_backward(**inp.as_f64()), 2e-2, "bf16 MT=2 several waves")
 
 
+def test_two_streams_with_wave_sync_do_not_deadlock(lib, force_big_tiles):
+    """Two multi-wave MT = 2 launches in flight on different streams can each hold SMs the other one's missing CTAs
+    need; the wave sync must give up instead of waiting for ever, and the results must not change."""
+    T, h, f = 5200, 1288, 5144
+    inps = [I.mlp_inputs(T, h, f, torch.bfloat16, seed=s) for s in (20, 21)]
+    want = [run_gpu(lib, inp, 1, torch.bfloat16) for inp in inps]
+    devs = [inp.to("cuda") for inp in inps]
+    ops = [lib.SplitMlp(T, h, f, torch.bfloat16, 1) for _ in inps]
+    streams = [torch.cuda.Stream() for _ in inps]
+    torch.cuda.synchronize()
+    outs = [None, None]
+    for _ in range(3):
+        for i, (d, op, st) in enumerate(zip(devs, ops, streams)):
+            with torch.cuda.stream(st):
+                Y = op.forward(d.X, d.W1, d.b1, d.W2, d.b2, stream=st)
+                g = op.backward(d.X, d.W1, d.b1, d.W2, d.dY, stream=st)
+            outs[i] = dict(Y=Y, **g)
+    torch.cuda.synchronize()
+    for o, w in zip(outs, want):
+        for n in NAMES:
+            assert np.array_equal(o[n].double().cpu().numpy(), w[n]), n
+
+
 def test_tuning_rejects_bad_arguments(lib):
     assert lib.osdp_set_tuning(99, 1, check=False) == lib.OSDP_ERR_ARG
     assert lib.osdp_set_tuning(lib.OSDP_TUNE_WAVE_SYNC, -1, check=False) == lib.OSDP_ERR_ARG
