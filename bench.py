@@ -347,6 +347,19 @@ def measure_peak_bytes(lib, cfg, k, axis="tokens"):
     return out
 
 
+def fit_gamma_delta(table):
+    """Device information for the planner ("profiled in advance"), from the per-k sweep: the cost model's
+    T(k) = gamma + (k - 1) delta (reading P2) with gamma = the measured k = 1 time and delta the least-squares
+    slope through it; max_rel_residual says how well the linear model holds."""
+    t1 = next((e["ms_per_step"] for e in table if e["k"] == 1), None)
+    pts = [(e["k"] - 1, e["ms_per_step"] - t1) for e in table if e["k"] > 1] if t1 is not None else []
+    if not pts:
+        return None
+    delta = sum(x * y for x, y in pts) / sum(x * x for x, _ in pts)
+    resid = max(abs(t1 + x * delta - (t1 + y)) / (t1 + y) for x, y in pts)
+    return {"gamma_s": t1 * 1e-3, "delta_s": delta * 1e-3, "max_rel_residual": resid}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -443,7 +456,7 @@ def main():
                "h2d_bytes_per_step": wl.h2d_bytes(), "d2h_bytes_per_step": wl.d2h_bytes()}
 
     # ---- per-k table: TFLOP/s and peak bytes vs the cost model (rank 0, N = 1 only)
-    per_k = per_k_ffn = None
+    per_k = per_k_ffn = cost_fit = None
     if not args.no_sweep and world == 1 and cfg.get("ks"):
         tables = {"tokens": [], "ffn": []}       # "ffn": the paper-literal split (osdp_ffn_split_mlp_*), DESIGN.md section 10
         n_sw = max(3, args.steps // 2)
@@ -463,6 +476,7 @@ def main():
             for ent in tab:
                 ent["peak_bytes"] = measure_peak_bytes(lib, cfg, ent["k"], axis)
         per_k, per_k_ffn = tables["tokens"], tables["ffn"]
+        cost_fit = {axis: fit_gamma_delta(tab) for axis, tab in tables.items()}
     cpu = None
     if not args.no_cpu_baseline and rank == 0 and world == 1:
         r = time_oracle(cfg, 1, 0)
@@ -479,7 +493,7 @@ def main():
                 "frac_of_sustained_peak": value / world / peak if peak else None,
                 "frac_of_nominal_peak": value / world / NOMINAL_BF16_TFLOPS,
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches) * args.steps,
-                "roofline": roofline, "kernels": kernels, "per_k": per_k, "per_k_ffn_split": per_k_ffn,
+                "roofline": roofline, "kernels": kernels, "per_k": per_k, "per_k_ffn_split": per_k_ffn, "cost_model_fit": cost_fit,
                 "cpu_baseline": cpu,
                 "wall_ms_timed_region": wall_ms}
         print(json.dumps(line), flush=True)

@@ -215,6 +215,23 @@ int osdp_plan(const osdp_op_cost* ops, int32_t n, const osdp_device* dev, int64_
               const int32_t* k_candidates, int32_t n_cand,
               int32_t* k_out, int32_t* mode_out, double* est_seconds, uint64_t* est_peak_bytes);
 
+/* Slice-level mode mixing ("partition the operator into 4 slices and process 1 of them in the ZDP
+ * mode and 3 of them in the DP mode ... a more fine-grained execution plan").  An operator cut into k slices runs
+ * zdp_slices of them in ZDP mode and the rest in DP mode (reading P10): each slice carries 1/k of the operator's
+ * model states and parameters, so
+ *   persist   = (model - zs) + ceil(zs / N) + batch*act + extra_fixed + ceil(extra_summed / k),  zs = ceil(model*zdp_slices / k)
+ *   transient = ceil(extra_transient / k)
+ *   seconds   = (2 + zdp_slices/k) (N-1)(alpha + S beta/N) + batch*gamma + (k-1) delta
+ * zdp_slices = 0 / = k are osdp_cost_eval's DP / ZDP values exactly.  OSDP_ERR_ARG unless 0 <= zdp_slices <= k.
+ * osdp_plan_mixed searches per operator over k in k_candidates (each <= 1024) x zdp_slices in 0..k, options ordered
+ * k ascending then zdp_slices ascending, otherwise exactly like osdp_plan (same prunings, strict "<", first optimum
+ * in traversal order).  Its optimum is never slower than osdp_plan's (a superset of plans). */
+int osdp_cost_eval_mixed(const osdp_op_cost* op, int32_t k, int32_t zdp_slices, int64_t batch, const osdp_device* dev,
+                         uint64_t* persist_bytes, uint64_t* transient_bytes, double* seconds);
+int osdp_plan_mixed(const osdp_op_cost* ops, int32_t n, const osdp_device* dev, int64_t batch,
+                    const int32_t* k_candidates, int32_t n_cand,
+                    int32_t* k_out, int32_t* zdp_slices_out, double* est_seconds, uint64_t* est_peak_bytes);
+
 /* Scheduler (Algorithm 1 in full): batch = 1, 2, 3, ... up to batch_max; stops at the first
  * batch with no feasible plan; returns the candidate minimising est_seconds / batch (Eq. 1) in *batch_out. */
 int osdp_plan_batch(const osdp_op_cost* ops, int32_t n, const osdp_device* dev, int64_t batch_max,

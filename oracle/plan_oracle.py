@@ -22,6 +22,7 @@ Follows the paper step by step:
   (reading P9): every T_i is rounded once to an integer count of picoseconds, floor(T_i * 1e12 + 0.5),
   and plan times are exact integer sums of those.
 * Infeasible (Algorithm 1 lines 12-14): returns None.
+* Slice-level mode mixing (reading P10): cost_eval_mixed / plan_brute_force_mixed.
 * Batch loop (Algorithm 1 lines 3-20, reading f3): b = 1, 2, 3, ...; stop at the first b with no feasible
   plan; return the candidate minimising T(b)/b (Eq. 1's objective is the per-sample time).
 
@@ -103,6 +104,42 @@ def plan_brute_force(ops, dev: Device, b: int, k_candidates):
         if mem <= dev.mem_limit and t < best_t:
             best_t = t
             best = (modes, ks, t, mem)
+    return best
+
+
+# ----- slice-level mode mixing (reading P10) --------------------------------------------------
+def cost_eval_mixed(op: OpCost, k: int, z: int, b: int, dev: Device):
+    """An operator partitioned into k slices, z of them processed in ZDP mode and k - z in DP mode ("partition the
+    operator into 4 slices and process 1 of them in the ZDP mode and 3 of them in the DP mode").
+    Every slice holds 1/k of the model states and moves 1/k of the parameters: the ZDP slices' share of the model
+    states, ceil(model z / k), is divided by N, the rest is replicated; a DP slice costs
+    2 collectives over its S/k bytes and a ZDP slice 3, with the latency term alpha shared in the
+    same proportion, so the operator's factor is (2 (k - z) + 3 z) / k = 2 + z / k."""
+    assert 0 <= z <= k
+    zdp_share = ceil_div(op.model * z, k)
+    model = (op.model - zdp_share) + ceil_div(zdp_share, dev.N)
+    persist = model + b * op.act + op.extra_fixed + ceil_div(op.extra_summed, k)
+    transient = ceil_div(op.extra_transient, k)
+    c = (2.0 * (k - z) + 3.0 * z) / k
+    t = c * (dev.N - 1) * (dev.alpha + op.S * dev.beta / dev.N) + b * op.gamma + (k - 1) * op.delta
+    return persist, transient, t
+
+
+def plan_brute_force_mixed(ops, dev: Device, b: int, k_candidates):
+    """Full enumeration over (k, z) per operator, k ascending then z ascending, strict '<' (first optimum wins).
+    Returns (ks, zs, picoseconds, peak_bytes) or None."""
+    options = [(k, z) for k in k_candidates for z in range(k + 1)]
+    best, best_t = None, math.inf
+    for choice in itertools.product(range(len(options)), repeat=len(ops)):
+        tot, tr, t = 0, 0, 0
+        for op, c in zip(ops, choice):
+            p, x, ti = cost_eval_mixed(op, options[c][0], options[c][1], b, dev)
+            tot += p
+            tr = max(tr, x)
+            t += to_ps(ti)
+        if tot + tr <= dev.mem_limit and t < best_t:
+            best_t = t
+            best = ([options[c][0] for c in choice], [options[c][1] for c in choice], t, tot + tr)
     return best
 
 

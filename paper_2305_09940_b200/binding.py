@@ -33,7 +33,7 @@ EXPORTS = (
     "osdp_split_mlp_forward", "osdp_split_mlp_backward", "osdp_last_launch_count", "osdp_cost_eval",
     "osdp_mlp_op_cost", "osdp_plan", "osdp_plan_batch", "osdp_trace_enable", "osdp_trace_read", "osdp_step_name",
     "osdp_set_tuning", "osdp_get_tuning", "osdp_ffn_split_mlp_workspace_bytes", "osdp_ffn_split_mlp_forward",
-    "osdp_ffn_split_mlp_backward", "osdp_ffn_split_mlp_op_cost",
+    "osdp_ffn_split_mlp_backward", "osdp_ffn_split_mlp_op_cost", "osdp_cost_eval_mixed", "osdp_plan_mixed",
 )
 
 
@@ -80,6 +80,11 @@ _lib.osdp_plan.restype = C.c_int
 _lib.osdp_plan.argtypes = [C.POINTER(osdp_op_cost), C.c_int32, C.POINTER(osdp_device), C.c_int64,
                            C.POINTER(C.c_int32), C.c_int32, C.POINTER(C.c_int32), C.POINTER(C.c_int32),
                            C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
+_lib.osdp_cost_eval_mixed.restype = C.c_int
+_lib.osdp_cost_eval_mixed.argtypes = [C.POINTER(osdp_op_cost), C.c_int32, C.c_int32, C.c_int64, C.POINTER(osdp_device),
+                                      C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_double)]
+_lib.osdp_plan_mixed.restype = C.c_int
+_lib.osdp_plan_mixed.argtypes = _lib.osdp_plan.argtypes
 _lib.osdp_plan_batch.restype = C.c_int
 _lib.osdp_plan_batch.argtypes = [C.POINTER(osdp_op_cost), C.c_int32, C.POINTER(osdp_device), C.c_int64,
                                  C.POINTER(C.c_int32), C.c_int32, C.POINTER(C.c_int32), C.POINTER(C.c_int32),
@@ -279,6 +284,32 @@ def osdp_plan(ops, dev: osdp_device, batch: int, k_candidates, check=True):
     if st != OSDP_OK:
         return st, None, None, None, None
     return st, list(ks), list(modes), float(sec.value), int(peak.value)
+
+
+def osdp_cost_eval_mixed(op: osdp_op_cost, k: int, zdp_slices: int, batch: int, dev: osdp_device, check=True):
+    """(persist_bytes, transient_bytes, seconds) of an operator with zdp_slices of its k slices in ZDP mode."""
+    p, t, s = C.c_uint64(), C.c_uint64(), C.c_double()
+    st = _lib.osdp_cost_eval_mixed(C.byref(op), k, zdp_slices, batch, C.byref(dev), C.byref(p), C.byref(t), C.byref(s))
+    if st != OSDP_OK:
+        if check:
+            raise OsdpError(st, "osdp_cost_eval_mixed")
+        return st
+    return int(p.value), int(t.value), float(s.value)
+
+
+def osdp_plan_mixed(ops, dev: osdp_device, batch: int, k_candidates, check=True):
+    """Returns (status, ks, zdp_slices, est_seconds, est_peak_bytes)."""
+    n = len(ops)
+    cand = (C.c_int32 * len(k_candidates))(*k_candidates)
+    ks, zs = (C.c_int32 * n)(), (C.c_int32 * n)()
+    sec, peak = C.c_double(), C.c_uint64()
+    st = _lib.osdp_plan_mixed(_op_array(ops), n, C.byref(dev), batch, cand, len(k_candidates), ks, zs, C.byref(sec),
+                              C.byref(peak))
+    if check and st not in (OSDP_OK, OSDP_ERR_INFEASIBLE):
+        raise OsdpError(st, "osdp_plan_mixed")
+    if st != OSDP_OK:
+        return st, None, None, None, None
+    return st, list(ks), list(zs), float(sec.value), int(peak.value)
 
 
 def osdp_plan_batch(ops, dev: osdp_device, batch_max: int, k_candidates, check=True):

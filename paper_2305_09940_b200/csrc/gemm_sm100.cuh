@@ -316,6 +316,9 @@ struct StorePipe {
   uint32_t buf;     // smem address of this warp's buffer
   int lane;
   __device__ __forceinline__ void begin() const {
+#ifdef OSDP_DBG_NOSTORE
+    return;
+#endif
     if (lane == 0) bulk_wait_read<0>();   // the previous store has read the buffer out
     __syncwarp();
   }
@@ -323,6 +326,9 @@ struct StorePipe {
     st_shared_v4(buf + lane * 128 + ((j ^ (lane & 7)) << 4), v);
   }
   __device__ __forceinline__ void commit(const CUtensorMap* map, int c_inner, int c_outer, bool reduce_add) const {
+#ifdef OSDP_DBG_NOSTORE   // probe: stage in smem (keeps the math alive) but never issue the TMA store
+    return;
+#endif
     fence_proxy_async_smem();   // generic-proxy writes -> visible to the async proxy (TMA)
     __syncwarp();
     if (lane == 0) {

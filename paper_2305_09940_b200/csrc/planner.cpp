@@ -27,19 +27,50 @@ struct OptionCost {
   int64_t ps;
 };
 
-bool eval(const osdp_op_cost& op, int mode, int32_t k, int64_t batch, const osdp_device& dev,
-          uint64_t* persist, uint64_t* transient, double* seconds) {
-  if (k < 1 || batch < 0 || dev.N < 1 || (mode != OSDP_DP && mode != OSDP_ZDP)) return false;
-  const uint64_t model = (mode == OSDP_ZDP) ? ceil_div_u64(op.model_bytes, (uint64_t)dev.N) : op.model_bytes;
+// One operator cut into k slices of which z run in ZDP mode and k - z in DP mode ("partition the
+// operator into 4 slices and process 1 of them in the ZDP mode and 3 of them in the DP mode"; reading P10).
+// Each slice carries 1/k of the operator's parameters and model states: the ZDP slices hold ceil(model z / k)
+// bytes, sharded N ways; communication is 2 collectives' worth for a DP slice and 3 for a ZDP slice
+// (PAPER.md:92-94), i.e. (2 + z/k) (N-1)(alpha + S beta / N) for the operator.  z = 0 and z = k are the
+// paper's pure DP and ZDP formulas exactly.
+bool eval_mixed(const osdp_op_cost& op, int32_t k, int32_t z, int64_t batch, const osdp_device& dev,
+                uint64_t* persist, uint64_t* transient, double* seconds) {
+  if (k < 1 || z < 0 || z > k || batch < 0 || dev.N < 1) return false;
+  const uint64_t zdp_share = (uint64_t)(((unsigned __int128)op.model_bytes * (uint64_t)z + (uint64_t)k - 1) / (uint64_t)k);
+  const uint64_t model = (op.model_bytes - zdp_share) + ceil_div_u64(zdp_share, (uint64_t)dev.N);
   if (persist)
     *persist = model + (uint64_t)batch * op.act_bytes + op.extra_fixed + ceil_div_u64(op.extra_summed, (uint64_t)k);
   if (transient) *transient = ceil_div_u64(op.extra_transient, (uint64_t)k);
   if (seconds) {
-    const double c = (mode == OSDP_ZDP) ? 3.0 : 2.0;
+    const double c = 2.0 + (double)z / (double)k;
     *seconds = c * (double)(dev.N - 1) * (dev.alpha + op.S * dev.beta / (double)dev.N) +
                (double)batch * op.gamma + (double)(k - 1) * op.delta;
   }
   return true;
+}
+
+bool eval(const osdp_op_cost& op, int mode, int32_t k, int64_t batch, const osdp_device& dev,
+          uint64_t* persist, uint64_t* transient, double* seconds) {
+  if (mode != OSDP_DP && mode != OSDP_ZDP) return false;
+  return eval_mixed(op, k, mode == OSDP_ZDP ? k : 0, batch, dev, persist, transient, seconds);
+}
+
+struct Option {
+  int32_t k, z;   // k slices, z of them in ZDP mode
+};
+// Pure modes, in the order of reading P5: DP before ZDP, k ascending.
+std::vector<Option> pure_options(const int32_t* cand, int32_t n_cand) {
+  std::vector<Option> o;
+  for (int m = 0; m < 2; ++m)
+    for (int i = 0; i < n_cand; ++i) o.push_back({cand[i], m == 0 ? 0 : cand[i]});
+  return o;
+}
+// Slice-level mixing, in the order of reading P10: k ascending, then z ascending (least split, DP-most first).
+std::vector<Option> mixed_options(const int32_t* cand, int32_t n_cand) {
+  std::vector<Option> o;
+  for (int i = 0; i < n_cand; ++i)
+    for (int32_t z = 0; z <= cand[i]; ++z) o.push_back({cand[i], z});
+  return o;
 }
 
 inline int64_t to_ps(double seconds) { return (int64_t)std::floor(seconds * kPsPerSecond + 0.5); }
@@ -118,16 +149,16 @@ struct Search {
 };
 
 int run_search(const osdp_op_cost* ops, int32_t n, const osdp_device* dev, int64_t batch,
-               const int32_t* cand, int32_t n_cand, Search& S) {
+               const std::vector<Option>& options, Search& S) {
   S.n = n;
-  S.n_opt = 2 * n_cand;
+  S.n_opt = (int)options.size();
   S.limit = dev->mem_limit_bytes;
   S.cost.resize((size_t)n * S.n_opt);
   for (int i = 0; i < n; ++i)
     for (int o = 0; o < S.n_opt; ++o) {
       OptionCost& oc = S.cost[(size_t)i * S.n_opt + o];
       double sec = 0;
-      if (!eval(ops[i], o / n_cand, cand[o % n_cand], batch, *dev, &oc.persist, &oc.transient, &sec))
+      if (!eval_mixed(ops[i], options[o].k, options[o].z, batch, *dev, &oc.persist, &oc.transient, &sec))
         return OSDP_ERR_ARG;
       if (!(sec >= 0) || sec > 9e6) return OSDP_ERR_ARG;
       oc.ps = to_ps(sec);
@@ -213,11 +244,39 @@ int osdp_plan(const osdp_op_cost* ops, int32_t n, const osdp_device* dev, int64_
   if (st != OSDP_OK) return st;
   if (batch < 0) return OSDP_ERR_ARG;
   Search S;
-  st = run_search(ops, n, dev, batch, k_candidates, n_cand, S);
+  const std::vector<Option> options = pure_options(k_candidates, n_cand);
+  st = run_search(ops, n, dev, batch, options, S);
   if (st != OSDP_OK) return st;
   for (int i = 0; i < n; ++i) {
-    mode_out[i] = S.best_choice[i] / n_cand;
-    k_out[i] = k_candidates[S.best_choice[i] % n_cand];
+    mode_out[i] = options[S.best_choice[i]].z == 0 ? OSDP_DP : OSDP_ZDP;
+    k_out[i] = options[S.best_choice[i]].k;
+  }
+  if (est_seconds) *est_seconds = (double)S.best_ps / kPsPerSecond;
+  if (est_peak_bytes) *est_peak_bytes = S.best_mem;
+  return OSDP_OK;
+}
+
+int osdp_cost_eval_mixed(const osdp_op_cost* op, int32_t k, int32_t zdp_slices, int64_t batch, const osdp_device* dev,
+                         uint64_t* persist_bytes, uint64_t* transient_bytes, double* seconds) {
+  if (!op || !dev) return OSDP_ERR_NULL;
+  return eval_mixed(*op, k, zdp_slices, batch, *dev, persist_bytes, transient_bytes, seconds) ? OSDP_OK : OSDP_ERR_ARG;
+}
+
+int osdp_plan_mixed(const osdp_op_cost* ops, int32_t n, const osdp_device* dev, int64_t batch,
+                    const int32_t* k_candidates, int32_t n_cand,
+                    int32_t* k_out, int32_t* zdp_slices_out, double* est_seconds, uint64_t* est_peak_bytes) {
+  int st = check_plan_args(ops, n, dev, k_candidates, n_cand, k_out, zdp_slices_out);
+  if (st != OSDP_OK) return st;
+  if (batch < 0) return OSDP_ERR_ARG;
+  for (int i = 0; i < n_cand; ++i)
+    if (k_candidates[i] > 1024) return OSDP_ERR_ARG;   // the option table has k + 1 entries per candidate
+  Search S;
+  const std::vector<Option> options = mixed_options(k_candidates, n_cand);
+  st = run_search(ops, n, dev, batch, options, S);
+  if (st != OSDP_OK) return st;
+  for (int i = 0; i < n; ++i) {
+    k_out[i] = options[S.best_choice[i]].k;
+    zdp_slices_out[i] = options[S.best_choice[i]].z;
   }
   if (est_seconds) *est_seconds = (double)S.best_ps / kPsPerSecond;
   if (est_peak_bytes) *est_peak_bytes = S.best_mem;
@@ -238,9 +297,10 @@ int osdp_plan_batch(const osdp_op_cost* ops, int32_t n, const osdp_device* dev, 
   int64_t best_b = 0, best_ps = 0;
   uint64_t best_mem = 0;
   std::vector<int> best_choice;
+  const std::vector<Option> options = pure_options(k_candidates, n_cand);
   for (int64_t b = 1; b <= batch_max; ++b) {
     Search S;
-    st = run_search(ops, n, dev, b, k_candidates, n_cand, S);
+    st = run_search(ops, n, dev, b, options, S);
     if (st == OSDP_ERR_INFEASIBLE) break;
     if (st != OSDP_OK) return st;
     // compare S.best_ps / b  <  best_ps / best_b  exactly: cross-multiply in 128-bit
@@ -252,8 +312,8 @@ int osdp_plan_batch(const osdp_op_cost* ops, int32_t n, const osdp_device* dev, 
   }
   if (!any) return OSDP_ERR_INFEASIBLE;
   for (int i = 0; i < n; ++i) {
-    mode_out[i] = best_choice[i] / n_cand;
-    k_out[i] = k_candidates[best_choice[i] % n_cand];
+    mode_out[i] = options[best_choice[i]].z == 0 ? OSDP_DP : OSDP_ZDP;
+    k_out[i] = options[best_choice[i]].k;
   }
   *batch_out = best_b;
   if (est_seconds) *est_seconds = (double)best_ps / kPsPerSecond;

@@ -193,6 +193,79 @@ def test_plan_ties_resolve_to_first_in_traversal_order(lib):
     assert st == 0 and ks == ref[1] == [1, 2, 2] and modes == ref[0] == [0, 0, 0]     # N = 1: DP (reading P7)
 
 
+# ------------------------------------------------------------------ slice-level mode mixing
+def test_mixed_cost_model_closed_forms():
+    """z = 0 / z = k are the paper's DP / ZDP formulas; the paper's own example, 4 slices with 1 in ZDP and 3 in DP
+    (PAPER.md:179): communication 2.25 collectives' worth, model states 3/4 + 1/(4 N) of the replica."""
+    op = P.OpCost(S=3.0e8, model=16 * 10 ** 9, act=12345, extra_fixed=77, extra_summed=4096, extra_transient=999, gamma=0.25,
+                  delta=0.01)
+    for N in (1, 2, 8, 64):
+        dev = P.Device(N=N, alpha=5e-6, beta=1e-10)
+        for k in (1, 2, 4, 7):
+            assert P.cost_eval_mixed(op, k, 0, 3, dev) == P.cost_eval(op, P.DP, k, 3, dev)
+            assert P.cost_eval_mixed(op, k, k, 3, dev) == P.cost_eval(op, P.ZDP, k, 3, dev)
+        comm = (N - 1) * (dev.alpha + op.S * dev.beta / N)
+        p, _, t = P.cost_eval_mixed(op, 4, 1, 0, dev)
+        assert math.isclose(t - 3 * op.delta, 2.25 * comm, rel_tol=1e-12, abs_tol=1e-18)
+        assert p - 77 - 1024 == 12 * 10 ** 9 + -(-4 * 10 ** 9 // N)
+        # memory falls and time rises monotonically with the number of ZDP slices
+        vals = [P.cost_eval_mixed(op, 8, z, 1, dev) for z in range(9)]
+        assert all(a[0] >= b[0] for a, b in zip(vals, vals[1:])) and all(a[2] <= b[2] for a, b in zip(vals, vals[1:]))
+
+
+def test_mixed_cost_eval_matches_oracle(lib):
+    rng = random.Random(6)
+    for op in _ops(12, 4):
+        for k in (1, 2, 3, 4, 16):
+            for z in sorted({0, 1 % (k + 1), k // 2, k}):
+                d = P.Device(N=rng.choice([1, 2, 8, 64]), alpha=rng.random() * 1e-3, beta=rng.random() * 1e-9)
+                b = rng.randrange(0, 9)
+                assert lib.osdp_cost_eval_mixed(_to_lib(lib, op), k, z, b, _dev(lib, d)) == P.cost_eval_mixed(op, k, z, b, d)
+    op = _to_lib(lib, _ops(1, 0)[0])
+    assert lib.osdp_cost_eval_mixed(op, 4, 5, 1, _dev(lib, P.Device()), check=False) == lib.OSDP_ERR_ARG
+    assert lib.osdp_cost_eval_mixed(op, 4, -1, 1, _dev(lib, P.Device()), check=False) == lib.OSDP_ERR_ARG
+    assert lib.osdp_cost_eval_mixed(op, 0, 0, 1, _dev(lib, P.Device()), check=False) == lib.OSDP_ERR_ARG
+
+
+@pytest.mark.parametrize("seed", range(10))
+def test_plan_mixed_matches_brute_force_and_never_loses_to_pure_modes(lib, seed):
+    rng = random.Random(300 + seed)
+    n = rng.choice([1, 2, 3])
+    cands = rng.choice([[1], [1, 2, 4], [2, 3], [1, 4]])
+    ops = _ops(n, 50 + seed, identical=(seed % 4 == 3))
+    N = rng.choice([2, 8])
+    base = P.Device(N=N, alpha=rng.random() * 1e-3, beta=rng.random() * 1e-9)
+    b = rng.randrange(1, 4)
+    lo = P.plan_memory_time(ops, [1] * n, [cands[-1]] * n, b, base)[0]
+    hi = P.plan_memory_time(ops, [0] * n, [cands[0]] * n, b, base)[0]
+    for frac in (-0.05, 0.0, 0.3, 0.6, 1.0, 1.5):
+        d = P.Device(N=N, alpha=base.alpha, beta=base.beta, mem_limit=max(0, int(lo + frac * (hi - lo))))
+        ref = P.plan_brute_force_mixed(ops, d, b, cands)
+        lops = [_to_lib(lib, o) for o in ops]
+        st, ks, zs, sec, peak = lib.osdp_plan_mixed(lops, _dev(lib, d), b, cands)
+        if ref is None:
+            assert st == lib.OSDP_ERR_INFEASIBLE
+            continue
+        assert st == lib.OSDP_OK and (ks, zs, peak) == (ref[0], ref[1], ref[3]) and round(sec * 1e12) == ref[2]
+        assert all(0 <= z <= k for k, z in zip(ks, zs)) and peak <= d.mem_limit
+        st2, _, _, sec2, _ = lib.osdp_plan(lops, _dev(lib, d), b, cands)
+        if st2 == lib.OSDP_OK:                      # pure modes are a subset of the mixed decision space
+            assert round(sec * 1e12) <= round(sec2 * 1e12)
+
+
+def test_plan_mixed_uses_a_partial_zdp_assignment_when_the_limit_is_between_the_pure_modes(lib):
+    """'a more fine-grained execution plan': with a limit that pure DP misses by a little, one ZDP slice
+    of four is enough, and it costs less communication than turning the whole operator to ZDP."""
+    op = P.OpCost(S=1.0e9, model=8 << 30, gamma=0.1)
+    d = P.Device(N=8, alpha=1e-5, beta=1e-10, mem_limit=(8 << 30) - (1 << 30))
+    st, ks, zs, sec, peak = lib.osdp_plan_mixed([_to_lib(lib, op)], _dev(lib, d), 1, [1, 4])
+    assert st == lib.OSDP_OK and ks == [4] and zs == [1]
+    st, ks2, modes, sec2, _ = lib.osdp_plan([_to_lib(lib, op)], _dev(lib, d), 1, [1, 4])
+    assert st == lib.OSDP_OK and modes == [1] and ks2 == [1] and sec < sec2
+    comm = 7 * (1e-5 + 1.0e9 * 1e-10 / 8)
+    assert math.isclose(sec, 0.1 + 2.25 * comm, rel_tol=1e-9) and math.isclose(sec2, 0.1 + 3 * comm, rel_tol=1e-9)
+
+
 def test_plan_batch_matches_algorithm1(lib):
     ops = _ops(3, 77)
     for o in ops:
