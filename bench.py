@@ -360,6 +360,43 @@ def fit_gamma_delta(table):
     return {"gamma_s": t1 * 1e-3, "delta_s": delta * 1e-3, "max_rel_residual": resid}
 
 
+def granularity_sweep(args, lib):
+    """Time and peak device bytes against the slice granularity for small and large operators ("for
+    models with small hidden sizes the time cost increases as the slice granularity gets larger", large operators
+    "require larger slice granularity" for the memory benefit).  The paper sweeps granularity 0-16 with hidden 768 /
+    1024 and 8192 / 12288 under ZDP on 8 GPUs; here: one GPU, one MLP operator, both split axes, k = 1 (the paper's
+    0) to 16.  One JSON line."""
+    rows = []
+    ks = (1, 2, 4, 8, 16)
+    for h in [int(x) for x in args.granularity_sweep.split(",")]:
+        cfg = dict(tokens=args.sweep_tokens, hidden=h, ffn=4 * h, dtype="bf16", seed=0)
+        wl = Workload(lib, cfg, 1, seed=0)
+        flops = executed_flops(cfg["tokens"], h, 4 * h)
+        small = wl.resident_bytes() < 2 * L2_BYTES
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda") if small else None
+        for axis in ("tokens", "ffn"):
+            for k in ks:
+                wl.set_k(k, axis)
+                for _ in range(3):
+                    wl.step()
+                torch.cuda.synchronize()
+                n = max(5, min(200, int(0.5 / max(1e-5, flops / 1.2e15))))     # about half a second per point
+                ms, _ = timed_steps(wl.step, n, 1, flush)
+                rows.append({"hidden": h, "axis": axis, "k": k, "steps": n, "ms_per_step": ms / n,
+                             "tflops": flops / (ms / n * 1e-3) / 1e12})
+        del wl, flush
+        torch.cuda.empty_cache()
+        for r in rows:
+            if r["hidden"] == h:
+                pk = measure_peak_bytes(lib, cfg, r["k"], r["axis"])
+                r["peak_bytes_fwd"], r["peak_bytes_bwd"] = pk["fwd"]["measured"], pk["bwd"]["measured"]
+                r["model_bytes_fwd"], r["model_bytes_bwd"] = pk["fwd"]["model"], pk["bwd"]["model"]
+    print(json.dumps({"granularity_sweep": rows, "tokens": args.sweep_tokens, "unit": UNIT, "dtype": "bf16",
+                      "data": "synthetic", "cite": "PAPER.md:231-247 (Fig. 7): shape only, the figure's numbers are an image"}),
+          flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -371,6 +408,11 @@ def main():
     ap.add_argument("--no-sweep", action="store_true", help="skip the per-k TFLOP/s and peak-bytes table")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--granularity-sweep", default=None, metavar="H1,H2,...",
+                    help="instead of the bench line: time and peak bytes vs split count for MLP operators of these "
+                         "hidden sizes (ffn = 4 hidden, --sweep-tokens tokens), both split axes - the shape of the "
+                         "paper's operator-splitting experiment (PAPER.md:231-247, Fig. 7)")
+    ap.add_argument("--sweep-tokens", type=int, default=8192)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -385,6 +427,8 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the osdp-b200 hot path has no CPU fallback")
     from paper_2305_09940_b200 import binding as lib     # raises if the library was not built
+    if args.granularity_sweep:
+        return granularity_sweep(args, lib)
     from paper_2305_09940_b200 import dist as D
     world, rank, local = D.init("nccl")
     peaks = load_peaks()
