@@ -10,7 +10,8 @@ through the C ABI) over one batch of seeded synthetic input of the named workloa
 TFLOP/s (14 T h f per step: 4 forward + 8 backward + 2 for the slice recompute of Z the method itself needs),
 summed over ranks (each rank runs the operator on its own token batch: data parallelism, weak scaling, no
 data-path collective).  Inputs are resident in HBM for `value`; `e2e` is the same metric with host (pinned)
-buffers, host<->device copies inside the timed region.
+buffers, host<->device copies of every input and output inside the timed region (three streams, so the copies
+of neighbouring steps overlap the kernels; the unpipelined figure is reported beside it).
 
 `--impl reference` times the fp64 CPU oracle (oracle/mlp_oracle.py) as it stands on the box's host cores on a
 bounded token sample of the same workload (the reference arm of this tier); only rank 0 runs it.
@@ -271,6 +272,64 @@ class Workload:
         for n, t in self.g.items():
             self.hg[n].copy_(t, non_blocking=True)
 
+    def run_e2e_pipelined(self, steps, world):
+        """The same per-step work as step_e2e (H2D of every input from pinned host memory, forward + backward, D2H of
+        every output), as a user's input pipeline would run it: three streams, device tensors double-buffered, so the
+        H2D of step i+1 and the D2H of step i-1 overlap the kernels of step i (PCIe is full duplex).  Returns ms/step
+        measured with CUDA events around all `steps` steps, barrier + synchronize on both sides."""
+        e = torch.empty
+        names = ("X", "W1", "b1", "W2", "b2", "dY")
+        ins = [self.dev, self.host.to("cuda")]
+        outs = [(self.Y, self.g), (torch.empty_like(self.Y), {n: torch.empty_like(t) for n, t in self.g.items()})]
+        s_in, s_cmp, s_out = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
+        ev_in = [torch.cuda.Event() for _ in range(2)]      # inputs of set b uploaded
+        ev_cmp = [torch.cuda.Event() for _ in range(2)]     # kernels that read set b / wrote out set b finished
+        ev_out = [torch.cuda.Event() for _ in range(2)]     # outputs of set b read back
+        start, stop = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+        def run(n, timed):
+            cur = torch.cuda.current_stream()
+            for st in (s_in, s_cmp, s_out):
+                st.wait_stream(cur)
+            if timed:
+                start.record(cur)
+                for st in (s_in, s_cmp, s_out):
+                    st.wait_event(start)
+            for i in range(n):
+                b = i % 2
+                with torch.cuda.stream(s_in):
+                    if i >= 2:
+                        s_in.wait_event(ev_cmp[b])          # the kernels of step i-2 no longer read this input set
+                    for nm in names:
+                        getattr(ins[b], nm).copy_(getattr(self.host, nm), non_blocking=True)
+                    ev_in[b].record(s_in)
+                with torch.cuda.stream(s_cmp):
+                    s_cmp.wait_event(ev_in[b])
+                    if i >= 2:
+                        s_cmp.wait_event(ev_out[b])         # the outputs of step i-2 have been read back
+                    Y, g = outs[b]
+                    d = ins[b]
+                    self.op.forward(d.X, d.W1, d.b1, d.W2, d.b2, Y=Y, stream=s_cmp)
+                    self.op.backward(d.X, d.W1, d.b1, d.W2, d.dY, out=g, stream=s_cmp)
+                    ev_cmp[b].record(s_cmp)
+                with torch.cuda.stream(s_out):
+                    s_out.wait_event(ev_cmp[b])
+                    Y, g = outs[b]
+                    self.hY.copy_(Y, non_blocking=True)
+                    for nm, t in g.items():
+                        self.hg[nm].copy_(t, non_blocking=True)
+                    ev_out[b].record(s_out)
+            for st in (s_in, s_cmp, s_out):
+                cur.wait_stream(st)
+            if timed:
+                stop.record(cur)
+
+        run(3, False)
+        barrier(world)
+        run(steps, True)
+        barrier(world)
+        return start.elapsed_time(stop) / steps
+
     def h2d_bytes(self):
         return sum(getattr(self.host, n).numel() * getattr(self.host, n).element_size()
                    for n in ("X", "W1", "b1", "W2", "b2", "dY"))
@@ -495,9 +554,14 @@ def main():
         wl.step_e2e()
         torch.cuda.synchronize()
         e_sum, _ = timed_steps(wl.step_e2e, args.steps, world, None)
-        e_ms = max_over_ranks(e_sum / args.steps, world)
+        serial_ms = max_over_ranks(e_sum / args.steps, world)
+        e_ms = max_over_ranks(wl.run_e2e_pipelined(args.steps, world), world)
         e2e = {"value": world * flops / (e_ms * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": e_ms,
-               "h2d_bytes_per_step": wl.h2d_bytes(), "d2h_bytes_per_step": wl.d2h_bytes()}
+               "h2d_bytes_per_step": wl.h2d_bytes(), "d2h_bytes_per_step": wl.d2h_bytes(),
+               "mode": "3 streams, double-buffered device tensors: H2D of step i+1 and D2H of step i-1 overlap the "
+                       "kernels of step i; every step uploads all inputs and reads back all outputs",
+               "serial_ms_per_step": serial_ms,
+               "serial_value": world * flops / (serial_ms * 1e-3) / 1e12}
 
     # ---- per-k table: TFLOP/s and peak bytes vs the cost model (rank 0, N = 1 only)
     per_k = per_k_ffn = cost_fit = None
