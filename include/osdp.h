@@ -18,7 +18,8 @@
  *     Outputs must not alias inputs or each other.
  *   - Every call returns an osdp_status; OSDP_OK = 0.  Nothing is printed, nothing aborts.  On any error
  *     before the first launch the outputs are untouched.
- *   - Re-entrant for distinct streams/workspaces.
+ *   - Re-entrant for distinct streams/workspaces.  After one warm-up call per (dtype, tile shape) the calls are
+ *     CUDA-graph capturable (they only enqueue kernels on `stream`).
  */
 #ifndef OSDP_H_
 #define OSDP_H_

@@ -156,6 +156,39 @@ def test_two_streams_with_wave_sync_do_not_deadlock(lib, force_big_tiles):
             assert np.array_equal(o[n].double().cpu().numpy(), w[n]), n
 
 
+def test_forward_backward_can_be_captured_in_a_cuda_graph(lib):
+    """The library only enqueues on the caller's stream (no allocation, no synchronisation), so after one warm-up call
+    (which caches function attributes and the driver entry point) a whole step can be stream-captured and replayed;
+    launch-bound small operators gain from that."""
+    T, h, f, k = 1000, 320, 1032, 4
+    inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=15)
+    want = {ax: (run_gpu if ax == "tokens" else run_gpu_ffn)(lib, inp, k, torch.bfloat16) for ax in ("tokens", "ffn")}
+    d = inp.to("cuda")
+    for axis in ("tokens", "ffn"):
+        op = lib.SplitMlp(T, h, f, torch.bfloat16, k, axis=axis)
+        Y = torch.empty_like(d.X)
+        g = dict(dX=torch.empty_like(d.X), dW1=torch.empty(h, f, device="cuda"), db1=torch.empty(f, device="cuda"),
+                 dW2=torch.empty(f, h, device="cuda"), db2=torch.empty(h, device="cuda"))
+        s = torch.cuda.Stream()
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            op.forward(d.X, d.W1, d.b1, d.W2, d.b2, Y=Y, stream=s)                 # warm-up outside the capture
+            op.backward(d.X, d.W1, d.b1, d.W2, d.dY, out=g, stream=s)
+            s.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=s):
+                op.forward(d.X, d.W1, d.b1, d.W2, d.b2, Y=Y, stream=s)
+                op.backward(d.X, d.W1, d.b1, d.W2, d.dY, out=g, stream=s)
+        for t in (Y, *g.values()):
+            t.fill_(7.0)
+        graph.replay()
+        graph.replay()
+        torch.cuda.synchronize()
+        got = dict(Y=Y, **g)
+        for n in NAMES:
+            assert np.array_equal(got[n].double().cpu().numpy(), want[axis][n]), (axis, n)
+
+
 def test_tuning_rejects_bad_arguments(lib):
     assert lib.osdp_set_tuning(99, 1, check=False) == lib.OSDP_ERR_ARG
     assert lib.osdp_set_tuning(lib.OSDP_TUNE_WAVE_SYNC, -1, check=False) == lib.OSDP_ERR_ARG
