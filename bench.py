@@ -223,7 +223,7 @@ def run_reference(args, cfg, rank):
 
 def workload_name(args, cfg):
     return (f"{args.config}: MLP operator tokens={cfg['tokens']} hidden={cfg['hidden']} ffn={cfg['ffn']} "
-            f"{cfg['dtype']}, fwd+bwd at k={args.k} token slices")
+            f"{cfg['dtype']}, fwd+bwd at k={args.k} {'token' if args.axis == 'tokens' else 'ffn'} slices")
 
 
 # --------------------------------------------------------------------------------------------------- our arm
@@ -464,6 +464,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--k", type=int, default=4)
+    ap.add_argument("--axis", default="tokens", choices=["tokens", "ffn"],
+                    help="split axis of the headline workload: token slices (north_star, default) or the paper-literal "
+                         "ffn-axis split (osdp_ffn_split_mlp_*)")
     ap.add_argument("--no-sweep", action="store_true", help="skip the per-k TFLOP/s and peak-bytes table")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -493,6 +496,8 @@ def main():
     peaks = load_peaks()
     T, h, f = cfg["tokens"], cfg["hidden"], cfg["ffn"]
     wl = Workload(lib, cfg, args.k, seed=D.rank_seed(cfg["seed"], rank))
+    if args.axis != "tokens":
+        wl.set_k(args.k, args.axis)
     flops = executed_flops(T, h, f)
     small = wl.resident_bytes() < 2 * L2_BYTES
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda") if small else None
@@ -528,7 +533,7 @@ def main():
                "share": sum(v) / total_traced}
         if sid <= 7:
             ent["tflops"] = gemm_flops / (avg * 1e-3) / 1e12
-        kernels[f"A{sid}"] = ent
+        kernels[f"A{sid}" if sid <= 8 else "acc_to_out"] = ent
     dom = max((s for s in per if s <= 7), key=lambda s: sum(per[s]))
     dom_avg = sum(per[dom]) / len(per[dom])
     achieved = gemm_flops / (dom_avg * 1e-3) / 1e12
@@ -536,7 +541,7 @@ def main():
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get(f"{args.config}:k{args.k}:A{dom}")
+        traffic = json.load(open(tpath)).get(f"{args.config}:k{args.k}:A{dom}") if args.axis == "tokens" else None
     roofline = {"bound": "tensor", "kernel": f"gemm_bf16_sm100_kernel [{lib.osdp_step_name(dom)}]",
                 "achieved": achieved, "peak": peak, "unit": UNIT, "frac": (achieved / peak) if peak else None,
                 "traffic": traffic, "peak_source": f"{peaks['source']} (bf16_tflops_sustained: kernel timed inside a long step)",
@@ -577,7 +582,7 @@ def main():
                 s_ms /= n_sw
                 tab.append({"k": k, "ms_per_step": s_ms, "tflops": flops / (s_ms * 1e-3) / 1e12,
                             "frac_of_sustained_peak": flops / (s_ms * 1e-3) / 1e12 / peak if peak else None})
-        wl.set_k(args.k)
+        wl.set_k(args.k, args.axis)
         del wl
         torch.cuda.empty_cache()
         for axis, tab in tables.items():
@@ -595,7 +600,7 @@ def main():
                 "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": cfg["dtype"], "data": "synthetic",
                 "config": {"workload": workload_name(args, cfg), "tokens_per_gpu": T, "hidden": h, "ffn": f,
-                           "k": args.k, "flops_per_step": flops, "flops_counted": "14*T*h*f executed (12*T*h*f model)",
+                           "k": args.k, "split_axis": args.axis, "flops_per_step": flops, "flops_counted": "14*T*h*f executed (12*T*h*f model)",
                            "l2": l2_note, "parallelism": f"dp{world} (independent token batches, no collective)"},
                 "value_model_flops_12x": value * 12.0 / 14.0,
                 "frac_of_sustained_peak": value / world / peak if peak else None,
