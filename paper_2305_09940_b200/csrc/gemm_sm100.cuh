@@ -47,7 +47,7 @@ constexpr int UMMA_K = 16;
 // Kernel selection knobs (osdp_set_tuning): defaults are the measured best on C3/C4.
 struct Tuning {
   std::atomic<int64_t> mt2_min_k{4096};     // MT = 2 from this contraction length on
-  std::atomic<int64_t> mt2_min_tiles{0};    // ... and at least this many 512 x 256 tiles (0 = SMs / 2)
+  std::atomic<int64_t> mt2_min_tiles{0};    // 0: MT = 2 when it idles at most ~10 % more MMA slots than MT = 1; > 0: plain threshold
   std::atomic<int64_t> wave_sync{1};        // line the producers up at tile boundaries (MT = 2 launches)
   std::atomic<int64_t> band_mib{32};        // L2 budget for the A rows of one raster band
 };
@@ -882,12 +882,12 @@ template <int A_MAJOR, int B_MAJOR, int EPI>
 inline int launch_gemm_bf16(const void* A, int64_t lda, const void* B, int64_t ldb, const GemmShape& s,
                             const EpiParams& ep, cudaStream_t st) {
   const int64_t tiles2 = ((s.M + 511) / 512) * ((s.N + BLOCK_N - 1) / BLOCK_N);
-  int64_t min_tiles = tuning().mt2_min_tiles.load();
-  const bool forced = min_tiles > 0;               // tests force MT = 2 on small shapes
-  if (min_tiles <= 0) min_tiles = num_sms() / 2;   // at least one 512 x 256 tile per CTA pair
-  // MT = 2 saves a quarter of the operand traffic; it is not worth more than ~10 % of idle MMA slots
-  const bool fits = forced || tile_efficiency(s, 512) >= 0.9 * tile_efficiency(s, 256);
-  if (s.K >= tuning().mt2_min_k.load() && tiles2 >= min_tiles && fits)
+  const int64_t min_tiles = tuning().mt2_min_tiles.load();
+  // MT = 2 saves a quarter of the operand traffic; it is not worth more than ~10 % of idle MMA slots (padding of M
+  // to 512 rows, fill of the last wave).  A positive OSDP_TUNE_MT2_MIN_TILES replaces that rule by a plain tile-count
+  // threshold (tests use it to force MT = 2 on small shapes).
+  const bool fits = min_tiles > 0 ? tiles2 >= min_tiles : tile_efficiency(s, 512) >= 0.9 * tile_efficiency(s, 256);
+  if (s.K >= tuning().mt2_min_k.load() && fits)
     return launch_gemm_bf16_mt<A_MAJOR, B_MAJOR, EPI, 2>(A, lda, B, ldb, s, ep, st);
   return launch_gemm_bf16_mt<A_MAJOR, B_MAJOR, EPI, 1>(A, lda, B, ldb, s, ep, st);
 }
