@@ -144,14 +144,17 @@ int64_t osdp_last_launch_count(void);
  * MT = 2 when K >= OSDP_TUNE_MT2_MIN_K and either OSDP_TUNE_MT2_MIN_TILES = 0 and the 512 x 256 tiling idles at
  * most ~10 % more MMA slots than the 256 x 256 one (row padding, fill of the last wave), or it has at least
  * OSDP_TUNE_MT2_MIN_TILES > 0 such tiles.  OSDP_TUNE_WAVE_SYNC (MT = 2 launches of more than one wave): 0 off,
- * 1 at tile boundaries, q > 1 also every q k-blocks (64 contraction elements each) inside a tile.  OSDP_TUNE_BAND_MIB: L2 budget (MiB) for the A rows of one raster band.  Results do not depend on
+ * 1 at tile boundaries, q > 1 also every q k-blocks (64 contraction elements each) inside a tile.  OSDP_TUNE_BAND_MIB: L2 budget (MiB) for the A rows of one raster band.
+ * OSDP_TUNE_CLUSTER_MIN_TILES: n > 0 = launches of at least n pair tiles run as 4-CTA clusters (two CTA pairs that
+ * TMA-multicast the A rows they share); 0 = never (clusters of 4 CTAs can occupy only 132 of the 148 SMs).  Results do not depend on
  * any knob beyond fp32 summation order inside a tile (there is none: one owner per output tile).
  * Returns OSDP_ERR_ARG for an unknown key or a value out of range.  osdp_get_tuning returns -1 for an unknown key. */
 typedef enum osdp_tune_key {
   OSDP_TUNE_MT2_MIN_K = 0,      /* default 4096 */
   OSDP_TUNE_MT2_MIN_TILES = 1,  /* default 0 (= efficiency rule) */
   OSDP_TUNE_WAVE_SYNC = 2,      /* default 1 */
-  OSDP_TUNE_BAND_MIB = 3        /* default 32 */
+  OSDP_TUNE_BAND_MIB = 3,       /* default 32 */
+  OSDP_TUNE_CLUSTER_MIN_TILES = 4  /* default 0 (multicast clusters off) */
 } osdp_tune_key;
 int osdp_set_tuning(int key, int64_t value);
 int64_t osdp_get_tuning(int key);

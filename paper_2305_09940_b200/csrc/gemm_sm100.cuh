@@ -50,6 +50,7 @@ struct Tuning {
   std::atomic<int64_t> mt2_min_tiles{0};    // 0: MT = 2 when it idles at most ~10 % more MMA slots than MT = 1; > 0: plain threshold
   std::atomic<int64_t> wave_sync{1};        // line the producers up at tile boundaries (MT = 2 launches)
   std::atomic<int64_t> band_mib{32};        // L2 budget for the A rows of one raster band
+  std::atomic<int64_t> cluster_min_tiles{0};   // > 0: multicast clusters for launches of at least this many pair tiles
 };
 inline Tuning& tuning() {
   static Tuning t;
@@ -849,22 +850,22 @@ inline int launch_gemm_bf16_cluster(const void* A, int64_t lda, const void* B, i
 // Tile shape and cluster shape per launch.
 //  * MT = 2 (512 x 256 pair tiles, 25 % less operand traffic, exposed epilogue) for long contractions, where the
 //    main loop of a tile dwarfs its epilogue; MT = 1 (256 x 256, overlapped epilogue) otherwise.
-//  * Multicast clusters (CM x CN pairs) are compiled only on request (-DOSDP_CM / -DOSDP_CN): clusters of more than
-//    2 CTAs can use at most 132 of the 148 SMs, which costs more than the saved L2 -> SM traffic returns.
+//  * Multicast clusters: OSDP_TUNE_CLUSTER_MIN_TILES = n > 0 takes clusters of OSDP_CM x OSDP_CN pairs (default 1 x 2: the two
+//    pairs of a cluster share their A rows) for launches of at least that many pair tiles (0 = never).
+//    Off by default: clusters of more than 2 CTAs can use at most 132 of the 148 SMs, which costs more than the
+//    saved L2 -> SM traffic returns.  Other cluster shapes: -DOSDP_CM / -DOSDP_CN.
 #ifndef OSDP_CM
 #define OSDP_CM 1
 #endif
 #ifndef OSDP_CN
-#define OSDP_CN 1
-#endif
-#ifndef OSDP_CLUSTER_MIN_TILES
-#define OSDP_CLUSTER_MIN_TILES 148
+#define OSDP_CN 2
 #endif
 template <int A_MAJOR, int B_MAJOR, int EPI, int MT>
 inline int launch_gemm_bf16_mt(const void* A, int64_t lda, const void* B, int64_t ldb, const GemmShape& s,
                                const EpiParams& ep, cudaStream_t st) {
   const int64_t num_m = (s.M + TileCfg<MT>::kPairM - 1) / TileCfg<MT>::kPairM, num_n = (s.N + BLOCK_N - 1) / BLOCK_N;
-  if (OSDP_CM * OSDP_CN > 1 && num_m * num_n >= OSDP_CLUSTER_MIN_TILES)
+  const int64_t cluster_min_tiles = tuning().cluster_min_tiles.load();   // 0 = never
+  if (OSDP_CM * OSDP_CN > 1 && cluster_min_tiles > 0 && num_m * num_n >= cluster_min_tiles)
     return launch_gemm_bf16_cluster<A_MAJOR, B_MAJOR, EPI, MT, OSDP_CM, OSDP_CN>(A, lda, B, ldb, s, ep, st);
   return launch_gemm_bf16_cluster<A_MAJOR, B_MAJOR, EPI, MT, 1, 1>(A, lda, B, ldb, s, ep, st);
 }

@@ -230,6 +230,10 @@ int osdp_set_tuning(int key, int64_t value) {
       if (value < 1 || value > 1024) return OSDP_ERR_ARG;
       t.band_mib = value;
       return OSDP_OK;
+    case OSDP_TUNE_CLUSTER_MIN_TILES:
+      if (value < 0) return OSDP_ERR_ARG;
+      t.cluster_min_tiles = value;
+      return OSDP_OK;
     default: return OSDP_ERR_ARG;
   }
 }
@@ -241,6 +245,7 @@ int64_t osdp_get_tuning(int key) {
     case OSDP_TUNE_MT2_MIN_TILES: return t.mt2_min_tiles;
     case OSDP_TUNE_WAVE_SYNC: return t.wave_sync;
     case OSDP_TUNE_BAND_MIB: return t.band_mib;
+    case OSDP_TUNE_CLUSTER_MIN_TILES: return t.cluster_min_tiles;
     default: return -1;
   }
 }

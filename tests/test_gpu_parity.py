@@ -93,7 +93,8 @@ def test_bf16_large_weights_stress_gelu_range(lib):
 def force_big_tiles(lib):
     """512 x 256 pair tiles (MT = 2) for every launch, whatever K and the tile count: the default build takes them
     only for long-K GEMMs that fill the machine (full-size tests), so the ragged small shapes would never see them."""
-    keys = (lib.OSDP_TUNE_MT2_MIN_K, lib.OSDP_TUNE_MT2_MIN_TILES, lib.OSDP_TUNE_WAVE_SYNC, lib.OSDP_TUNE_BAND_MIB)
+    keys = (lib.OSDP_TUNE_MT2_MIN_K, lib.OSDP_TUNE_MT2_MIN_TILES, lib.OSDP_TUNE_WAVE_SYNC, lib.OSDP_TUNE_BAND_MIB,
+            lib.OSDP_TUNE_CLUSTER_MIN_TILES)
     old = {k: lib.osdp_get_tuning(k) for k in keys}
     lib.osdp_set_tuning(lib.OSDP_TUNE_MT2_MIN_K, 1)
     lib.osdp_set_tuning(lib.OSDP_TUNE_MT2_MIN_TILES, 1)
@@ -115,6 +116,19 @@ def test_bf16_big_tiles_match_oracle(lib, force_big_tiles, T, h, f, k):
     check(run_gpu(lib, inp, k, torch.bfloat16), ref, 2e-2, f"bf16 MT=2 {T}x{h}x{f} k={k}")
 
 
+@pytest.mark.parametrize("T,h,f,k", [(333, 136, 520, 3), (1000, 320, 1032, 2), (130, 72, 264, 1), (512, 256, 768, 1)])
+@pytest.mark.parametrize("big", [False, True])
+def test_bf16_multicast_clusters_match_oracle(lib, force_big_tiles, T, h, f, k, big):
+    """4-CTA clusters (two CTA pairs sharing their A rows through TMA multicast) on ragged shapes, including odd
+    tile counts where one pair of a cluster has no tile of its own."""
+    lib.osdp_set_tuning(lib.OSDP_TUNE_CLUSTER_MIN_TILES, 1)
+    if not big:
+        lib.osdp_set_tuning(lib.OSDP_TUNE_MT2_MIN_K, 1 << 40)
+    inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=16)
+    ref = O.mlp_forward_backward(**inp.as_f64())
+    check(run_gpu(lib, inp, k, torch.bfloat16), ref, 2e-2, f"bf16 clusters MT={2 if big else 1} {T}x{h}x{f} k={k}")
+
+
 def test_bf16_tile_shapes_and_wave_sync_agree_bitwise(lib, force_big_tiles):
     """One owner CTA per output element and ascending-k accumulation in every configuration: tile shape, raster
     band and wave sync change the schedule, not a single bit of the result.  Shape: more 512 x 256 tiles than CTA
@@ -122,10 +136,12 @@ def test_bf16_tile_shapes_and_wave_sync_agree_bitwise(lib, force_big_tiles):
     T, h, f = 5200, 1288, 5144
     inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=10)
     outs = []
-    for min_k, sync, band in ((1, 1, 32), (1, 0, 32), (1, 4, 32), (1, 1, 1), (1 << 40, 1, 32)):
+    for min_k, sync, band, cluster in ((1, 1, 32, 0), (1, 0, 32, 0), (1, 4, 32, 0), (1, 1, 1, 0), (1 << 40, 1, 32, 0),
+                                       (1, 1, 32, 1), (1 << 40, 1, 32, 1)):        # last two: 4-CTA multicast clusters
         lib.osdp_set_tuning(lib.OSDP_TUNE_MT2_MIN_K, min_k)
         lib.osdp_set_tuning(lib.OSDP_TUNE_WAVE_SYNC, sync)
         lib.osdp_set_tuning(lib.OSDP_TUNE_BAND_MIB, band)
+        lib.osdp_set_tuning(lib.OSDP_TUNE_CLUSTER_MIN_TILES, cluster)
         outs.append(run_gpu(lib, inp, 2, torch.bfloat16))
     for o in outs[1:]:
         for n in NAMES:
