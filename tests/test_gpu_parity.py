@@ -205,6 +205,28 @@ def test_forward_backward_can_be_captured_in_a_cuda_graph(lib):
             assert np.array_equal(got[n].double().cpu().numpy(), want[axis][n]), (axis, n)
 
 
+def test_trace_records_every_launch_with_its_step(lib):
+    """osdp_trace_*: one (step id, milliseconds) entry per kernel launch, in launch order, both split axes."""
+    T, h, f, k = 600, 128, 512, 3
+    d = I.mlp_inputs(T, h, f, torch.bfloat16, seed=17).to("cuda")
+    for axis, fwd_steps, bwd_steps in (("tokens", [1, 2] * k, [3, 4, 5, 8, 8, 6, 7] * k),
+                                       ("ffn", [1, 2] * k + [10], [3, 4, 5, 8, 8, 6, 7] * k + [10])):
+        op = lib.SplitMlp(T, h, f, torch.bfloat16, k, axis=axis)
+        op.forward(d.X, d.W1, d.b1, d.W2, d.b2)                      # warm-up, untraced
+        lib.osdp_trace_enable(True)
+        op.forward(d.X, d.W1, d.b1, d.W2, d.b2)
+        n_fwd = lib.osdp_last_launch_count()
+        op.backward(d.X, d.W1, d.b1, d.W2, d.dY)
+        n_bwd = lib.osdp_last_launch_count()
+        tr = lib.osdp_trace_read()
+        lib.osdp_trace_enable(False)
+        assert [s for s, _ in tr] == fwd_steps + bwd_steps and (n_fwd, n_bwd) == (len(fwd_steps), len(bwd_steps)), axis
+        assert all(0.0 < ms < 50.0 for _, ms in tr)
+        assert lib.osdp_trace_read() == []                           # reading clears the trace
+    assert "GEMM1" in lib.osdp_step_name(1) and "column sums" in lib.osdp_step_name(8)
+    assert "accumulator" in lib.osdp_step_name(10) and lib.osdp_step_name(99) == "unknown"
+
+
 def test_tuning_rejects_bad_arguments(lib):
     assert lib.osdp_set_tuning(99, 1, check=False) == lib.OSDP_ERR_ARG
     assert lib.osdp_set_tuning(lib.OSDP_TUNE_WAVE_SYNC, -1, check=False) == lib.OSDP_ERR_ARG
