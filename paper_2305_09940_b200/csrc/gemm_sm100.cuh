@@ -153,8 +153,12 @@ __device__ __forceinline__ uint32_t mapa(uint32_t addr, uint32_t rank) {
   asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
   return r;
 }
+// Arrive on an mbarrier of another CTA of the cluster (shared::cluster address).  Default semantics (release at CTA
+// scope): the barriers signalled this way hand over TMEM, whose ordering comes from tcgen05.wait::ld and the
+// tcgen05 fences on both sides, not from generic-memory visibility; a cluster-scope release was measured to hold
+// the arrival back by ~1.2 us (profiles/r01c_power_probes.md section 8).
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
-  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+  asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
 __device__ __forceinline__ void cluster_sync() {
   asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
@@ -618,19 +622,23 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
     const StorePipe pipe{smem_store + (uint32_t)(warp - kEpiWarp0) * kStoreBufBytes, lane};
     const uint32_t tempty_leader = mapa(tempty_bar, leader_crank);
     const __nv_bfloat16* bias = reinterpret_cast<const __nv_bfloat16*>(ep.bias);
-    // 8 consecutive accumulator columns (+ bias) -> fp32 values
-    auto load8 = [&](const uint32_t* a, int ng, float (&v)[8]) {
+    constexpr bool kHasBias = (EPI == EPI_BIAS_GELU || EPI == EPI_BIAS || EPI == EPI_BIAS_GELU_DUAL);
+    // The bias of a warp's column chunks is fetched BEFORE the wait for the accumulator (a global load inside the
+    // chunk loop costs ~1.3 us per chunk on the exposed path): lane l keeps columns 2 l, 2 l + 1 of chunk ci in
+    // bias_reg[ci]; the chunk loop reads them back with shuffles.  Both row halves of an MT = 2 tile use the same columns.
+    constexpr int kBiasChunks = BLOCK_N / (2 * 64);   // chunks of 64 columns this warp owns per tile (bf16 outputs)
+    uint32_t bias_reg[kBiasChunks] = {};
+    // 8 consecutive accumulator columns (+ bias) -> fp32 values; j = index of the 8-column group inside chunk ci
+    static_assert(kBiasChunks == 2, "bias registers: two column chunks per epilogue warp");
+    auto load8 = [&](const uint32_t* a, uint32_t bias_cur, int j, float (&v)[8]) {
 #pragma unroll
       for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(a[i]);
-      if constexpr (EPI == EPI_BIAS_GELU || EPI == EPI_BIAS || EPI == EPI_BIAS_GELU_DUAL) {
-        if (ng < shape.N) {   // warp-uniform
-          const uint4 b = __ldg(reinterpret_cast<const uint4*>(bias + ng));
-          const uint32_t bw[4] = {b.x, b.y, b.z, b.w};
+      if constexpr (kHasBias) {
 #pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            v[2 * i] += bf16_lo(bw[i]);
-            v[2 * i + 1] += bf16_hi(bw[i]);
-          }
+        for (int i = 0; i < 4; ++i) {
+          const uint32_t bw = __shfl_sync(0xFFFFFFFFu, bias_cur, 4 * j + i);
+          v[2 * i] += bf16_lo(bw);
+          v[2 * i + 1] += bf16_hi(bw);
         }
       }
     };
@@ -644,6 +652,13 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
       const uint32_t aphase = (it / kAccStages) & 1;
       const int n0 = (tc.n_blk * CN + pj) * BLOCK_N;
       const int n_end = min(n0 + BLOCK_N, shape.N);
+      if constexpr (kHasBias) {
+#pragma unroll
+        for (int ci = 0; ci < kBiasChunks; ++ci) {
+          const int c = n0 + (cg + 2 * ci) * 64 + 2 * lane;
+          bias_reg[ci] = c < shape.N ? __ldg(reinterpret_cast<const uint32_t*>(bias + c)) : 0u;   // N is even
+        }
+      }
       mbar_wait_long(tfull_bar + 8 * as, aphase);
       tc_fence_after();
       bool released = false;   // the accumulator stage goes back to the MMA warp right after this warp's last tcgen05.ld
@@ -680,6 +695,7 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
             if (lane == 0) mbar_arrive_cluster(tempty_leader + 8 * as);
             released = true;
           }
+          [[maybe_unused]] const uint32_t bias_cur = (n - n0) >= 2 * kChunk ? bias_reg[1] : bias_reg[0];
           if constexpr (Tr::kF32Out) {
             pipe.begin();
 #pragma unroll
@@ -691,7 +707,7 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
 #pragma unroll
               for (int j = 0; j < 8; ++j) {
                 float v[8];
-                load8(&acc[8 * j], n + 8 * j, v);
+                load8(&acc[8 * j], bias_cur, j, v);
                 pipe.put(j, pack8(v));
               }
               pipe.commit(&tmap_out0, n, row0, false);
@@ -700,7 +716,7 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
               float v[8];
-              load8(&acc[8 * j], n + 8 * j, v);
+              load8(&acc[8 * j], bias_cur, j, v);
               if constexpr (EPI == EPI_BIAS_GELU || EPI == EPI_BIAS_GELU_DUAL) {
 #pragma unroll
                 for (int i = 0; i < 8; ++i) v[i] = gelu_fwd<false>(v[i]);
