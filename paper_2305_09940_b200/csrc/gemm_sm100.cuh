@@ -164,6 +164,12 @@ __device__ __forceinline__ void cluster_sync() {
   asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
   asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
+// Rendezvous only (no memory is handed over): the teardown, where a CTA just must not exit while a peer can still
+// signal its barriers, write its smem or run UMMAs on its TMEM.
+__device__ __forceinline__ void cluster_sync_relaxed() {
+  asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");
+  asm volatile("barrier.cluster.wait.aligned;" ::: "memory");
+}
 // Long waits (an epilogue warp waiting a whole main loop for its accumulator): optionally back off between polls.
 __device__ __forceinline__ void mbar_wait_long(uint32_t bar, uint32_t parity) {
 #if OSDP_WAIT_SLEEP_NS > 0
@@ -747,7 +753,7 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
 
   // No CTA may exit (or free TMEM) while a peer can still signal its barriers, write its smem or run UMMAs on its TMEM.
   tc_fence_before();
-  cluster_sync();
+  cluster_sync_relaxed();
   if (warp == 2) {
     tc_fence_after();
     tmem_dealloc(tmem_base, kTmemCols);
