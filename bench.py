@@ -456,6 +456,103 @@ def granularity_sweep(args, lib):
     return 0
 
 
+def stack_bench(args, lib, cfg):
+    """BASELINE.json config 5: a chain of `layers` MLP operators (X_{l+1} = MLP_l(X_l), reading S13), forward through
+    all layers then backward, the split count of each layer chosen by osdp_plan under the activation cap.
+    Device information for the planner (alpha, beta, gamma "profiled in advance") is calibrated here:
+    one layer is timed at k = 1, 2, 4, 8, 16 and T(k) = gamma + (k - 1) delta is fitted (fit_gamma_delta).  The
+    memory factors are the paper's accounting (Eq. 1 sums M_i over operators; 8 B per T x f element for an unfused
+    autograd MLP, SURVEY.md section 8 note), under which the 24 GiB cap binds.  One JSON line: measured stack
+    throughput, the plan, and the planner's time estimate next to the measured time."""
+    from paper_2305_09940_b200 import inputs as I
+    T, h, f, L = cfg["tokens"], cfg["hidden"], cfg["ffn"], cfg.get("layers", 24)
+    dt = I.torch_dtype(cfg["dtype"])
+    ks_cal = (1, 2, 4, 8, 16)
+    wl = Workload(lib, cfg, 1, seed=0)
+    table = []
+    for k in ks_cal:
+        wl.set_k(k)
+        for _ in range(3):
+            wl.step()
+        ms, _ = timed_steps(wl.step, 20, 1, None)
+        n = max(20, min(400, int(600.0 / max(ms / 20, 1e-3))))      # ~0.6 s per point: at the power cap, like the stack itself
+        ms, _ = timed_steps(wl.step, n, 1, None)
+        table.append({"k": k, "ms_per_step": ms / n, "steps": n})
+    fit = fit_gamma_delta(table)
+    del wl
+    torch.cuda.empty_cache()
+
+    desc1 = lib.make_desc(T, h, f, dt, 1)
+    ops = []
+    for _ in range(L):
+        oc = lib.osdp_mlp_op_cost(desc1, lib.OSDP_BWD)
+        oc.model_bytes = (2 * h * f + f + h) * 2          # weights; gradients / optimizer states outside the activation cap
+        oc.extra_fixed = 0
+        oc.extra_transient = 0
+        oc.extra_summed = 8 * T * f                       # Z, H, dH, dZ in bf16: the unfused-autograd view of the intermediate
+        oc.act_bytes = T * h * 2                          # saved layer input
+        oc.gamma, oc.delta = fit["gamma_s"], max(fit["delta_s"], 0.0)
+        ops.append(oc)
+    cap = cfg.get("act_cap_bytes", 24 << 30)
+    st, ks, modes, est_s, est_peak = lib.osdp_plan(ops, lib.osdp_device(1, 0.0, 0.0, cap), 1, [1, 2, 4, 8, 16, 32])
+    if st != lib.OSDP_OK:
+        raise SystemExit(f"osdp_plan: status {st}")
+
+    t0 = time.time()
+    layers = []
+    for l in range(L):
+        w = I.mlp_inputs(1, h, f, dt, seed=l)             # weights and biases of layer l (seed = layer, reading S13)
+        layers.append(dict(W1=w.W1.cuda(), b1=w.b1.cuda(), W2=w.W2.cuda(), b2=w.b2.cuda(),
+                           op=lib.SplitMlp(T, h, f, dt, ks[l]),
+                           g=dict(dX=torch.empty((T, h), dtype=dt, device="cuda"),
+                                  dW1=torch.empty((h, f), dtype=torch.float32, device="cuda"),
+                                  db1=torch.empty((f,), dtype=torch.float32, device="cuda"),
+                                  dW2=torch.empty((f, h), dtype=torch.float32, device="cuda"),
+                                  db2=torch.empty((h,), dtype=torch.float32, device="cuda"))))
+    Xs = [I.normal_tensor(0, I.STREAM_X, (T, h), 1.0, dt).cuda()] + [torch.empty((T, h), dtype=dt, device="cuda") for _ in range(L)]
+    dYL = I.normal_tensor(0, I.STREAM_DY, (T, h), 1.0, dt).cuda()
+    log(f"[bench] stack inputs generated in {time.time() - t0:.1f}s; plan k = {ks}")
+    launches = [0]
+
+    def step():
+        n = 0
+        for l, ly in enumerate(layers):
+            ly["op"].forward(Xs[l], ly["W1"], ly["b1"], ly["W2"], ly["b2"], Y=Xs[l + 1])
+            n += lib.osdp_last_launch_count()
+        dY = dYL
+        for l in reversed(range(L)):
+            ly = layers[l]
+            ly["op"].backward(Xs[l], ly["W1"], ly["b1"], ly["W2"], dY, out=ly["g"])
+            n += lib.osdp_last_launch_count()
+            dY = ly["g"]["dX"]
+        launches[0] = n
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    steps = max(3, min(args.steps, 20))
+    sampler = ClockSampler(0)
+    sampler.start()
+    ms_sum, _ = timed_steps(step, steps, 1, None)
+    clocks = sampler.stop()
+    ms = ms_sum / steps
+    flops = executed_flops(T, h, f) * L
+    peaks = load_peaks()
+    print(json.dumps({
+        "metric": METRIC, "value": flops / (ms * 1e-3) / 1e12, "unit": UNIT, "n_gpus": 1, "steps": steps,
+        "warmup": max(3, args.warmup), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": cfg["dtype"], "data": "synthetic",
+        "config": {"workload": f"C5: {L}-layer MLP stack tokens={T} hidden={h} ffn={f} bf16, fwd through all layers then bwd, "
+                               f"k per layer from osdp_plan under a {cap >> 30} GiB activation cap",
+                   "k_per_layer": ks, "flops_per_step": flops, "l2": "inputs+outputs exceed L2 (126 MB); no flush"},
+        "frac_of_sustained_peak": flops / (ms * 1e-3) / 1e12 / peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]),
+        "frac_of_nominal_peak": flops / (ms * 1e-3) / 1e12 / NOMINAL_BF16_TFLOPS,
+        "planner": {"calibration_ms_per_layer": {str(e["k"]): e["ms_per_step"] for e in table}, "fit": fit,
+                    "est_ms_per_step": est_s * 1e3, "measured_ms_per_step": ms, "est_over_measured": est_s * 1e3 / ms,
+                    "est_peak_bytes_paper_accounting": est_peak, "cap_bytes": cap},
+        "clocks": clocks, "gpu_launches": launches[0] * steps}), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -475,6 +572,9 @@ def main():
                          "hidden sizes (ffn = 4 hidden, --sweep-tokens tokens), both split axes - the shape of the "
                          "paper's operator-splitting experiment (PAPER.md:231-247, Fig. 7)")
     ap.add_argument("--sweep-tokens", type=int, default=8192)
+    ap.add_argument("--stack", action="store_true",
+                    help="with --config C5: instead of the bench line, run the 24-layer MLP stack with the split count "
+                         "per layer chosen by osdp_plan from gamma/delta calibrated on this GPU (BASELINE.json config 5)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -491,6 +591,8 @@ def main():
     from paper_2305_09940_b200 import binding as lib     # raises if the library was not built
     if args.granularity_sweep:
         return granularity_sweep(args, lib)
+    if args.stack:
+        return stack_bench(args, lib, cfg)
     from paper_2305_09940_b200 import dist as D
     world, rank, local = D.init("nccl")
     peaks = load_peaks()
