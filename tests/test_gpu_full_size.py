@@ -80,6 +80,17 @@ def test_c4_ffn_split_sampled_oracle(lib):
     check_sampled(lib, inp, inp.as_f64(), (4, 32), "C4 ffn split", axis="ffn")
 
 
+def test_large_token_count_offsets_beyond_2_gib(lib):
+    """Maximum-size edge: tokens x ffn = 2^30 elements, so every [T x f] workspace tensor is 2 GiB and byte offsets
+    inside it pass 2^31; rows at the far end and columns across tile edges are checked against the sampled oracle,
+    for both split axes (unsplit and split)."""
+    T, h, f = 262144, 1024, 4096
+    inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=3)
+    x64 = inp.as_f64()
+    check_sampled(lib, inp, x64, (1, 3), "2^30-element intermediate")
+    check_sampled(lib, inp, x64, (2,), "2^30-element intermediate, ffn split", axis="ffn")
+
+
 def test_c4_token_downscaled_full_oracle(lib):
     """Full oracle on a token-downscaled copy (T/8) of the largest config: every output element checked."""
     c = I.CONFIGS["C4"]
