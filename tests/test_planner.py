@@ -111,6 +111,114 @@ def test_oracle_splits_bigger_operators_first():
     assert ks == [1, 2, 1]
 
 
+# ------------------------------------------------------------------ oracle pins that do not involve the library
+def test_oracle_schedule_hand_worked_algorithm1_example():
+    """Algorithm 1 in full on a two-operator model worked by hand.  N = 2, alpha = 0, beta = 1, so an
+    operator's collective costs c_i = (N - 1) S_i / N = S_i / 2.  M_limit = 290 bytes, k in {1, 2}.
+
+        A: S = 2 (c = 1), model 100, act 10, sliceable extra 80, gamma 0.5, delta 1.5
+        B: S = 0.4 (c = 0.2), model 40, act 30, gamma 0.25
+
+        memory  A: DP k1 180 + 10 b | DP k2 140 + 10 b | ZDP k1 130 + 10 b | ZDP k2 90 + 10 b;   B: DP 40 + 30 b | ZDP 20 + 30 b
+        time    A: DP k1 2 + b/2    | DP k2 3.5 + b/2  | ZDP k1 3 + b/2    | ZDP k2 4.5 + b/2;   B: DP 0.4 + b/4 | ZDP 0.6 + b/4
+
+        b = 1: all DP fits (260)                            T* = 2 + 0.5 + 0.4 + 0.25           = 3.15   T*/b = 3.15
+        b = 2: all DP is 300 > 290; A DP k1 + B ZDP = 280   T* = 2 + 1 + 0.6 + 0.5              = 4.1    T*/b = 2.05
+        b = 3: A ZDP k1 + B DP = 160 + 130 = 290 (= limit)  T* = 3 + 1.5 + 0.4 + 0.75           = 5.65   T*/b = 1.8833
+               (A DP k2 + B ZDP = 280 fits too but costs 6.35; A DP k1 needs 210 + 110 = 320)
+        b = 4: only A ZDP k2 fits: + B DP = 130 + 160 = 290 T* = 4.5 + 2 + 0.4 + 1              = 7.9    T*/b = 1.975
+        b = 5: the smallest plan (A ZDP k2 + B ZDP) needs 140 + 170 = 310 > 290: stop (lines 12-14).
+
+    Eq. 1 minimises T/b, so the answer is b* = 3 with p* = (ZDP, DP), k = (1, 1).  Taking argmin T(b)
+    instead would return b = 1, taking the last candidate would return b = 4, and a '<' instead of '<=' in the memory
+    test (Algorithm 1 line 8) would lose the b = 3 plan that meets the limit exactly."""
+    A = P.OpCost(S=2.0, model=100, act=10, extra_summed=80, gamma=0.5, delta=1.5)
+    B = P.OpCost(S=0.4, model=40, act=30, gamma=0.25)
+    dev = P.Device(N=2, alpha=0.0, beta=1.0, mem_limit=290)
+    per_b = {1: ([P.DP, P.DP], [1, 1], 3_150_000_000_000, 260), 2: ([P.DP, P.ZDP], [1, 1], 4_100_000_000_000, 280),
+             3: ([P.ZDP, P.DP], [1, 1], 5_650_000_000_000, 290), 4: ([P.ZDP, P.DP], [2, 1], 7_900_000_000_000, 290)}
+    for b, want in per_b.items():
+        assert P.plan_brute_force([A, B], dev, b, [1, 2]) == want, b
+    assert P.plan_brute_force([A, B], dev, 5, [1, 2]) is None
+    assert P.schedule_brute_force([A, B], dev, [1, 2]) == ([P.ZDP, P.DP], [1, 1], 5_650_000_000_000, 290, 3)
+    # b_max cuts the loop short: with b <= 2 the best per-sample time is b = 2's
+    assert P.schedule_brute_force([A, B], dev, [1, 2], b_max=2) == ([P.DP, P.ZDP], [1, 1], 4_100_000_000_000, 280, 2)
+
+
+def test_oracle_schedule_stops_at_the_first_infeasible_batch(monkeypatch):
+    """Algorithm 1 lines 12-14: 'Stop searching since all plans exceed memory limit under the current
+    batch size' - a break, not a skip.  In the cost model memory grows with b, so a later batch can never fit again; the
+    loop structure is pinned by replacing the inner search with one that is infeasible at b = 2 only: b = 3 (which
+    would win on T/b) must never be reached."""
+    calls = []
+
+    def fake(ops, dev, b, cands):
+        calls.append(b)
+        return None if b == 2 else ([P.DP], [1], 10 ** 12 if b == 1 else 10 ** 6, 1)
+
+    monkeypatch.setattr(P, "plan_brute_force", fake)
+    assert P.schedule_brute_force([P.OpCost()], P.Device(mem_limit=1), [1], b_max=8) == ([P.DP], [1], 10 ** 12, 1, 1)
+    assert calls == [1, 2]
+    calls.clear()
+    monkeypatch.setattr(P, "plan_brute_force", lambda *a: None)
+    assert P.schedule_brute_force([P.OpCost()], P.Device(mem_limit=1), [1], b_max=8) is None
+
+
+def test_oracle_mixed_plan_papers_own_example():
+    """'partition the operator into 4 slices and process 1 of them in the ZDP mode and 3 of them in the DP
+    mode'.  One operator of 8 GiB model states on N = 8 devices, limit 7 GiB: pure DP (8 GiB) does not fit, pure ZDP
+    (1 GiB) fits at 3 collectives; four slices with one in ZDP hold 6 GiB + 2 GiB / 8 = 6.25 GiB and cost
+    (3 * 2 + 1 * 3) / 4 = 2.25 collectives (PAPER.md:92-94 per slice).  Asserted on the ORACLE."""
+    GiB = 1 << 30
+    op = P.OpCost(S=1.0e9, model=8 * GiB, gamma=0.1)
+    dev = P.Device(N=8, alpha=1e-5, beta=1e-10, mem_limit=7 * GiB)
+    comm = 7 * (1e-5 + 1.0e9 * 1e-10 / 8)
+    ks, zs, ps, peak = P.plan_brute_force_mixed([op], dev, 1, [1, 4])
+    assert (ks, zs) == ([4], [1]) and peak == 6 * GiB + GiB // 4
+    assert ps == P.to_ps(0.1 + 2.25 * comm)
+    # the pure-mode search can only take whole-operator ZDP: 3 collectives, 1 GiB
+    modes, ks1, ps1, peak1 = P.plan_brute_force([op], dev, 1, [1, 4])
+    assert (modes, ks1, peak1) == ([P.ZDP], [1], GiB) and ps1 == P.to_ps(0.1 + 3 * comm) and ps < ps1
+    # with a limit just under 6.25 GiB one ZDP slice is not enough: two of four (5.5 GiB, 2.5 collectives)
+    dev2 = P.Device(N=8, alpha=1e-5, beta=1e-10, mem_limit=6 * GiB + GiB // 4 - 1)
+    ks, zs, ps, peak = P.plan_brute_force_mixed([op], dev2, 1, [1, 4])
+    assert (ks, zs, peak) == ([4], [2], 4 * GiB + 4 * GiB // 8) and ps == P.to_ps(0.1 + 2.5 * comm)
+
+
+def _golden_peak_rows():
+    rows = []
+    for line in open(os.path.join(GOLDEN, "peak_bytes_mib.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        c, T, h, f, e, k, fwd, bwd = line.split()
+        rows.append((c, int(T), int(h), int(f), int(e), int(k), float(fwd), float(bwd)))
+    return rows
+
+
+def test_oracle_byte_calculators_reproduce_the_worked_peak_bytes():
+    """mlp_persistent_bytes + mlp_workspace_bytes against the figures SURVEY.md section 8(d) works out by hand (MiB;
+    tests/golden/peak_bytes_mib.txt).  The printed figures leave out the bias vectors and the fixed column-sum scratch:
+    the scratch is stated separately (REDUCE_ROW_CHUNKS x (h + f) fp32 partial sums) and the biases
+    are (f + h) e bytes forward, (f + h)(e + 4) backward (db1, db2 are fp32)."""
+    rows = _golden_peak_rows()
+    assert len(rows) == 9
+    MiB = 1 << 20
+    for c, T, h, f, e, k, fwd, bwd in rows:
+        scratch = P.mlp_reduce_scratch_bytes(h, f)
+        assert scratch == -(-32 * (h + f) * 4 // 256) * 256
+        got_f = P.mlp_persistent_bytes(T, h, f, e, False) + P.mlp_workspace_bytes(T, h, f, e, k, False)
+        got_b = P.mlp_persistent_bytes(T, h, f, e, True) + P.mlp_workspace_bytes(T, h, f, e, k, True) - scratch
+        assert got_f - (f + h) * e == fwd * MiB, (c, k)
+        assert got_b - (f + h) * (e + 4) == bwd * MiB, (c, k)
+    # size / slice_granularity (PAPER.md:167): the workspace is the only term that moves with k
+    for T, h, f, e in ((8192, 8192, 32768, 2), (512, 256, 1024, 4)):
+        for bw in (False, True):
+            fixed = P.mlp_reduce_scratch_bytes(h, f) if bw else 0
+            w1 = P.mlp_workspace_bytes(T, h, f, e, 1, bw) - fixed
+            for k in (2, 4, 8):
+                assert (P.mlp_workspace_bytes(T, h, f, e, k, bw) - fixed) * k == w1
+
+
 # ------------------------------------------------------------------ library == oracle
 def _to_lib(lib, op):
     return lib.osdp_op_cost(op.S, op.model, op.act, op.extra_fixed, op.extra_summed, op.extra_transient, op.gamma,
