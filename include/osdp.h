@@ -18,8 +18,11 @@
  *     Outputs must not alias inputs or each other.
  *   - Every call returns an osdp_status; OSDP_OK = 0.  Nothing is printed, nothing aborts.  On any error
  *     before the first launch the outputs are untouched.
- *   - Re-entrant for distinct streams/workspaces.  After one warm-up call per (dtype, tile shape) the calls are
- *     CUDA-graph capturable (they only enqueue kernels on `stream`).
+ *   - Re-entrant for distinct streams/workspaces, from any number of host threads, on any device with ordinal < 64:
+ *     launch state (SM count, shared-memory opt-in, resident cluster count, wave-sync counters) is kept per device
+ *     ordinal; the device used is the one current to the calling thread, which must own every pointer passed.  Only
+ *     the osdp_set_tuning knobs are process-wide.  After one warm-up call per (dtype, tile shape, device) the calls
+ *     are CUDA-graph capturable (they only enqueue kernels on `stream`).
  */
 #ifndef OSDP_H_
 #define OSDP_H_
@@ -154,7 +157,8 @@ typedef enum osdp_tune_key {
   OSDP_TUNE_MT2_MIN_TILES = 1,  /* default 0 (= efficiency rule) */
   OSDP_TUNE_WAVE_SYNC = 2,      /* default 1 */
   OSDP_TUNE_BAND_MIB = 3,       /* default 32 */
-  OSDP_TUNE_CLUSTER_MIN_TILES = 4  /* default 0 (multicast clusters off) */
+  OSDP_TUNE_CLUSTER_MIN_TILES = 4, /* default 0 (multicast clusters off) */
+  OSDP_TUNE_MT2_MIN_K_ACC = 5      /* OSDP_TUNE_MT2_MIN_K for the fp32-accumulate launches (dW GEMMs, K = slice rows) */
 } osdp_tune_key;
 int osdp_set_tuning(int key, int64_t value);
 int64_t osdp_get_tuning(int key);
@@ -203,9 +207,13 @@ int osdp_cost_eval(const osdp_op_cost* op, int mode, int32_t k, int64_t batch, c
                    uint64_t* persist_bytes, uint64_t* transient_bytes, double* seconds);
 
 /* Fills an osdp_op_cost for this library's MLP operator as ONE call sees it:
- * pass = OSDP_FWD / OSDP_BWD.  model_bytes = the caller tensors live during the call (inputs, outputs, fp32
- * gradients); extra_transient = workspace at k = 1 minus the fixed scratch; extra_fixed = that scratch;
- * S = (2 h f + f + h) * sizeof(dtype); act_bytes = 0; gamma/delta = 0 (the caller calibrates them). */
+ * pass = OSDP_FWD / OSDP_BWD.  model_bytes = the model states live during the call (W1, W2, b1, b2; in the backward
+ * also the fp32 gradients dW1, dW2, db1, db2) - the part ZDP divides by N; act_bytes = the tokens x hidden tensors
+ * of the call (X, Y forward; X, dY, dX backward) per unit batch, ONE UNIT OF BATCH = desc->tokens TOKENS (evaluate
+ * with batch = 1 for the call as described); extra_transient = workspace at k = 1 minus the fixed scratch;
+ * extra_fixed = that scratch; S = (2 h f + f + h) * sizeof(dtype); gamma/delta = 0 (the caller calibrates them).
+ * The ZDP rows of the planner describe a sharded placement of the model states; on one GPU (N = 1) they coincide
+ * with DP, and the multi-GPU execution of a ZDP decision is osdp_zdp_ffn_split_mlp_* below. */
 int osdp_mlp_op_cost(const osdp_mlp_desc* desc, int pass, osdp_op_cost* out);
 int osdp_ffn_split_mlp_op_cost(const osdp_mlp_desc* desc, int pass, osdp_op_cost* out);   /* ffn-axis split, see above */
 

@@ -99,6 +99,7 @@ _lib.osdp_get_tuning.restype = C.c_int64
 _lib.osdp_get_tuning.argtypes = [C.c_int]
 OSDP_TUNE_MT2_MIN_K, OSDP_TUNE_MT2_MIN_TILES, OSDP_TUNE_WAVE_SYNC, OSDP_TUNE_BAND_MIB = 0, 1, 2, 3
 OSDP_TUNE_CLUSTER_MIN_TILES = 4
+OSDP_TUNE_MT2_MIN_K_ACC = 5
 _lib.osdp_trace_read.restype = C.c_int64
 _lib.osdp_trace_read.argtypes = [C.c_int64, C.POINTER(C.c_int32), C.POINTER(C.c_float)]
 _lib.osdp_step_name.restype = C.c_char_p
@@ -106,9 +107,9 @@ _lib.osdp_step_name.argtypes = [C.c_int]
 
 
 class OsdpError(RuntimeError):
-    def __init__(self, status: int, where: str):
+    def __init__(self, status: int, where: str, detail: str = ""):
         self.status = status
-        msg = f"{where}: {osdp_status_string(status)} (status {status})"
+        msg = f"{where}: {osdp_status_string(status)} (status {status})" + (f": {detail}" if detail else "")
         if status == OSDP_ERR_CUDA:
             msg += f": {osdp_last_cuda_error()}"
         super().__init__(msg)
@@ -181,7 +182,6 @@ def _ptr(t):
         return None
     if isinstance(t, int):
         return t
-    assert t.is_contiguous(), "osdp tensors are dense row-major"
     return t.data_ptr()
 
 
@@ -191,27 +191,105 @@ def _stream_ptr(stream):
     return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
 
 
-def osdp_split_mlp_forward(desc, X, W1, b1, W2, b2, Y, workspace, workspace_bytes=None, stream=None, check=True):
-    """Enqueue the split forward.  Tensors are torch CUDA tensors (or raw device addresses)."""
+_TORCH_DTYPE = {OSDP_F32: torch.float32, OSDP_BF16: torch.bfloat16}
+
+
+def _validate(where, desc, spec, workspace, workspace_bytes):
+    """Marshalling checks (no arithmetic of the method): every torch tensor handed to the C ABI must be a dense CUDA
+    tensor of the dtype and element count the descriptor implies, all on one device; raw integer addresses are taken
+    on trust.  Returns that device (or None) so the call can run with it current - the library launches on the
+    calling thread's current device.  Returns (device, status, detail)."""
+    T, h, f = desc.tokens, desc.hidden, desc.ffn
+    st = _TORCH_DTYPE.get(desc.dtype)
+    numel = {"X": T * h, "Y": T * h, "dY": T * h, "dX": T * h, "W1": h * f, "W2": f * h, "b1": f, "b2": h,
+             "dW1": h * f, "dW2": f * h, "db1": f, "db2": h}
+    dev = None
+    for name, t in spec:
+        if t is None or isinstance(t, int):
+            continue
+        want = torch.float32 if name in ("dW1", "dW2", "db1", "db2") else st
+        if not t.is_cuda:
+            return None, OSDP_ERR_ARG, f"{name} is not a CUDA tensor"
+        if not t.is_contiguous():
+            return None, OSDP_ERR_ARG, f"{name} is not dense row-major"
+        if want is not None and t.dtype != want:
+            return None, OSDP_ERR_DTYPE, f"{name} has dtype {t.dtype}, descriptor needs {want}"
+        if t.numel() != numel[name]:
+            return None, OSDP_ERR_SHAPE, f"{name} has {t.numel()} elements, descriptor needs {numel[name]}"
+        if dev is not None and t.device != dev:
+            return None, OSDP_ERR_ARG, f"{name} is on {t.device}, other tensors on {dev}"
+        dev = t.device
+    if workspace is not None and not isinstance(workspace, int):
+        if not workspace.is_cuda or not workspace.is_contiguous():
+            return None, OSDP_ERR_WORKSPACE, f"workspace must be a dense CUDA tensor"
+        if dev is not None and workspace.device != dev:
+            return None, OSDP_ERR_ARG, f"workspace is on {workspace.device}, tensors on {dev}"
+        if workspace_bytes > workspace.numel() * workspace.element_size():
+            return None, OSDP_ERR_WORKSPACE, f"workspace_bytes exceeds the workspace tensor"
+        dev = dev or workspace.device
+    return dev, OSDP_OK, ""
+
+
+class _on_device:
+    """Runs the C call with the tensors' device current (a no-op when it already is, or when only raw addresses came)."""
+
+    def __init__(self, dev):
+        self.ctx = torch.cuda.device(dev) if dev is not None and dev.index != torch.cuda.current_device() else None
+
+    def __enter__(self):
+        if self.ctx is not None:
+            self.ctx.__enter__()
+
+    def __exit__(self, *a):
+        if self.ctx is not None:
+            self.ctx.__exit__(*a)
+
+
+def _call_fwd(fn, where, desc, X, W1, b1, W2, b2, Y, workspace, workspace_bytes, stream, check):
     if workspace_bytes is None:
         workspace_bytes = workspace.numel() * workspace.element_size()
-    st = _lib.osdp_split_mlp_forward(C.byref(desc), _ptr(X), _ptr(W1), _ptr(b1), _ptr(W2), _ptr(b2), _ptr(Y),
-                                     _ptr(workspace), int(workspace_bytes), _stream_ptr(stream))
+    dev, vs, detail = _validate(where, desc, (("X", X), ("W1", W1), ("b1", b1), ("W2", W2), ("b2", b2), ("Y", Y)),
+                                workspace, int(workspace_bytes))
+    if vs != OSDP_OK:
+        if check:
+            raise OsdpError(vs, where, detail)
+        return vs
+    with _on_device(dev):
+        st = fn(C.byref(desc), _ptr(X), _ptr(W1), _ptr(b1), _ptr(W2), _ptr(b2), _ptr(Y), _ptr(workspace),
+                int(workspace_bytes), _stream_ptr(stream))
     if check and st != OSDP_OK:
-        raise OsdpError(st, "osdp_split_mlp_forward")
+        raise OsdpError(st, where)
     return st
+
+
+def _call_bwd(fn, where, desc, X, W1, b1, W2, b2, dY, dX, dW1, db1, dW2, db2, workspace, workspace_bytes, stream, check):
+    if workspace_bytes is None:
+        workspace_bytes = workspace.numel() * workspace.element_size()
+    dev, vs, detail = _validate(where, desc, (("X", X), ("W1", W1), ("b1", b1), ("W2", W2), ("b2", b2), ("dY", dY),
+                                              ("dX", dX), ("dW1", dW1), ("db1", db1), ("dW2", dW2), ("db2", db2)),
+                                workspace, int(workspace_bytes))
+    if vs != OSDP_OK:
+        if check:
+            raise OsdpError(vs, where, detail)
+        return vs
+    with _on_device(dev):
+        st = fn(C.byref(desc), _ptr(X), _ptr(W1), _ptr(b1), _ptr(W2), _ptr(b2), _ptr(dY), _ptr(dX), _ptr(dW1),
+                _ptr(db1), _ptr(dW2), _ptr(db2), _ptr(workspace), int(workspace_bytes), _stream_ptr(stream))
+    if check and st != OSDP_OK:
+        raise OsdpError(st, where)
+    return st
+
+
+def osdp_split_mlp_forward(desc, X, W1, b1, W2, b2, Y, workspace, workspace_bytes=None, stream=None, check=True):
+    """Enqueue the split forward.  Tensors are torch CUDA tensors (or raw device addresses)."""
+    return _call_fwd(_lib.osdp_split_mlp_forward, "osdp_split_mlp_forward", desc, X, W1, b1, W2, b2, Y, workspace,
+                     workspace_bytes, stream, check)
 
 
 def osdp_split_mlp_backward(desc, X, W1, b1, W2, b2, dY, dX, dW1, db1, dW2, db2, workspace, workspace_bytes=None,
                             stream=None, check=True):
-    if workspace_bytes is None:
-        workspace_bytes = workspace.numel() * workspace.element_size()
-    st = _lib.osdp_split_mlp_backward(C.byref(desc), _ptr(X), _ptr(W1), _ptr(b1), _ptr(W2), _ptr(b2), _ptr(dY),
-                                      _ptr(dX), _ptr(dW1), _ptr(db1), _ptr(dW2), _ptr(db2), _ptr(workspace),
-                                      int(workspace_bytes), _stream_ptr(stream))
-    if check and st != OSDP_OK:
-        raise OsdpError(st, "osdp_split_mlp_backward")
-    return st
+    return _call_bwd(_lib.osdp_split_mlp_backward, "osdp_split_mlp_backward", desc, X, W1, b1, W2, b2, dY, dX, dW1, db1,
+                     dW2, db2, workspace, workspace_bytes, stream, check)
 
 
 def osdp_ffn_split_mlp_workspace_bytes(desc: osdp_mlp_desc, pass_: int) -> int:
@@ -219,25 +297,14 @@ def osdp_ffn_split_mlp_workspace_bytes(desc: osdp_mlp_desc, pass_: int) -> int:
 
 
 def osdp_ffn_split_mlp_forward(desc, X, W1, b1, W2, b2, Y, workspace, workspace_bytes=None, stream=None, check=True):
-    if workspace_bytes is None:
-        workspace_bytes = workspace.numel() * workspace.element_size()
-    st = _lib.osdp_ffn_split_mlp_forward(C.byref(desc), _ptr(X), _ptr(W1), _ptr(b1), _ptr(W2), _ptr(b2), _ptr(Y),
-                                         _ptr(workspace), int(workspace_bytes), _stream_ptr(stream))
-    if check and st != OSDP_OK:
-        raise OsdpError(st, "osdp_ffn_split_mlp_forward")
-    return st
+    return _call_fwd(_lib.osdp_ffn_split_mlp_forward, "osdp_ffn_split_mlp_forward", desc, X, W1, b1, W2, b2, Y,
+                     workspace, workspace_bytes, stream, check)
 
 
 def osdp_ffn_split_mlp_backward(desc, X, W1, b1, W2, b2, dY, dX, dW1, db1, dW2, db2, workspace, workspace_bytes=None,
                                 stream=None, check=True):
-    if workspace_bytes is None:
-        workspace_bytes = workspace.numel() * workspace.element_size()
-    st = _lib.osdp_ffn_split_mlp_backward(C.byref(desc), _ptr(X), _ptr(W1), _ptr(b1), _ptr(W2), _ptr(b2), _ptr(dY),
-                                          _ptr(dX), _ptr(dW1), _ptr(db1), _ptr(dW2), _ptr(db2), _ptr(workspace),
-                                          int(workspace_bytes), _stream_ptr(stream))
-    if check and st != OSDP_OK:
-        raise OsdpError(st, "osdp_ffn_split_mlp_backward")
-    return st
+    return _call_bwd(_lib.osdp_ffn_split_mlp_backward, "osdp_ffn_split_mlp_backward", desc, X, W1, b1, W2, b2, dY, dX,
+                     dW1, db1, dW2, db2, workspace, workspace_bytes, stream, check)
 
 
 def osdp_ffn_split_mlp_op_cost(desc: osdp_mlp_desc, pass_: int) -> osdp_op_cost:

@@ -31,6 +31,7 @@
 #include <cuda.h>
 
 #include <atomic>
+#include <mutex>
 
 #include "common.cuh"
 #include "epilogue_math.cuh"
@@ -46,7 +47,8 @@ constexpr int BLOCK_K = 64;
 constexpr int UMMA_K = 16;
 // Kernel selection knobs (osdp_set_tuning): defaults are the measured best on C3/C4.
 struct Tuning {
-  std::atomic<int64_t> mt2_min_k{4096};     // MT = 2 from this contraction length on
+  std::atomic<int64_t> mt2_min_k{4096};     // MT = 2 from this contraction length on (bf16-output epilogues)
+  std::atomic<int64_t> mt2_min_k_acc{4096}; // the same for the fp32-accumulate epilogue (dW GEMMs: K = slice rows)
   std::atomic<int64_t> mt2_min_tiles{0};    // 0: MT = 2 when it idles at most ~10 % more MMA slots than MT = 1; > 0: plain threshold
   std::atomic<int64_t> wave_sync{1};        // line the producers up at tile boundaries (MT = 2 launches)
   std::atomic<int64_t> band_mib{32};        // L2 budget for the A rows of one raster band
@@ -56,16 +58,12 @@ inline Tuning& tuning() {
   static Tuning t;
   return t;
 }
-#ifndef OSDP_WAIT_SLEEP_NS
-#define OSDP_WAIT_SLEEP_NS 0      // > 0: nanosleep between failed mbarrier polls of the long (epilogue) waits
-#endif
 constexpr int kTmemCols = 512;
 constexpr int kThreads = 384;      // warps 0-3: TMA, MMA, TMEM alloc, (idle); warps 4-11: epilogue
 constexpr int kEpiWarp0 = 4;
 constexpr int kNumEpiWarps = 8;    // two per TMEM lane quarter (warp % 4), taking alternate column chunks
 constexpr uint32_t kBStageBytes = HALF_N * BLOCK_K * 2;    // 16 KiB (this CTA's half of the B tile)
 constexpr uint32_t kStoreBufBytes = 32 * 128;              // one warp's 32 rows x 128 B output segment
-constexpr uint32_t kSmemStore = kNumEpiWarps * kStoreBufBytes;   // 32 KiB
 
 // Two tile shapes share the kernel.  MT = M-halves (UMMAs of 128 rows) per CTA:
 //   MT = 1: CTA 128 x 256, pair 256 x 256; TMEM holds TWO accumulator stages, so the epilogue of tile i overlaps
@@ -74,29 +72,29 @@ constexpr uint32_t kSmemStore = kNumEpiWarps * kStoreBufBytes;   // 32 KiB
 //           exposed); 4 smem stages of 48 KiB; 96 KiB of operands per 16.8 MFLOP k-block, i.e. 25 % less
 //           L2 -> SM -> smem traffic per flop.  Large GEMMs run power-limited, where that traffic is what
 //           decides the clock, so long-K GEMMs take MT = 2.
-template <int MT>
+template <int MT, int NBUF>
 struct TileCfg {
   static constexpr int kCtaM = MT * BLOCK_M;       // rows per CTA
   static constexpr int kPairM = 2 * kCtaM;         // rows per pair tile
-  static constexpr int kStages = MT == 1 ? 6 : 4;
+  // NBUF = output staging buffers per epilogue warp.  The fp32 epilogue (EPI_ACCUM_F32) moves twice the bytes of the
+  // bf16 ones and a warp with ONE buffer waits, chunk after chunk, until TMA has read the previous chunk out
+  // (~15 k cycles to drain a 512 x 256 fp32 tile, exposed at MT = 2); with two buffers the wait disappears.  The second
+  // buffer is paid for with one ring stage.
+  static constexpr int kStoreBufs = NBUF;
+  static constexpr uint32_t kSmemStore = kNumEpiWarps * NBUF * kStoreBufBytes;   // 32 / 64 KiB
+  static constexpr int kStages = (MT == 1 ? 6 : 4) - (NBUF - 1);
   static constexpr int kAccStages = 2 / MT;
   static constexpr uint32_t kAStageBytes = kCtaM * BLOCK_K * 2;          // 16 / 32 KiB
   static constexpr uint32_t kStageBytes = kAStageBytes + kBStageBytes;   // per CTA; the leader's barrier expects 2x
-  static constexpr uint32_t kSmemTiles = kStages * kStageBytes;          // 192 KiB
+  static constexpr uint32_t kSmemTiles = kStages * kStageBytes;
   static constexpr uint32_t kSmemBytes = kSmemTiles + kSmemStore + 1024 /*align slack*/ + 256 /*barriers*/;
+  static_assert(kSmemBytes <= 227 * 1024, "shared memory per CTA");
 };
 
-// L2 cache-hint descriptors (what createpolicy.fractional.L2::evict_*.b64 with fraction 1.0 produces).
+// L2 cache-hint descriptor of the operand loads: evict_normal (what createpolicy.fractional.L2::evict_normal produces).
+// evict_first on the streamed operand / evict_last on the band's rows were measured and doubled the DRAM reads
+// (DESIGN.md section 7), so every load uses the default policy.
 constexpr uint64_t kEvictNormal = 0x1000000000000000ull;
-constexpr uint64_t kEvictFirst = 0x12F0000000000000ull;
-constexpr uint64_t kEvictLast = 0x14F0000000000000ull;
-#ifndef OSDP_HINT_A
-#define OSDP_HINT_A 0     // 0 normal, 1 evict_first, 2 evict_last (both hints measured worse: DESIGN.md section 7)
-#endif
-#ifndef OSDP_HINT_B
-#define OSDP_HINT_B 0
-#endif
-__host__ __device__ constexpr uint64_t hint_policy(int h) { return h == 1 ? kEvictFirst : h == 2 ? kEvictLast : kEvictNormal; }
 
 // ---------------------------------------------------------------------------------------------- PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -170,28 +168,10 @@ __device__ __forceinline__ void cluster_sync_relaxed() {
   asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");
   asm volatile("barrier.cluster.wait.aligned;" ::: "memory");
 }
-// Long waits (an epilogue warp waiting a whole main loop for its accumulator): optionally back off between polls.
-__device__ __forceinline__ void mbar_wait_long(uint32_t bar, uint32_t parity) {
-#if OSDP_WAIT_SLEEP_NS > 0
-  if (mbar_try_wait(bar, parity)) return;
-  uint64_t t0 = 0;
-  uint32_t spins = 0;
-  while (!mbar_try_wait(bar, parity)) {
-    __nanosleep(OSDP_WAIT_SLEEP_NS);
-    if ((++spins & 0xFFFu) == 0) {
-      const uint64_t now = global_timer_ns();
-      if (t0 == 0) t0 = now;
-      else if (now - t0 > 20ull * 1000 * 1000 * 1000) __trap();
-    }
-  }
-#else
-  mbar_wait(bar, parity);
-#endif
-}
 __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 
 // dst: this CTA's smem; bar: shared::cluster address of the mbarrier that receives complete_tx (the leader's).
-// policy: an L2 cache-hint descriptor (kEvictFirst / kEvictNormal / kEvictLast below).
+// policy: an L2 cache-hint descriptor (kEvictNormal below).
 __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c_inner, int c_outer,
                                             uint64_t policy) {
   asm volatile(
@@ -317,36 +297,38 @@ template <int EPI>
 struct EpiTraits {
   static constexpr bool kF32Out = (EPI == EPI_ACCUM_F32);
   static constexpr int kChunkCols = kF32Out ? 32 : 64;
+  // Staging buffers per epilogue warp (TileCfg).  Two buffers (and one ring stage fewer) remove the wait for the
+  // previous TMA store in the exposed MT = 2 epilogue; measured twice (bf16 and fp32 outputs, C4 k = 1 / 4 / 16): no
+  // gain at the power cap and -2 % at k = 16 from the lost stage, so one buffer it is.
+  static constexpr int kStoreBufs = 1;
 };
 
-// Per-warp output staging: one buffer of 32 rows x 128 B (128B swizzle: 16-byte chunk j of row r sits at chunk
+// Per-warp output staging: NBUF buffers of 32 rows x 128 B (128B swizzle: 16-byte chunk j of row r sits at chunk
 // j ^ (r & 7), which is also what makes the 16-byte st.shared of 8 consecutive rows conflict-free).  A warp fills
 // it, hands it to TMA and meanwhile loads and computes its next chunk; the second warp of the same lane quarter
 // covers the remaining latency.
+template <int NBUF>
 struct StorePipe {
-  uint32_t buf;     // smem address of this warp's buffer
+  uint32_t base;    // smem address of this warp's NBUF buffers
   int lane;
+  int cur = 0;      // buffer the next chunk goes to
+  __device__ __forceinline__ uint32_t buf() const { return base + (uint32_t)cur * kStoreBufBytes; }
   __device__ __forceinline__ void begin() const {
-#ifdef OSDP_DBG_NOSTORE
-    return;
-#endif
-    if (lane == 0) bulk_wait_read<0>();   // the previous store has read the buffer out
+    if (lane == 0) bulk_wait_read<NBUF - 1>();   // the store that last used this buffer has read it out
     __syncwarp();
   }
   __device__ __forceinline__ void put(int j, const uint4& v) const {
-    st_shared_v4(buf + lane * 128 + ((j ^ (lane & 7)) << 4), v);
+    st_shared_v4(buf() + lane * 128 + ((j ^ (lane & 7)) << 4), v);
   }
-  __device__ __forceinline__ void commit(const CUtensorMap* map, int c_inner, int c_outer, bool reduce_add) const {
-#ifdef OSDP_DBG_NOSTORE   // probe: stage in smem (keeps the math alive) but never issue the TMA store
-    return;
-#endif
+  __device__ __forceinline__ void commit(const CUtensorMap* map, int c_inner, int c_outer, bool reduce_add) {
     fence_proxy_async_smem();   // generic-proxy writes -> visible to the async proxy (TMA)
     __syncwarp();
     if (lane == 0) {
-      if (reduce_add) tma_reduce_add_2d(map, buf, c_inner, c_outer);
-      else            tma_store_2d(map, buf, c_inner, c_outer);
+      if (reduce_add) tma_reduce_add_2d(map, buf(), c_inner, c_outer);
+      else            tma_store_2d(map, buf(), c_inner, c_outer);
       bulk_commit();
     }
+    if constexpr (NBUF > 1) cur = cur + 1 == NBUF ? 0 : cur + 1;
   }
 };
 
@@ -410,8 +392,9 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
                        const __grid_constant__ CUtensorMap tmap_out0, const __grid_constant__ CUtensorMap tmap_out1,
                        const GemmShape shape, const EpiParams ep, const int group_m, unsigned int* wave_sync,
                        const int sync_kb) {
-  using Cfg = TileCfg<MT>;
+  using Cfg = TileCfg<MT, EpiTraits<EPI>::kStoreBufs>;
   constexpr int kStages = Cfg::kStages, kAccStages = Cfg::kAccStages;
+  constexpr uint32_t kSmemStore = Cfg::kSmemStore;
   constexpr int kCtaM = Cfg::kCtaM, kPairM = Cfg::kPairM;
   constexpr uint32_t kAStageBytes = Cfg::kAStageBytes, kStageBytes = Cfg::kStageBytes, kSmemTiles = Cfg::kSmemTiles;
   constexpr int kPairs = CM * CN;
@@ -484,14 +467,11 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
     for (int i = 0; i < CM; ++i) mask_b |= (uint16_t)(1u << (2 * (i * CN + pj) + (int)rank));
     // Tiles walk along n inside a band of group_m cluster-tile rows: the band's A rows are re-used by every wave
     // of the band (keep them in L2), B streams through once per band (let it go first).
-    constexpr uint64_t pol_a = hint_policy(OSDP_HINT_A), pol_b = hint_policy(OSDP_HINT_B);
+    constexpr uint64_t pol_a = kEvictNormal, pol_b = kEvictNormal;
     constexpr int kARows = kCtaM / CN;     // A rows (K-major) this CTA fetches; it is part pj of the tile
     constexpr int kBRows = HALF_N / CM;    // B columns this CTA fetches; it is part pi of the half-tile
     int stage = 0;
     uint32_t phase = 0;
-#ifdef OSDP_DBG_NOLOAD
-    int dbg_filled = 0;
-#endif
     int it = 0;
     bool waiting = true;   // false once a wait has timed out (see wave_wait)
     for (int t = cluster_id; t < num_tiles; t += num_clusters, ++it) {
@@ -503,16 +483,8 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
         waiting = __shfl_sync(0xFFFFFFFFu, lane == 0 ? (int)wave_wait(wave_sync, sync_base) : 0, 0) != 0;
       }
       const TileCoord tc = tile_coord(t, num_cm, num_cn, group_m);
-      int m0 = (tc.m_blk * CM + pi) * kPairM + (int)rank * kCtaM;       // this CTA's rows of A
-      int n0 = (tc.n_blk * CN + pj) * BLOCK_N + (int)rank * HALF_N;     // this CTA's half of the B tile
-#ifdef OSDP_DBG_PRIVTILE   // probe: every pair re-reads its own private operand tiles (all L2 hits, nothing shared)
-      m0 = (cluster_id * kPairM) % (num_m * kPairM) + (int)rank * kCtaM;
-      n0 = (cluster_id * BLOCK_N) % (num_n * BLOCK_N) + (int)rank * HALF_N;
-#endif
-#ifdef OSDP_DBG_SAMETILE   // probe: every pair re-reads tile (0, 0)
-      m0 = (int)rank * kCtaM;
-      n0 = (int)rank * HALF_N;
-#endif
+      const int m0 = (tc.m_blk * CM + pi) * kPairM + (int)rank * kCtaM;       // this CTA's rows of A
+      const int n0 = (tc.n_blk * CN + pj) * BLOCK_N + (int)rank * HALF_N;     // this CTA's half of the B tile
       for (int kb = 0; kb < num_kb; ++kb) {
         if (wave_sync != nullptr && sync_kb > 0 && kb > 0 && kb % sync_kb == 0) {   // stay in step inside the tile too
           int ok = 1;
@@ -523,24 +495,11 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
           waiting = waiting && __shfl_sync(0xFFFFFFFFu, ok, 0) != 0;
         }
         mbar_wait(empty_bar + 8 * stage, phase ^ 1);   // the slot is free in every CTA of the cluster
-#ifdef OSDP_DBG_NOLOAD   // probe: after the ring has been filled once, re-use its contents (no L2->SM traffic)
-        if (dbg_filled >= kStages) {
-          if (lane == 0 && leader) mbar_arrive(full_bar + 8 * stage);
-          __syncwarp();
-          if (++stage == kStages) { stage = 0; phase ^= 1; }
-          continue;
-        }
-        ++dbg_filled;
-#endif
         if (lane == 0) {
           const uint32_t fb_local = full_bar + 8 * stage;
           const uint32_t fb = mapa(fb_local, leader_crank);     // the pair leader's barrier receives both CTAs' bytes
           const uint32_t sa = smem_a + stage * kAStageBytes, sb = smem_b + stage * kBStageBytes;
-#ifdef OSDP_DBG_KWRAP
-          const int k0 = (kb % OSDP_DBG_KWRAP) * BLOCK_K;
-#else
           const int k0 = kb * BLOCK_K;
-#endif
           if (leader) mbar_expect_tx(fb_local, 2 * kStageBytes);
           if constexpr (kPairs == 1) {
             if constexpr (A_MAJOR == MAJOR_K) {
@@ -625,7 +584,7 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
     constexpr int kChunk = Tr::kChunkCols;
     const int q = warp % 4;                    // TMEM lane quarter this warp may access
     const int cg = (warp - kEpiWarp0) / 4;     // which of the two warps of that quarter: takes chunks cg, cg + 2, ...
-    const StorePipe pipe{smem_store + (uint32_t)(warp - kEpiWarp0) * kStoreBufBytes, lane};
+    StorePipe<Cfg::kStoreBufs> pipe{smem_store + (uint32_t)(warp - kEpiWarp0) * (Cfg::kStoreBufs * kStoreBufBytes), lane};
     const uint32_t tempty_leader = mapa(tempty_bar, leader_crank);
     const __nv_bfloat16* bias = reinterpret_cast<const __nv_bfloat16*>(ep.bias);
     constexpr bool kHasBias = (EPI == EPI_BIAS_GELU || EPI == EPI_BIAS || EPI == EPI_BIAS_GELU_DUAL);
@@ -665,7 +624,7 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
           bias_reg[ci] = c < shape.N ? __ldg(reinterpret_cast<const uint32_t*>(bias + c)) : 0u;   // N is even
         }
       }
-      mbar_wait_long(tfull_bar + 8 * as, aphase);
+      mbar_wait(tfull_bar + 8 * as, aphase);
       tc_fence_after();
       bool released = false;   // the accumulator stage goes back to the MMA warp right after this warp's last tcgen05.ld
 #pragma unroll 1
@@ -674,11 +633,7 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
         const int64_t row = row0 + lane;
         const bool row_ok = row < shape.M;
         const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * (MT * BLOCK_N) + h * BLOCK_N;
-        bool skip = row0 >= shape.M;   // nothing of this warp's band lies inside C (warp-uniform)
-#ifdef OSDP_DBG_NOEPI   // probe: drain nothing, hand the accumulator straight back (no tcgen05.ld, no stores)
-        skip = true;
-#endif
-        if (skip) continue;
+        if (row0 >= shape.M) continue;   // nothing of this warp's band lies inside C (warp-uniform)
 #pragma unroll 1
         for (int n = n0 + cg * kChunk; n < n_end; n += 2 * kChunk) {
           uint32_t acc[kChunk];
@@ -766,11 +721,57 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 EncodeTiledFn encode_tiled_fn();   // osdp_api.cu: resolved through cudaGetDriverEntryPoint (no libcuda link)
-int num_sms();                     // osdp_api.cu
+
+// Per-device launch state.  A process may drive several GPUs from several host threads (one device current per
+// thread), so nothing about a device is cached in a plain static: the SM count, the wave-sync counters (a __device__
+// array has one instance per device) and, per kernel instantiation, the shared-memory opt-in and the resident cluster
+// count are all kept per device ordinal and initialised under a mutex (osdp_api.cu).
+constexpr int kMaxDevices = 64;
+struct DeviceInfo {
+  int ordinal;
+  int sms;
+};
+int current_device(DeviceInfo* out);   // osdp_api.cu; OSDP_OK / OSDP_ERR_CUDA / OSDP_ERR_ARG (ordinal >= kMaxDevices)
+std::mutex& launch_setup_mutex();      // osdp_api.cu
 
 // Matrix stored row-major [outer x inner] with `ld` elements between rows; 128B-swizzled box.
+// cuTensorMapEncodeTiled is a pure function of its arguments and costs about a microsecond; a slice loop re-creates
+// the same few maps call after call (launch-bound shapes feel it), so each host thread keeps the last encodings in a
+// small direct-mapped cache keyed on every argument.
+struct TmapKey {
+  const void* ptr;
+  int64_t inner, outer, ld;
+  int box_inner, box_outer, f32;
+  bool operator==(const TmapKey& o) const {
+    return ptr == o.ptr && inner == o.inner && outer == o.outer && ld == o.ld && box_inner == o.box_inner &&
+           box_outer == o.box_outer && f32 == o.f32;
+  }
+};
+struct TmapCache {
+  static constexpr int kSlots = 256;
+  struct Slot {
+    TmapKey key;
+    CUtensorMap map;
+    bool used;
+  };
+  Slot slots[kSlots] = {};
+  static size_t slot_of(const TmapKey& k) {
+    uint64_t h = (uint64_t)(uintptr_t)k.ptr * 0x9E3779B97F4A7C15ull;
+    h ^= (uint64_t)k.inner * 0xBF58476D1CE4E5B9ull + (uint64_t)k.outer * 0x94D049BB133111EBull + (uint64_t)k.ld;
+    h ^= ((uint64_t)k.box_inner << 40) ^ ((uint64_t)k.box_outer << 20) ^ (uint64_t)k.f32;
+    h ^= h >> 29;
+    return (size_t)(h % kSlots);
+  }
+};
 inline int make_tmap(CUtensorMap* map, const void* ptr, int64_t inner, int64_t outer, int64_t ld, int box_inner,
                      int box_outer, bool f32 = false) {
+  static thread_local TmapCache cache;
+  const TmapKey key{ptr, inner, outer, ld, box_inner, box_outer, f32 ? 1 : 0};
+  TmapCache::Slot& slot = cache.slots[TmapCache::slot_of(key)];
+  if (slot.used && slot.key == key) {
+    *map = slot.map;
+    return OSDP_OK;
+  }
   EncodeTiledFn fn = encode_tiled_fn();
   if (!fn) return OSDP_ERR_CUDA;
   const cuuint64_t dims[2] = {(cuuint64_t)inner, (cuuint64_t)outer};
@@ -784,6 +785,9 @@ inline int make_tmap(CUtensorMap* map, const void* ptr, int64_t inner, int64_t o
     note_cuda_error(cudaErrorInvalidValue, "cuTensorMapEncodeTiled");
     return OSDP_ERR_CUDA;
   }
+  slot.key = key;
+  slot.map = *map;
+  slot.used = true;
   return OSDP_OK;
 }
 
@@ -791,7 +795,7 @@ inline int make_tmap(CUtensorMap* map, const void* ptr, int64_t inner, int64_t o
 template <int A_MAJOR, int B_MAJOR, int EPI, int MT, int CM, int CN>
 inline int launch_gemm_bf16_cluster(const void* A, int64_t lda, const void* B, int64_t ldb, const GemmShape& s,
                                     const EpiParams& ep, cudaStream_t st) {
-  using Cfg = TileCfg<MT>;
+  using Cfg = TileCfg<MT, EpiTraits<EPI>::kStoreBufs>;
   CUtensorMap ta, tb, to0, to1;
   int rc;
   // one TMA box = what ONE CTA fetches per k-block: 1/CN of its A rows, 1/CM of its B half (MN-major: 64-wide boxes)
@@ -826,18 +830,25 @@ inline int launch_gemm_bf16_cluster(const void* A, int64_t lda, const void* B, i
   attr[1].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 2;
-  static int max_clusters = 0;   // one process per GPU: attribute and occupancy are per function per device
+  DeviceInfo dev;
+  rc = current_device(&dev);
+  if (rc != OSDP_OK) return rc;
+  // per (kernel instantiation, device): the dynamic shared-memory opt-in and the number of co-resident clusters
+  static std::atomic<int> max_clusters_of[kMaxDevices];
+  int max_clusters = max_clusters_of[dev.ordinal].load(std::memory_order_acquire);
   if (max_clusters == 0) {
+    std::lock_guard<std::mutex> lock(launch_setup_mutex());
     OSDP_CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::kSmemBytes));
     int n = 0;
     cfg.gridDim = dim3(kCluster * 64);
-    if (kCluster == 2) n = num_sms() / 2;   // one CTA pair per TPC
+    if (kCluster == 2) n = dev.sms / 2;   // one CTA pair per TPC
     else OSDP_CUDA_TRY(cudaOccupancyMaxActiveClusters(&n, kernel, &cfg));
     if (n < 1) {
       note_cuda_error(cudaErrorInvalidConfiguration, "cudaOccupancyMaxActiveClusters");
       return OSDP_ERR_CUDA;
     }
     max_clusters = n;
+    max_clusters_of[dev.ordinal].store(n, std::memory_order_release);
   }
   const int num_m = (s.M + Cfg::kPairM - 1) / Cfg::kPairM, num_n = (s.N + BLOCK_N - 1) / BLOCK_N;   // pair tiles
   const int tiles = ((num_m + CM - 1) / CM) * ((num_n + CN - 1) / CN);                      // cluster tiles
@@ -853,9 +864,13 @@ inline int launch_gemm_bf16_cluster(const void* A, int64_t lda, const void* B, i
   const int64_t sync_mode = tuning().wave_sync.load();   // 0 off, 1 tile boundaries, q > 1: also every q k-blocks
   // (MT = 1 overlaps its epilogue with the next main loop, so a wait at the tile boundary would be exposed)
   if (MT == 2 && tiles > max_clusters && sync_mode != 0) {
-    static unsigned int* base = nullptr;
+    static std::atomic<unsigned int*> base_of[kMaxDevices];   // this device's instance of g_wave_sync
     static std::atomic<unsigned int> seq{0};
-    if (!base) OSDP_CUDA_TRY(cudaGetSymbolAddress(reinterpret_cast<void**>(&base), g_wave_sync));
+    unsigned int* base = base_of[dev.ordinal].load(std::memory_order_acquire);
+    if (!base) {
+      OSDP_CUDA_TRY(cudaGetSymbolAddress(reinterpret_cast<void**>(&base), g_wave_sync));
+      base_of[dev.ordinal].store(base, std::memory_order_release);
+    }
     wave_sync = base + (seq.fetch_add(1) % kWaveSyncSlots);
   }
   cudaError_t err;
@@ -885,7 +900,7 @@ inline int launch_gemm_bf16_cluster(const void* A, int64_t lda, const void* B, i
 template <int A_MAJOR, int B_MAJOR, int EPI, int MT>
 inline int launch_gemm_bf16_mt(const void* A, int64_t lda, const void* B, int64_t ldb, const GemmShape& s,
                                const EpiParams& ep, cudaStream_t st) {
-  const int64_t num_m = (s.M + TileCfg<MT>::kPairM - 1) / TileCfg<MT>::kPairM, num_n = (s.N + BLOCK_N - 1) / BLOCK_N;
+  const int64_t num_m = (s.M + (2 * MT * BLOCK_M) - 1) / (2 * MT * BLOCK_M), num_n = (s.N + BLOCK_N - 1) / BLOCK_N;
   const int64_t cluster_min_tiles = tuning().cluster_min_tiles.load();   // 0 = never
   if (OSDP_CM * OSDP_CN > 1 && cluster_min_tiles > 0 && num_m * num_n >= cluster_min_tiles)
     return launch_gemm_bf16_cluster<A_MAJOR, B_MAJOR, EPI, MT, OSDP_CM, OSDP_CN>(A, lda, B, ldb, s, ep, st);
@@ -894,9 +909,9 @@ inline int launch_gemm_bf16_mt(const void* A, int64_t lda, const void* B, int64_
 // Fraction of the machine's MMA slots that do useful work for pair tiles of pair_m rows: padding of M to whole
 // tiles (N is a multiple of 256 in every workload; its padding is the same for both shapes) times the fill of
 // the last wave.
-inline double tile_efficiency(const GemmShape& s, int pair_m) {
+inline double tile_efficiency(const GemmShape& s, int pair_m, int sms) {
   const int64_t num_m = (s.M + pair_m - 1) / pair_m, num_n = (s.N + BLOCK_N - 1) / BLOCK_N;
-  const int64_t tiles = num_m * num_n, pairs = num_sms() / 2;
+  const int64_t tiles = num_m * num_n, pairs = sms / 2;
   const int64_t waves = (tiles + pairs - 1) / pairs;
   return ((double)s.M / (double)(num_m * pair_m)) * ((double)tiles / (double)(waves * pairs));
 }
@@ -909,8 +924,12 @@ inline int launch_gemm_bf16(const void* A, int64_t lda, const void* B, int64_t l
   // MT = 2 saves a quarter of the operand traffic; it is not worth more than ~10 % of idle MMA slots (padding of M
   // to 512 rows, fill of the last wave).  A positive OSDP_TUNE_MT2_MIN_TILES replaces that rule by a plain tile-count
   // threshold (tests use it to force MT = 2 on small shapes).
-  const bool fits = min_tiles > 0 ? tiles2 >= min_tiles : tile_efficiency(s, 512) >= 0.9 * tile_efficiency(s, 256);
-  if (s.K >= tuning().mt2_min_k.load() && fits)
+  DeviceInfo dev;
+  const int drc = current_device(&dev);
+  if (drc != OSDP_OK) return drc;
+  const bool fits = min_tiles > 0 ? tiles2 >= min_tiles : tile_efficiency(s, 512, dev.sms) >= 0.9 * tile_efficiency(s, 256, dev.sms);
+  const int64_t min_k = EpiTraits<EPI>::kF32Out ? tuning().mt2_min_k_acc.load() : tuning().mt2_min_k.load();
+  if (s.K >= min_k && fits)
     return launch_gemm_bf16_mt<A_MAJOR, B_MAJOR, EPI, 2>(A, lda, B, ldb, s, ep, st);
   return launch_gemm_bf16_mt<A_MAJOR, B_MAJOR, EPI, 1>(A, lda, B, ldb, s, ep, st);
 }

@@ -71,15 +71,25 @@ EncodeTiledFn encode_tiled_fn() {
   if (!fn) note_cuda_error(cudaErrorNotSupported, "cudaGetDriverEntryPoint(cuTensorMapEncodeTiled)");
   return fn;
 }
-int num_sms() {
-  static int n = 0;
+std::mutex& launch_setup_mutex() {
+  static std::mutex m;
+  return m;
+}
+// Ordinal and SM count of the device current to the calling thread (cached per ordinal after the first query).
+int current_device(DeviceInfo* out) {
+  static std::atomic<int> sms_of[kMaxDevices];
+  int dev = 0;
+  OSDP_CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return OSDP_ERR_ARG;
+  int n = sms_of[dev].load(std::memory_order_acquire);
   if (n == 0) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+    OSDP_CUDA_TRY(cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev));
     if (n <= 0) n = 1;
+    sms_of[dev].store(n, std::memory_order_release);
   }
-  return n;
+  out->ordinal = dev;
+  out->sms = n;
+  return OSDP_OK;
 }
 }  // namespace sm100
 
@@ -234,6 +244,10 @@ int osdp_set_tuning(int key, int64_t value) {
       if (value < 0) return OSDP_ERR_ARG;
       t.cluster_min_tiles = value;
       return OSDP_OK;
+    case OSDP_TUNE_MT2_MIN_K_ACC:
+      if (value < 1) return OSDP_ERR_ARG;
+      t.mt2_min_k_acc = value;
+      return OSDP_OK;
     default: return OSDP_ERR_ARG;
   }
 }
@@ -246,6 +260,7 @@ int64_t osdp_get_tuning(int key) {
     case OSDP_TUNE_WAVE_SYNC: return t.wave_sync;
     case OSDP_TUNE_BAND_MIB: return t.band_mib;
     case OSDP_TUNE_CLUSTER_MIN_TILES: return t.cluster_min_tiles;
+    case OSDP_TUNE_MT2_MIN_K_ACC: return t.mt2_min_k_acc;
     default: return -1;
   }
 }
@@ -303,12 +318,16 @@ int osdp_mlp_op_cost(const osdp_mlp_desc* desc, int pass, osdp_op_cost* out) {
   const uint64_t T = desc->tokens, h = desc->hidden, f = desc->ffn, e = elem_size(desc->dtype);
   osdp_op_cost c = {};
   c.S = (double)((2 * h * f + f + h) * e);
+  // Model states (what ZDP shards) are the parameters and, in the backward, their fp32 gradients; the
+  // T x h tensors are activations of this call's token batch (one unit of batch = desc->tokens tokens).
   if (pass == OSDP_FWD) {
-    c.model_bytes = (2 * T * h + 2 * h * f + f + h) * e;             // X, Y, W1, W2, b1, b2
+    c.model_bytes = (2 * h * f + f + h) * e;                          // W1, W2, b1, b2
+    c.act_bytes = 2 * T * h * e;                                      // X, Y
     c.extra_transient = T * f * e;                                    // H
     c.extra_fixed = 0;
   } else {
-    c.model_bytes = (3 * T * h + 2 * h * f + f + h) * e + (2 * h * f + f + h) * 4;   // X, dY, dX, W, b; fp32 grads
+    c.model_bytes = (2 * h * f + f + h) * e + (2 * h * f + f + h) * 4;   // W, b; fp32 dW, db
+    c.act_bytes = 3 * T * h * e;                                      // X, dY, dX
     c.extra_transient = 2 * T * f * e;                                // Z/dZ and H
     c.extra_fixed = reduce_scratch_bytes(desc);
   }
@@ -423,11 +442,13 @@ int osdp_ffn_split_mlp_op_cost(const osdp_mlp_desc* desc, int pass, osdp_op_cost
   c.S = (double)((2 * h * f + f + h) * e);
   const uint64_t acc = align_up((size_t)T * h * 4, 256);   // cross-slice fp32 accumulator (any k > 1)
   if (pass == OSDP_FWD) {
-    c.model_bytes = (2 * T * h + 2 * h * f + f + h) * e;
+    c.model_bytes = (2 * h * f + f + h) * e;
+    c.act_bytes = 2 * T * h * e;
     c.extra_transient = T * f * e;
     c.extra_fixed = acc;
   } else {
-    c.model_bytes = (3 * T * h + 2 * h * f + f + h) * e + (2 * h * f + f + h) * 4;
+    c.model_bytes = (2 * h * f + f + h) * e + (2 * h * f + f + h) * 4;
+    c.act_bytes = 3 * T * h * e;
     c.extra_transient = 2 * T * f * e;
     c.extra_fixed = acc + reduce_scratch_bytes(desc);
   }
@@ -474,7 +495,9 @@ int osdp_ffn_split_mlp_forward(const osdp_mlp_desc* desc, const void* X, const v
   }
   if (k > 1) {   // Y = storage(Yacc + b2)
     trace_set_step(10);
-    OSDP_TRY(launch_acc_to_out(dt, Yacc, b2, Y, T, (int)h, sm100::num_sms(), st));
+    sm100::DeviceInfo dev;
+    OSDP_TRY(sm100::current_device(&dev));
+    OSDP_TRY(launch_acc_to_out(dt, Yacc, b2, Y, T, (int)h, dev.sms, st));
   }
   return OSDP_OK;
 }
@@ -538,7 +561,9 @@ int osdp_ffn_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const 
   }
   if (k > 1) {   // dX = storage(dXacc)
     trace_set_step(10);
-    OSDP_TRY(launch_acc_to_out(dt, dXacc, nullptr, dX, T, (int)h, sm100::num_sms(), st));
+    sm100::DeviceInfo dev;
+    OSDP_TRY(sm100::current_device(&dev));
+    OSDP_TRY(launch_acc_to_out(dt, dXacc, nullptr, dX, T, (int)h, dev.sms, st));
   }
   return OSDP_OK;
 }

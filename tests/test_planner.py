@@ -422,7 +422,8 @@ def test_workspace_and_mlp_factors_match_cost_model(lib, T, h, f, dt, e):
             ws = lib.osdp_split_mlp_workspace_bytes(desc, pass_)
             assert ws == P.mlp_workspace_bytes(T, h, f, e, k, bwd)
             c = lib.osdp_mlp_op_cost(desc, pass_)
-            assert c.model_bytes == P.mlp_persistent_bytes(T, h, f, e, bwd)
+            assert c.model_bytes + c.act_bytes == P.mlp_persistent_bytes(T, h, f, e, bwd)
+            assert c.act_bytes == (3 if bwd else 2) * T * h * e          # only the T x h tensors scale with the batch
             assert c.extra_fixed == (P.mlp_reduce_scratch_bytes(h, f) if bwd else 0)
             assert c.extra_transient == (2 if bwd else 1) * T * f * e
             # cost model predicts the workspace: sliceable/k + fixed, up to 256 B padding per buffer and
@@ -430,6 +431,24 @@ def test_workspace_and_mlp_factors_match_cost_model(lib, T, h, f, dt, e):
             pred = -(-c.extra_transient // k) + c.extra_fixed
             slack = (2 if bwd else 1) * (256 + (f * e if T % k else 0))
             assert 0 <= ws - pred <= slack
+
+
+def test_mlp_factors_zdp_shards_only_the_model_states(lib):
+    """ZDP divides M_model by N and nothing else; the T x h activations of the call must sit in
+    act_bytes (they scale with the batch and are never sharded)."""
+    T, h, f, e = 8192, 1024, 4096, 2
+    desc = lib.make_desc(T, h, f, 1, 4)
+    for pass_, n_act, grads in ((lib.OSDP_FWD, 2, 0), (lib.OSDP_BWD, 3, 4)):
+        c = lib.osdp_mlp_op_cost(desc, pass_)
+        params = 2 * h * f + f + h
+        assert c.model_bytes == params * (e + grads) and c.act_bytes == n_act * T * h * e
+        for N in (2, 8):
+            dev = lib.osdp_device(N, 0.0, 0.0, 1 << 62)
+            pd, td, _ = lib.osdp_cost_eval(c, lib.OSDP_DP, 4, 1, dev)
+            pz, tz, _ = lib.osdp_cost_eval(c, lib.OSDP_ZDP, 4, 1, dev)
+            assert td == tz and pd - pz == c.model_bytes - -(-c.model_bytes // N)
+            p2, _, _ = lib.osdp_cost_eval(c, lib.OSDP_DP, 4, 2, dev)
+            assert p2 - pd == c.act_bytes                                 # memory grows with the batch
 
 
 def test_descriptor_validation(lib):
