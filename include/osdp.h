@@ -158,7 +158,11 @@ typedef enum osdp_tune_key {
   OSDP_TUNE_WAVE_SYNC = 2,      /* default 1 */
   OSDP_TUNE_BAND_MIB = 3,       /* default 32 */
   OSDP_TUNE_CLUSTER_MIN_TILES = 4, /* default 0 (multicast clusters off) */
-  OSDP_TUNE_MT2_MIN_K_ACC = 5      /* OSDP_TUNE_MT2_MIN_K for the fp32-accumulate launches (dW GEMMs, K = slice rows) */
+  OSDP_TUNE_MT2_MIN_K_ACC = 5,     /* OSDP_TUNE_MT2_MIN_K for the fp32-accumulate launches (dW GEMMs, K = slice rows) */
+  OSDP_TUNE_FORK_MAX_TILES = 6     /* default 148: in the token-split backward, the launches that only depend on dZ_s
+                                      (dW2, dW1, dX, column sums) are enqueued side by side on helper streams that fork
+                                      from and join `stream` when each GEMM has at most this many 256 x 256 output tiles
+                                      (small slices: every launch is a fraction of a wave); 0 = always in sequence */
 } osdp_tune_key;
 int osdp_set_tuning(int key, int64_t value);
 int64_t osdp_get_tuning(int key);

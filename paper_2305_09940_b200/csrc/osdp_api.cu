@@ -186,6 +186,54 @@ int colsum2(int dtype, const void* dYs, int h, float* db2, const void* dZs, int 
   return launch_colsum2<float>((const float*)dYs, h, h, db2, (const float*)dZs, f, f, db1, rows, scratch, beta, st);
 }
 
+// ---- helper streams: independent launches of one slice side by side ------------------------------------------
+// Once dZ_s exists, dW2 (+)= H_s^T dY_s, dW1 (+)= X_s^T dZ_s, dX_s = dZ_s W1^T and the two column sums are independent
+// (SURVEY.md section 7 "co-scheduling").  On small slices each of them fills a fraction of the machine for a few
+// microseconds, most of it fixed cost, so they are enqueued side by side: the caller's stream forks into helper
+// streams (event record + wait) and joins them again before the next slice reuses the slice buffers.  Seen from the
+// caller the call still only adds work to `stream` in order (and stays CUDA-graph capturable: fork/join through events
+// becomes parallel branches).  Streams and events belong to the calling host thread and the current device, are
+// created on first use and never shared between host threads.
+constexpr int kForkBranches = 3;
+struct ForkCtx {
+  cudaStream_t side[kForkBranches] = {};
+  cudaEvent_t fork_ev = nullptr;
+  cudaEvent_t join_ev[kForkBranches] = {};
+  bool ready = false;
+};
+int fork_ctx(ForkCtx** out) {
+  static thread_local ForkCtx ctx[sm100::kMaxDevices];
+  sm100::DeviceInfo dev;
+  const int rc = sm100::current_device(&dev);
+  if (rc != OSDP_OK) return rc;
+  ForkCtx& c = ctx[dev.ordinal];
+  if (!c.ready) {
+    for (int i = 0; i < kForkBranches; ++i) {
+      OSDP_CUDA_TRY(cudaStreamCreateWithFlags(&c.side[i], cudaStreamNonBlocking));
+      OSDP_CUDA_TRY(cudaEventCreateWithFlags(&c.join_ev[i], cudaEventDisableTiming));
+    }
+    OSDP_CUDA_TRY(cudaEventCreateWithFlags(&c.fork_ev, cudaEventDisableTiming));
+    c.ready = true;
+  }
+  *out = &c;
+  return OSDP_OK;
+}
+// Everything enqueued on `st` so far happens before whatever is enqueued on the side streams from now on.
+int fork_from(ForkCtx* c, cudaStream_t st) {
+  OSDP_CUDA_TRY(cudaEventRecord(c->fork_ev, st));
+  for (int i = 0; i < kForkBranches; ++i) OSDP_CUDA_TRY(cudaStreamWaitEvent(c->side[i], c->fork_ev, 0));
+  return OSDP_OK;
+}
+// Everything enqueued on the side streams so far happens before whatever is enqueued on `st` from now on.
+int join_into(ForkCtx* c, cudaStream_t st) {
+  for (int i = 0; i < kForkBranches; ++i) {
+    OSDP_CUDA_TRY(cudaEventRecord(c->join_ev[i], c->side[i]));
+    OSDP_CUDA_TRY(cudaStreamWaitEvent(st, c->join_ev[i], 0));
+  }
+  return OSDP_OK;
+}
+inline int64_t tiles_256(int64_t m, int64_t n) { return ((m + 255) / 256) * ((n + 255) / 256); }
+
 #define OSDP_TRY(expr)            \
   do {                            \
     int _rc = (expr);             \
@@ -248,6 +296,10 @@ int osdp_set_tuning(int key, int64_t value) {
       if (value < 1) return OSDP_ERR_ARG;
       t.mt2_min_k_acc = value;
       return OSDP_OK;
+    case OSDP_TUNE_FORK_MAX_TILES:
+      if (value < 0) return OSDP_ERR_ARG;
+      t.fork_max_tiles = value;
+      return OSDP_OK;
     default: return OSDP_ERR_ARG;
   }
 }
@@ -261,6 +313,7 @@ int64_t osdp_get_tuning(int key) {
     case OSDP_TUNE_BAND_MIB: return t.band_mib;
     case OSDP_TUNE_CLUSTER_MIN_TILES: return t.cluster_min_tiles;
     case OSDP_TUNE_MT2_MIN_K_ACC: return t.mt2_min_k_acc;
+    case OSDP_TUNE_FORK_MAX_TILES: return t.fork_max_tiles;
     default: return -1;
   }
 }
@@ -390,6 +443,13 @@ int osdp_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const void
   void* Hs = (char*)workspace + buf;                     // H_s
   float* scratch = (float*)((char*)workspace + 2 * buf);   // column-sum partials
 
+  // Small slices: the three GEMMs and the column sums that only need dZ_s run side by side (helper streams above).
+  const int64_t ts_max = (T + desc->k - 1) / desc->k;
+  const int64_t fork_max = sm100::tuning().fork_max_tiles.load();
+  const bool fork = dt == OSDP_BF16 && fork_max > 0 && tiles_256(f, h) <= fork_max && tiles_256(ts_max, h) <= fork_max;
+  ForkCtx* fc = nullptr;
+  if (fork) OSDP_TRY(fork_ctx(&fc));
+
   int first = 1;
   for (int s = 0; s < desc->k; ++s) {
     const int64_t lo = (int64_t)s * T / desc->k, hi = (int64_t)(s + 1) * T / desc->k;
@@ -408,21 +468,25 @@ int osdp_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const void
     trace_set_step(4);
     EpiParams e4 = {nullptr, Zs, nullptr, Zs, f, 0};
     OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_DGELU>(dt, dYs, h, W2, h, GemmShape{Ts, (int)f, (int)h}, e4, st)));
+    if (fork) OSDP_TRY(fork_from(fc, st));
     // A5: dW2 (+)= H_s^T dY_s
     trace_set_step(5);
     EpiParams e5 = {nullptr, dW2, nullptr, nullptr, h, beta};
     OSDP_TRY((gemm<MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32>(dt, Hs, f, dYs, h, GemmShape{(int)f, (int)h, Ts}, e5, st)));
     // A8: db2 (+)= colsum(dY_s);  db1 (+)= colsum(dZ_s)
     trace_set_step(8);
-    OSDP_TRY(colsum2(dt, dYs, (int)h, db2, Zs, (int)f, db1, Ts, scratch, beta, st));
+    OSDP_TRY(colsum2(dt, dYs, (int)h, db2, Zs, (int)f, db1, Ts, scratch, beta, fork ? fc->side[2] : st));
     // A6: dW1 (+)= X_s^T dZ_s
     trace_set_step(6);
     EpiParams e6 = {nullptr, dW1, nullptr, nullptr, f, beta};
-    OSDP_TRY((gemm<MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32>(dt, Xs, h, Zs, f, GemmShape{(int)h, (int)f, Ts}, e6, st)));
+    OSDP_TRY((gemm<MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32>(dt, Xs, h, Zs, f, GemmShape{(int)h, (int)f, Ts}, e6,
+                                                      fork ? fc->side[0] : st)));
     // A7: dX_s = dZ_s W1^T
     trace_set_step(7);
     EpiParams e7 = {nullptr, dXs, nullptr, nullptr, h, 0};
-    OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_PLAIN>(dt, Zs, f, W1, f, GemmShape{Ts, (int)h, (int)f}, e7, st)));
+    OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_PLAIN>(dt, Zs, f, W1, f, GemmShape{Ts, (int)h, (int)f}, e7,
+                                                fork ? fc->side[1] : st)));
+    if (fork) OSDP_TRY(join_into(fc, st));   // the next slice overwrites Z_s / H_s
   }
   return OSDP_OK;
 }
