@@ -136,6 +136,44 @@ int osdp_ffn_split_mlp_backward(const osdp_mlp_desc* desc,
                                 void* dX, float* dW1, float* db1, float* dW2, float* db2,
                                 void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- Linear operator: the other operator type of the paper's models -----------------------------------------
+ * Table 1 counts two operators per layer, an attention block and an MLP block; the MatMuls of the
+ * attention block are plain Linear operators (minGPT's hidden -> 3 hidden QKV projection and hidden -> hidden output
+ * projection).  Operator splitting applies to them as to any MatMul:
+ *     forward : Y  = X W + b                 X [tokens x in], W [in x out], b [out] (optional), Y [tokens x out]
+ *     backward: dX = dY W^T [tokens x in];   dW = X^T dY [in x out] fp32;   db = colsum(dY) [out] fp32
+ * axis = OSDP_SPLIT_CONTRACTION (the paper-literal split: "the last dimension of the input data and the first
+ *   dimension of the operator are partitioned ... all computation results are summed"): slice s owns input features
+ *   [lo_s, lo_{s+1}), lo_s = floor(s * units / k) * unit, unit = 16 bytes of elements, units = in / unit.
+ *   Forward: Y (+)= X[:, lo:hi] W[lo:hi, :] summed over slices in an fp32 [tokens x out] accumulator (workspace, k > 1),
+ *   then + b and one rounding.  Backward: dX[:, lo:hi] and dW[lo:hi, :] belong to one slice each (written once).
+ * axis = OSDP_SPLIT_TOKENS (the north_star's axis): slice s = rows [floor(s T / k), floor((s+1) T / k)); Y_s, dX_s
+ *   are rows of the outputs, dW and db are summed over slices in fp32 ("=" on slice 0, "+=" after).
+ * Same conventions as the MLP calls (device pointers of the current device, 16-byte aligned, workspace 256-byte
+ * aligned and caller-owned, nothing allocated, only `stream` is used from the caller's point of view, status codes).
+ * b and db may be NULL when has_bias = 0.  dW, db are OVERWRITTEN.  workspace may be NULL when the size query says 0.
+ * osdp_split_linear_workspace_bytes: FWD = the fp32 accumulator (contraction axis, k > 1) else 0; BWD = the column-sum
+ * scratch 32 x out floats (has_bias) else 0; each rounded up to 256 B.  Returns a status; *bytes is written on OSDP_OK.
+ * osdp_linear_op_cost: cost-model factors of one call (like osdp_mlp_op_cost): model_bytes = W, b (+ fp32 dW, db in the
+ * backward), act_bytes = the tokens x in / tokens x out tensors of the call (one unit of batch = desc->tokens tokens),
+ * extra_fixed = the workspace, S = (in out + out) sizeof(dtype). */
+typedef enum osdp_split_axis { OSDP_SPLIT_TOKENS = 0, OSDP_SPLIT_CONTRACTION = 1 } osdp_split_axis;
+typedef struct osdp_linear_desc {
+  int64_t tokens;        /* T >= 1 */
+  int64_t in_features;   /* multiple of 8 (bf16) / 4 (f32) */
+  int64_t out_features;  /* multiple of 8 (bf16) / 4 (f32) */
+  int32_t dtype;         /* osdp_dtype */
+  int32_t k;             /* slices: 1 <= k <= tokens (token axis) or <= in_features / unit (contraction axis) */
+  int32_t axis;          /* osdp_split_axis */
+  int32_t has_bias;      /* 0 / 1 */
+} osdp_linear_desc;
+int osdp_split_linear_workspace_bytes(const osdp_linear_desc* desc, int pass, size_t* bytes);
+int osdp_split_linear_forward(const osdp_linear_desc* desc, const void* X, const void* W, const void* b, void* Y,
+                              void* workspace, size_t workspace_bytes, void* stream);
+int osdp_split_linear_backward(const osdp_linear_desc* desc, const void* X, const void* W, const void* dY,
+                               void* dX, float* dW, float* db, void* workspace, size_t workspace_bytes, void* stream);
+/* (osdp_linear_op_cost is declared below, after osdp_op_cost.) */
+
 /* Number of kernel launches the last forward/backward call of the calling thread enqueued (for bench.py's
  * gpu_launches claim). */
 int64_t osdp_last_launch_count(void);
@@ -159,10 +197,12 @@ typedef enum osdp_tune_key {
   OSDP_TUNE_BAND_MIB = 3,       /* default 32 */
   OSDP_TUNE_CLUSTER_MIN_TILES = 4, /* default 0 (multicast clusters off) */
   OSDP_TUNE_MT2_MIN_K_ACC = 5,     /* OSDP_TUNE_MT2_MIN_K for the fp32-accumulate launches (dW GEMMs, K = slice rows) */
-  OSDP_TUNE_FORK_MAX_TILES = 6     /* default 148: in the token-split backward, the launches that only depend on dZ_s
+  OSDP_TUNE_FORK_MAX_TILES = 6     /* default 256: in the token-split backward, the launches that only depend on dZ_s
                                       (dW2, dW1, dX, column sums) are enqueued side by side on helper streams that fork
                                       from and join `stream` when each GEMM has at most this many 256 x 256 output tiles
-                                      (small slices: every launch is a fraction of a wave); 0 = always in sequence */
+                                      (small slices: every launch is a wave or two; measured +4-8 % at C2, +5 % at the
+                                      C5 layer shape, neutral to -1 % at C3 / C4, which the default excludes); 0 = always
+                                      in sequence */
 } osdp_tune_key;
 int osdp_set_tuning(int key, int64_t value);
 int64_t osdp_get_tuning(int key);
@@ -220,6 +260,7 @@ int osdp_cost_eval(const osdp_op_cost* op, int mode, int32_t k, int64_t batch, c
  * with DP, and the multi-GPU execution of a ZDP decision is osdp_zdp_ffn_split_mlp_* below. */
 int osdp_mlp_op_cost(const osdp_mlp_desc* desc, int pass, osdp_op_cost* out);
 int osdp_ffn_split_mlp_op_cost(const osdp_mlp_desc* desc, int pass, osdp_op_cost* out);   /* ffn-axis split, see above */
+int osdp_linear_op_cost(const osdp_linear_desc* desc, int pass, osdp_op_cost* out);        /* Linear operator, see above */
 
 /* Search engine (Algorithm 1 lines 4-11 at a fixed batch; PAPER.md:149 DFS with two prunings).
  * Decision per operator: mode in {DP, ZDP} x k in k_candidates (ascending, each >= 1).  Minimises

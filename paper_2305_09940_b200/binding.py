@@ -34,12 +34,21 @@ EXPORTS = (
     "osdp_mlp_op_cost", "osdp_plan", "osdp_plan_batch", "osdp_trace_enable", "osdp_trace_read", "osdp_step_name",
     "osdp_set_tuning", "osdp_get_tuning", "osdp_ffn_split_mlp_workspace_bytes", "osdp_ffn_split_mlp_forward",
     "osdp_ffn_split_mlp_backward", "osdp_ffn_split_mlp_op_cost", "osdp_cost_eval_mixed", "osdp_plan_mixed",
+    "osdp_split_linear_workspace_bytes", "osdp_split_linear_forward", "osdp_split_linear_backward", "osdp_linear_op_cost",
 )
 
 
 class osdp_mlp_desc(C.Structure):
     _fields_ = [("tokens", C.c_int64), ("hidden", C.c_int64), ("ffn", C.c_int64), ("dtype", C.c_int32),
                 ("k", C.c_int32)]
+
+
+class osdp_linear_desc(C.Structure):
+    _fields_ = [("tokens", C.c_int64), ("in_features", C.c_int64), ("out_features", C.c_int64), ("dtype", C.c_int32),
+                ("k", C.c_int32), ("axis", C.c_int32), ("has_bias", C.c_int32)]
+
+
+OSDP_SPLIT_TOKENS, OSDP_SPLIT_CONTRACTION = 0, 1
 
 
 class osdp_op_cost(C.Structure):
@@ -91,6 +100,14 @@ _lib.osdp_plan_batch.argtypes = [C.POINTER(osdp_op_cost), C.c_int32, C.POINTER(o
                                  C.POINTER(C.c_int64), C.POINTER(C.c_double), C.POINTER(C.c_uint64)]
 
 
+_lib.osdp_split_linear_workspace_bytes.restype = C.c_int
+_lib.osdp_split_linear_workspace_bytes.argtypes = [C.POINTER(osdp_linear_desc), C.c_int, C.POINTER(C.c_size_t)]
+_lib.osdp_split_linear_forward.restype = C.c_int
+_lib.osdp_split_linear_forward.argtypes = [C.POINTER(osdp_linear_desc)] + [C.c_void_p] * 5 + [C.c_size_t, C.c_void_p]
+_lib.osdp_split_linear_backward.restype = C.c_int
+_lib.osdp_split_linear_backward.argtypes = [C.POINTER(osdp_linear_desc)] + [C.c_void_p] * 7 + [C.c_size_t, C.c_void_p]
+_lib.osdp_linear_op_cost.restype = C.c_int
+_lib.osdp_linear_op_cost.argtypes = [C.POINTER(osdp_linear_desc), C.c_int, C.POINTER(osdp_op_cost)]
 _lib.osdp_trace_enable.restype = C.c_int
 _lib.osdp_trace_enable.argtypes = [C.c_int]
 _lib.osdp_set_tuning.restype = C.c_int
@@ -314,6 +331,115 @@ def osdp_ffn_split_mlp_op_cost(desc: osdp_mlp_desc, pass_: int) -> osdp_op_cost:
     if st != OSDP_OK:
         raise OsdpError(st, "osdp_ffn_split_mlp_op_cost")
     return out
+
+
+# ------------------------------------------------------------------------------------- Linear operator
+def make_linear_desc(tokens, in_features, out_features, dtype, k, axis=OSDP_SPLIT_TOKENS, has_bias=True) -> osdp_linear_desc:
+    code = dtype if isinstance(dtype, int) else _dtype_code(dtype)
+    return osdp_linear_desc(int(tokens), int(in_features), int(out_features), int(code), int(k), int(axis),
+                            1 if has_bias else 0)
+
+
+def osdp_split_linear_workspace_bytes(desc: osdp_linear_desc, pass_: int, check=True) -> int:
+    out = C.c_size_t()
+    st = _lib.osdp_split_linear_workspace_bytes(C.byref(desc), int(pass_), C.byref(out))
+    if st != OSDP_OK:
+        if check:
+            raise OsdpError(st, "osdp_split_linear_workspace_bytes")
+        return -st
+    return int(out.value)
+
+
+def _validate_linear(desc, spec, workspace, workspace_bytes):
+    T, i, o = desc.tokens, desc.in_features, desc.out_features
+    st = _TORCH_DTYPE.get(desc.dtype)
+    numel = {"X": T * i, "dX": T * i, "Y": T * o, "dY": T * o, "W": i * o, "dW": i * o, "b": o, "db": o}
+    dev = None
+    for name, t in spec:
+        if t is None or isinstance(t, int):
+            continue
+        want = torch.float32 if name in ("dW", "db") else st
+        if not t.is_cuda or not t.is_contiguous():
+            return None, OSDP_ERR_ARG, f"{name} must be a dense CUDA tensor"
+        if want is not None and t.dtype != want:
+            return None, OSDP_ERR_DTYPE, f"{name} has dtype {t.dtype}, descriptor needs {want}"
+        if t.numel() != numel[name]:
+            return None, OSDP_ERR_SHAPE, f"{name} has {t.numel()} elements, descriptor needs {numel[name]}"
+        if dev is not None and t.device != dev:
+            return None, OSDP_ERR_ARG, f"{name} is on {t.device}, other tensors on {dev}"
+        dev = t.device
+    if workspace is not None and not isinstance(workspace, int):
+        if not workspace.is_cuda or (dev is not None and workspace.device != dev):
+            return None, OSDP_ERR_WORKSPACE, "workspace must be a CUDA tensor on the tensors' device"
+        if workspace_bytes > workspace.numel() * workspace.element_size():
+            return None, OSDP_ERR_WORKSPACE, "workspace_bytes exceeds the workspace tensor"
+    return dev, OSDP_OK, ""
+
+
+def osdp_split_linear_forward(desc, X, W, b, Y, workspace=None, workspace_bytes=None, stream=None, check=True):
+    if workspace_bytes is None:
+        workspace_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    dev, vs, detail = _validate_linear(desc, (("X", X), ("W", W), ("b", b), ("Y", Y)), workspace, int(workspace_bytes))
+    if vs != OSDP_OK:
+        if check:
+            raise OsdpError(vs, "osdp_split_linear_forward", detail)
+        return vs
+    with _on_device(dev):
+        st = _lib.osdp_split_linear_forward(C.byref(desc), _ptr(X), _ptr(W), _ptr(b), _ptr(Y), _ptr(workspace),
+                                            int(workspace_bytes), _stream_ptr(stream))
+    if check and st != OSDP_OK:
+        raise OsdpError(st, "osdp_split_linear_forward")
+    return st
+
+
+def osdp_split_linear_backward(desc, X, W, dY, dX, dW, db, workspace=None, workspace_bytes=None, stream=None, check=True):
+    if workspace_bytes is None:
+        workspace_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    dev, vs, detail = _validate_linear(desc, (("X", X), ("W", W), ("dY", dY), ("dX", dX), ("dW", dW), ("db", db)),
+                                       workspace, int(workspace_bytes))
+    if vs != OSDP_OK:
+        if check:
+            raise OsdpError(vs, "osdp_split_linear_backward", detail)
+        return vs
+    with _on_device(dev):
+        st = _lib.osdp_split_linear_backward(C.byref(desc), _ptr(X), _ptr(W), _ptr(dY), _ptr(dX), _ptr(dW), _ptr(db),
+                                             _ptr(workspace), int(workspace_bytes), _stream_ptr(stream))
+    if check and st != OSDP_OK:
+        raise OsdpError(st, "osdp_split_linear_backward")
+    return st
+
+
+def osdp_linear_op_cost(desc: osdp_linear_desc, pass_: int) -> osdp_op_cost:
+    out = osdp_op_cost()
+    st = _lib.osdp_linear_op_cost(C.byref(desc), pass_, C.byref(out))
+    if st != OSDP_OK:
+        raise OsdpError(st, "osdp_linear_op_cost")
+    return out
+
+
+class SplitLinear:
+    """Descriptor + caller-owned workspace for repeated calls of the split Linear operator (marshalling only)."""
+
+    def __init__(self, tokens, in_features, out_features, dtype: torch.dtype, k: int, axis="contraction", has_bias=True,
+                 device="cuda"):
+        ax = {"tokens": OSDP_SPLIT_TOKENS, "contraction": OSDP_SPLIT_CONTRACTION}[axis]
+        self.desc = make_linear_desc(tokens, in_features, out_features, dtype, k, ax, has_bias)
+        self.dtype, self.device = dtype, torch.device(device)
+        n = max(osdp_split_linear_workspace_bytes(self.desc, OSDP_FWD), osdp_split_linear_workspace_bytes(self.desc, OSDP_BWD))
+        self.workspace = torch.empty(max(n, 256), dtype=torch.uint8, device=self.device)
+
+    def forward(self, X, W, b, Y=None, stream=None):
+        if Y is None:
+            Y = torch.empty((self.desc.tokens, self.desc.out_features), dtype=self.dtype, device=X.device)
+        osdp_split_linear_forward(self.desc, X, W, b, Y, self.workspace, stream=stream)
+        return Y
+
+    def backward(self, X, W, dY, out=None, stream=None):
+        if out is None:
+            out = dict(dX=torch.empty_like(X), dW=torch.empty(W.shape, dtype=torch.float32, device=X.device),
+                       db=torch.empty(W.shape[1], dtype=torch.float32, device=X.device) if self.desc.has_bias else None)
+        osdp_split_linear_backward(self.desc, X, W, dY, out["dX"], out["dW"], out["db"], self.workspace, stream=stream)
+        return out
 
 
 # ---------------------------------------------------------------------------------------------- planner

@@ -53,7 +53,7 @@ struct Tuning {
   std::atomic<int64_t> wave_sync{1};        // line the producers up at tile boundaries (MT = 2 launches)
   std::atomic<int64_t> band_mib{32};        // L2 budget for the A rows of one raster band
   std::atomic<int64_t> cluster_min_tiles{0};   // > 0: multicast clusters for launches of at least this many pair tiles
-  std::atomic<int64_t> fork_max_tiles{148};    // backward: A5 | A6 | A7 | column sums run concurrently when each GEMM has at most this many 256 x 256 tiles
+  std::atomic<int64_t> fork_max_tiles{256};    // backward: A5 | A6 | A7 | column sums run concurrently when each GEMM has at most this many 256 x 256 tiles
 };
 inline Tuning& tuning() {
   static Tuning t;

@@ -354,7 +354,10 @@ const char* osdp_step_name(int step_id) {
     case 6: return "A6 dW1 += X^T dZ";
     case 7: return "A7 dX = dZ W1^T";
     case 8: return "A8 db2 and db1 column sums";
-    case 10: return "fp32 accumulator -> output (ffn-axis split)";
+    case 10: return "fp32 accumulator -> output (ffn / contraction-axis split)";
+    case 11: return "Linear fwd Y = X W + b";
+    case 12: return "Linear bwd dX = dY W^T";
+    case 13: return "Linear bwd dW += X^T dY";
     default: return "unknown";
   }
 }
@@ -633,3 +636,5 @@ int osdp_ffn_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const 
 }
 
 }  // extern "C"
+
+#include "linear_api.inl"

@@ -117,6 +117,32 @@ def mlp_inputs(tokens: int, hidden: int, ffn: int, dtype: torch.dtype, seed: int
     )
 
 
+@dataclasses.dataclass
+class LinearInputs:
+    """One Linear operator's tensors (attention projection), stored values (CPU).  W is [in x out]."""
+    X: torch.Tensor    # [T, in]
+    W: torch.Tensor    # [in, out]
+    b: torch.Tensor    # [out]
+    dY: torch.Tensor   # [T, out]
+
+    def as_f64(self) -> dict:
+        return {k: getattr(self, k).to(torch.float64).numpy() for k in ("X", "W", "b", "dY")}
+
+    def to(self, device) -> "LinearInputs":
+        return LinearInputs(*[getattr(self, k).to(device) for k in ("X", "W", "b", "dY")])
+
+
+def linear_inputs(tokens: int, in_features: int, out_features: int, dtype: torch.dtype, seed: int = 0,
+                  w_std: float = 0.02) -> LinearInputs:
+    """Same recipe and stream ids as the MLP's first Linear: X, dY ~ N(0, 1); W, b ~ N(0, std 0.02)."""
+    return LinearInputs(
+        X=normal_tensor(seed, STREAM_X, (tokens, in_features), 1.0, dtype),
+        W=normal_tensor(seed, STREAM_W1, (in_features, out_features), w_std, dtype),
+        b=normal_tensor(seed, STREAM_B1, (out_features,), w_std, dtype),
+        dY=normal_tensor(seed, STREAM_DY, (tokens, out_features), 1.0, dtype),
+    )
+
+
 # BASELINE.json configs, by short name.  k lists are the split counts each config is run at.
 CONFIGS = {
     "C1": dict(tokens=512, hidden=256, ffn=1024, dtype="f32", ks=(4,), seed=0),

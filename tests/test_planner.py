@@ -451,6 +451,56 @@ def test_mlp_factors_zdp_shards_only_the_model_states(lib):
             assert p2 - pd == c.act_bytes                                 # memory grows with the batch
 
 
+def test_linear_factors_and_a_table1_shaped_two_operators_per_layer_model(lib):
+    """Table 1: Operator Num = 2 x Layer Num + 2 - every layer is an attention operator plus an MLP
+    operator.  Cost records from osdp_linear_op_cost (QKV + output projection of a layer's attention block, folded into
+    one operator) and osdp_mlp_op_cost feed osdp_plan; the plan equals the oracle's brute force on a W&S-sized model
+    (2 layers -> 6 operators)."""
+    T, h, e = 2048, 1024, 2
+    qkv = lib.make_linear_desc(T, h, 3 * h, 1, 1, lib.OSDP_SPLIT_CONTRACTION, True)
+    proj = lib.make_linear_desc(T, h, h, 1, 1, lib.OSDP_SPLIT_CONTRACTION, True)
+    for d, n_in, n_out in ((qkv, h, 3 * h), (proj, h, h)):
+        for pass_, grads, acts in ((lib.OSDP_FWD, 0, T * (n_in + n_out)), (lib.OSDP_BWD, 4, T * (2 * n_in + n_out))):
+            c = lib.osdp_linear_op_cost(d, pass_)
+            params = n_in * n_out + n_out
+            assert c.S == params * e and c.model_bytes == params * (e + grads) and c.act_bytes == acts * e
+            assert c.extra_fixed == lib.osdp_split_linear_workspace_bytes(d, pass_) and c.extra_transient == 0
+    d4 = lib.make_linear_desc(T, h, 3 * h, 1, 4, lib.OSDP_SPLIT_CONTRACTION, True)
+    assert lib.osdp_split_linear_workspace_bytes(d4, lib.OSDP_FWD) == T * 3 * h * 4        # the fp32 accumulator of Y
+    assert lib.osdp_split_linear_workspace_bytes(d4, lib.OSDP_BWD) == 32 * 3 * h * 4       # column-sum scratch
+    assert lib.osdp_split_linear_workspace_bytes(lib.make_linear_desc(T, h, h, 1, 1, 0, False), lib.OSDP_BWD) == 0
+
+    def attn_op():
+        a, b = lib.osdp_linear_op_cost(qkv, lib.OSDP_BWD), lib.osdp_linear_op_cost(proj, lib.OSDP_BWD)
+        # under ZDP the gathered parameters are the sliceable surge (PAPER.md:163-167): S bytes, / k with splitting
+        return P.OpCost(S=a.S + b.S, model=a.model_bytes + b.model_bytes, act=a.act_bytes + b.act_bytes,
+                        extra_fixed=a.extra_fixed + b.extra_fixed, extra_transient=int(a.S + b.S), gamma=2e-4, delta=1e-5)
+
+    def mlp_op():
+        c = lib.osdp_mlp_op_cost(lib.make_desc(T, h, 4 * h, 1, 1), lib.OSDP_BWD)
+        return P.OpCost(S=c.S, model=c.model_bytes, act=c.act_bytes, extra_fixed=c.extra_fixed,
+                        extra_transient=c.extra_transient + int(c.S), gamma=4e-4, delta=2e-5)
+
+    layers = 2
+    emb = P.OpCost(S=50304 * h * e, model=50304 * h * (e + 4), gamma=1e-5)
+    head = P.OpCost(S=h * 50304 * e, model=h * 50304 * (e + 4), act=T * 50304 * e, gamma=3e-4)
+    ops = [emb] + [o for _ in range(layers) for o in (attn_op(), mlp_op())] + [head]
+    assert len(ops) == 2 * layers + 2
+    full = sum(o.model + o.act + o.extra_fixed for o in ops) + max(o.extra_transient for o in ops)
+    for frac in (1.0, 0.8, 0.6, 0.45):
+        d = P.Device(N=8, alpha=5e-6, beta=1 / 400e9, mem_limit=int(full * frac))
+        ref = P.plan_brute_force(ops, d, 1, [1, 4])
+        st, ks, modes, sec, peak = lib.osdp_plan([_to_lib(lib, o) for o in ops], _dev(lib, d), 1, [1, 4])
+        if ref is None:
+            assert st == lib.OSDP_ERR_INFEASIBLE
+            continue
+        assert st == lib.OSDP_OK and (modes, ks, peak) == (ref[0], ref[1], ref[3]) and round(sec * 1e12) == ref[2]
+        if frac == 1.0:
+            assert modes == [0] * len(ops) and ks == [1] * len(ops)
+        if frac <= 0.6:
+            assert 1 in modes                                       # a tighter limit forces ZDP on some operators
+
+
 def test_descriptor_validation(lib):
     assert lib.osdp_split_mlp_workspace_bytes(lib.make_desc(0, 8, 8, 1, 1), 0) == 0
     assert lib.osdp_split_mlp_workspace_bytes(lib.make_desc(8, 12, 8, 1, 1), 0) == 0       # h % 8
