@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — split-MLP forward+backward throughput on B200 (BASELINE.json metric), one JSON line on stdout.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C4] [--k 4] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C4] [--k 4] [--graph] [--impl ours|reference]
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
         bench.py --gpus N --steps K --warmup W
 
@@ -343,7 +343,8 @@ class Workload:
 
 def timed_steps(fn, steps, world, flush=None):
     """EXACTLY `steps` steps between barrier+synchronize brackets; per-step CUDA events on the current stream.
-    Returns (sum of step ms, wall ms of the bracket)."""
+    Returns (sum of step ms, wall ms of the bracket); the per-step times of the last call are kept in
+    timed_steps.last (median and min are reported beside the mean)."""
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     barrier(world)
     t0 = time.perf_counter()
@@ -355,7 +356,30 @@ def timed_steps(fn, steps, world, flush=None):
         b.record()
     barrier(world)
     wall = (time.perf_counter() - t0) * 1e3
-    return sum(a.elapsed_time(b) for a, b in evs), wall
+    timed_steps.last = [a.elapsed_time(b) for a, b in evs]
+    return sum(timed_steps.last), wall
+
+
+timed_steps.last = []
+
+
+def graph_step_ms(wl, steps, world, flush):
+    """The same step captured once in a CUDA graph and replayed: what is left of the host-side launch cost (tensor-map
+    encoding, argument checks, ~10 launches per slice) disappears; the kernels are the same.  Returns ms/step."""
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        for _ in range(2):
+            wl.step()
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        wl.step()
+    for _ in range(3):
+        g.replay()
+    ms, _ = timed_steps(g.replay, steps, world, flush)
+    return ms / steps, statistics.median(timed_steps.last), min(timed_steps.last)
 
 
 def measure_peak_bytes(lib, cfg, k, axis="tokens"):
@@ -498,17 +522,43 @@ def stack_bench(args, lib, cfg):
     if st != lib.OSDP_OK:
         raise SystemExit(f"osdp_plan: status {st}")
 
+    # ---- memory as the library really uses it (not the paper's accounting above): model states + the T x h tensors
+    # the chain keeps per layer (saved input X_l and dX_l; dY_l is dX_{l+1}) summed over layers, ONE transient workspace
+    # shared by all layers (slices and layers run one after another: "released serially"), predicted with
+    # osdp_mlp_op_cost + osdp_cost_eval for the plan that is run, and measured below as the allocator's peak and as the
+    # device's own used-memory delta (cudaMemGetInfo).
+    torch.cuda.synchronize()
+    torch.cuda.empty_cache()
+    free0, _ = torch.cuda.mem_get_info()
+    alloc0 = torch.cuda.memory_allocated()
+    torch.cuda.reset_peak_memory_stats()
+    real_persist, real_transient = 0, 0
+    for l in range(L):
+        oc = lib.osdp_mlp_op_cost(desc1, lib.OSDP_BWD)
+        oc.act_bytes = 2 * T * h * 2                       # X_l and dX_l
+        p_, t_, _ = lib.osdp_cost_eval(oc, lib.OSDP_DP, ks[l], 1, lib.osdp_device(1, 0.0, 0.0, 1 << 62))
+        real_persist += p_ - oc.extra_fixed                # the column-sum scratch lives inside the shared workspace
+        real_transient = max(real_transient, t_ + oc.extra_fixed)
+    est_real = real_persist + real_transient + 2 * T * h * 2        # + X_L (the stack's output) and dY_L
+
     t0 = time.time()
     layers = []
+    ws_bytes = 0
     for l in range(L):
         w = I.mlp_inputs(1, h, f, dt, seed=l)             # weights and biases of layer l (seed = layer, reading S13)
-        layers.append(dict(W1=w.W1.cuda(), b1=w.b1.cuda(), W2=w.W2.cuda(), b2=w.b2.cuda(),
-                           op=lib.SplitMlp(T, h, f, dt, ks[l]),
+        op = lib.SplitMlp(T, h, f, dt, ks[l])
+        ws_bytes = max(ws_bytes, op.workspace.numel())
+        op.workspace = None
+        layers.append(dict(W1=w.W1.cuda(), b1=w.b1.cuda(), W2=w.W2.cuda(), b2=w.b2.cuda(), op=op,
                            g=dict(dX=torch.empty((T, h), dtype=dt, device="cuda"),
                                   dW1=torch.empty((h, f), dtype=torch.float32, device="cuda"),
                                   db1=torch.empty((f,), dtype=torch.float32, device="cuda"),
                                   dW2=torch.empty((f, h), dtype=torch.float32, device="cuda"),
                                   db2=torch.empty((h,), dtype=torch.float32, device="cuda"))))
+    torch.cuda.empty_cache()
+    shared_ws = torch.empty(ws_bytes, dtype=torch.uint8, device="cuda")      # one transient workspace for the whole stack
+    for ly in layers:
+        ly["op"].workspace = shared_ws
     Xs = [I.normal_tensor(0, I.STREAM_X, (T, h), 1.0, dt).cuda()] + [torch.empty((T, h), dtype=dt, device="cuda") for _ in range(L)]
     dYL = I.normal_tensor(0, I.STREAM_DY, (T, h), 1.0, dt).cuda()
     log(f"[bench] stack inputs generated in {time.time() - t0:.1f}s; plan k = {ks}")
@@ -537,6 +587,15 @@ def stack_bench(args, lib, cfg):
     ms = ms_sum / steps
     flops = executed_flops(T, h, f) * L
     peaks = load_peaks()
+    torch.cuda.synchronize()
+    measured_alloc = torch.cuda.max_memory_allocated() - alloc0
+    free1, _ = torch.cuda.mem_get_info()
+    memory = {"est_peak_bytes_library_factors": int(est_real), "measured_peak_bytes_allocator": int(measured_alloc),
+              "measured_device_used_delta_bytes": int(free0 - free1), "measured_over_est": measured_alloc / est_real,
+              "workspace_bytes_shared": int(ws_bytes),
+              "note": "library factors: osdp_mlp_op_cost + osdp_cost_eval per layer (model states, X_l, dX_l) + one shared "
+                      "transient workspace; the 24 GiB cap does not bind under them (the fused, recomputing path keeps no "
+                      "T x f tensor per layer) - est_peak_bytes_paper_accounting is the paper-style sum the cap is meant for"}
     print(json.dumps({
         "metric": METRIC, "value": flops / (ms * 1e-3) / 1e12, "unit": UNIT, "n_gpus": 1, "steps": steps,
         "warmup": max(3, args.warmup), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -549,7 +608,7 @@ def stack_bench(args, lib, cfg):
         "planner": {"calibration_ms_per_layer": {str(e["k"]): e["ms_per_step"] for e in table}, "fit": fit,
                     "est_ms_per_step": est_s * 1e3, "measured_ms_per_step": ms, "est_over_measured": est_s * 1e3 / ms,
                     "est_peak_bytes_paper_accounting": est_peak, "cap_bytes": cap},
-        "clocks": clocks, "gpu_launches": launches[0] * steps}), flush=True)
+        "memory": memory, "clocks": clocks, "gpu_launches": launches[0] * steps}), flush=True)
     return 0
 
 
@@ -565,6 +624,8 @@ def main():
                     help="split axis of the headline workload: token slices (north_star, default) or the paper-literal "
                          "ffn-axis split (osdp_ffn_split_mlp_*)")
     ap.add_argument("--no-sweep", action="store_true", help="skip the per-k TFLOP/s and peak-bytes table")
+    ap.add_argument("--graph", action="store_true",
+                    help="also time the step captured in a CUDA graph and replayed (launch-bound configs: C1, C2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--granularity-sweep", default=None, metavar="H1,H2,...",
@@ -613,7 +674,15 @@ def main():
     ms_sum, wall_ms = timed_steps(wl.step, args.steps, world, flush)
     clocks = sampler.stop()
     ms_step = max_over_ranks(ms_sum / args.steps, world)
+    ms_median = max_over_ranks(statistics.median(timed_steps.last), world)
+    ms_min = max_over_ranks(min(timed_steps.last), world)
     value = world * flops / (ms_step * 1e-3) / 1e12
+    graph = None
+    if args.graph:
+        g_ms, g_med, g_min = graph_step_ms(wl, args.steps, world, flush)
+        g_ms = max_over_ranks(g_ms, world)
+        graph = {"ms_per_step": g_ms, "ms_median": g_med, "ms_min": g_min, "value": world * flops / (g_ms * 1e-3) / 1e12,
+                 "unit": UNIT, "how": "one step (forward + backward through the C ABI) captured in a CUDA graph, replayed"}
 
     # ---- per-launch trace of the same steps (CUDA events on the call's stream, inside the library)
     lib.osdp_trace_enable(True)
@@ -640,20 +709,34 @@ def main():
     dom_avg = sum(per[dom]) / len(per[dom])
     achieved = gemm_flops / (dom_avg * 1e-3) / 1e12
     peak = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]) if cfg["dtype"] == "bf16" else None
-    traffic = None
+    # DRAM bytes of the dominant kernel per launch, from the committed ncu --set full capture (profiles/traffic.json; its
+    # .md names the command).  The dW GEMMs launch with beta = 0 on slice 0 (store only) and beta = 1 afterwards (fp32
+    # read-modify-write): both are listed and `traffic` is the per-launch mean over the k launches of a step.
+    traffic = traffic_detail = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get(f"{args.config}:k{args.k}:A{dom}") if args.axis == "tokens" else None
+    if os.path.exists(tpath) and args.axis == "tokens":
+        tj = json.load(open(tpath))
+        key = f"{args.config}:k{args.k}:A{dom}"
+        b0, b1 = tj.get(key + ":beta0"), tj.get(key + ":beta1")
+        if b0 is not None and b1 is not None:
+            traffic = (b0 + (args.k - 1) * b1) / args.k
+            traffic_detail = {"beta0_launch": b0, "beta1_launch": b1, "launches_per_step": {"beta0": 1, "beta1": args.k - 1},
+                              "source": tj.get("source")}
+        elif tj.get(key) is not None:
+            traffic = tj.get(key)
+            traffic_detail = {"source": tj.get("source")}
     roofline = {"bound": "tensor", "kernel": f"gemm_bf16_sm100_kernel [{lib.osdp_step_name(dom)}]",
                 "achieved": achieved, "peak": peak, "unit": UNIT, "frac": (achieved / peak) if peak else None,
-                "traffic": traffic, "peak_source": f"{peaks['source']} (bf16_tflops_sustained: kernel timed inside a long step)",
+                "traffic": traffic, "traffic_detail": traffic_detail, "peak_source": f"{peaks['source']} (bf16_tflops_sustained: kernel timed inside a long step)",
                 "frac_of_burst": achieved / peaks["bf16_tflops"], "frac_of_nominal": achieved / NOMINAL_BF16_TFLOPS,
                 "flops_per_launch": gemm_flops, "avg_launch_ms": dom_avg,
                 "how": "per-launch CUDA events recorded by the library on the call's stream over K traced steps"}
     if cfg["dtype"] != "bf16":
-        roofline.update({"bound": "alu", "peak": 148 * 128 * 2 * 1.965e-3,
-                         "frac": achieved / (148 * 128 * 2 * 1.965e-3),
-                         "peak_source": "148 SMs x 128 FFMA/clk x 2 flop x 1.965 GHz (fp32 FFMA path)"})
+        ghz = (clocks.get("sm_mhz") or 1965.0) * 1e-3          # the clock sampled during the timed region
+        alu_peak = 148 * 128 * 2 * ghz * 1e-3
+        roofline.update({"bound": "alu", "kernel": f"gemm_f32_kernel [{lib.osdp_step_name(dom)}]", "peak": alu_peak,
+                         "frac": achieved / alu_peak,
+                         "peak_source": f"148 SMs x 128 FFMA/clk x 2 flop x {ghz:.3f} GHz (SM clock sampled in this run; fp32 FFMA path)"})
 
     # ---- end to end: host buffers, copies inside the timed region
     e2e = None
@@ -694,12 +777,13 @@ def main():
         cost_fit = {axis: fit_gamma_delta(tab) for axis, tab in tables.items()}
     cpu = None
     if not args.no_cpu_baseline and rank == 0 and world == 1:
-        r = time_oracle(cfg, 1, 0)
+        r = time_oracle(cfg, 1, 1)          # one untimed warm-up call, one timed
         cpu = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+                "warmup": args.warmup, "ms_per_step": ms_step, "ms_per_step_median": ms_median, "ms_per_step_min": ms_min,
+                "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": cfg["dtype"], "data": "synthetic",
                 "config": {"workload": workload_name(args, cfg), "tokens_per_gpu": T, "hidden": h, "ffn": f,
                            "k": args.k, "split_axis": args.axis, "flops_per_step": flops, "flops_counted": "14*T*h*f executed (12*T*h*f model)",
@@ -707,7 +791,7 @@ def main():
                 "value_model_flops_12x": value * 12.0 / 14.0,
                 "frac_of_sustained_peak": value / world / peak if peak else None,
                 "frac_of_nominal_peak": value / world / NOMINAL_BF16_TFLOPS,
-                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches) * args.steps,
+                "clocks": clocks, "e2e": e2e, "graph": graph, "gpu_launches": int(launches) * args.steps,
                 "roofline": roofline, "kernels": kernels, "per_k": per_k, "per_k_ffn_split": per_k_ffn, "cost_model_fit": cost_fit,
                 "cpu_baseline": cpu,
                 "wall_ms_timed_region": wall_ms}

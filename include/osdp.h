@@ -297,6 +297,78 @@ int osdp_plan_batch(const osdp_op_cost* ops, int32_t n, const osdp_device* dev, 
                     int32_t* k_out, int32_t* mode_out, int64_t* batch_out,
                     double* est_seconds, uint64_t* est_peak_bytes);
 
+/* ---- ZDP mode across GPUs with weight-slice gathering -----------------------------------
+ * in ZDP mode the model states of an operator are sharded over the N data-parallel ranks, the parameters
+ * are all-gathered before the forward and again before the backward, and the gradients are reduce-scattered (three
+ * collectives).  PAPER.md:163-167: gathering a huge operator whole is the memory surge operator splitting
+ * removes - "Combined with ZDP, operator splitting amortizes the memory from size(MatMul) to
+ * size(MatMul) / slice_granularity".  These calls run the ffn-axis split MLP (osdp_ffn_split_mlp_*) in that mode: slice
+ * s + 1 of the weights is gathered on `comm_stream` while slice s computes on `compute_stream` ("our
+ * distributed training deployment supports the overlapping between computation and communication"), and the slice's
+ * weight gradients are reduce-scattered while the next slice computes.  Each rank runs the call on its own token batch.
+ *
+ * Slices and shards.  unit = 16 bytes of elements.  Slice s = ffn columns [lo_s, lo_{s+1}), lo_s = floor(s G / k) N unit
+ * with G = ffn / (N unit): whole groups of N units, so every rank's piece is whole 16-byte units.  Requires
+ * hidden % (N unit) == 0, ffn % (N unit) == 0, 1 <= k <= G.  A rank's PARAMETER SHARD is one dense buffer of
+ * osdp_zdp_shard_elems() elements of the storage dtype: for s = 0..k-1 the pieces
+ *     W1[r h/N : (r+1) h/N, lo:hi]   ((h/N) x fs, row-major)      - gathered: rows concatenate to [h x fs]
+ *     b1[lo + r fs/N : lo + (r+1) fs/N]
+ *     W2[lo + r fs/N : lo + (r+1) fs/N, :]   ((fs/N) x h)          - gathered: rows concatenate to [fs x h]
+ * then b2[r h/N : (r+1) h/N].  osdp_zdp_slice_layout gives the element offsets (s = k: the b2 piece, in b1_off/b1_elems).
+ * The GRADIENT SHARD is an fp32 buffer with the same element offsets; it receives the SUM over ranks (data parallelism)
+ * of this rank's pieces of dW1, db1, dW2, db2 and is OVERWRITTEN.
+ *
+ * Collectives come from the caller (osdp_comm): all_gather(send, recv, bytes_per_rank) writes the ranks' send buffers
+ * in rank order into recv; reduce_scatter_f32(send, recv, floats_per_rank) sums send (N chunks) over ranks and writes
+ * chunk `rank` to recv; both enqueue on the given stream and return 0 on success.  The binding provides them over
+ * torch.distributed (NCCL over NVLink / NVSwitch).  comm may be NULL when world == 1 (the collectives are device copies).
+ * compute_stream / comm_stream: two cudaStream_t of the current device; the call forks comm_stream from compute_stream
+ * at entry and joins it back before returning (in stream order: no host synchronisation); they may be the same stream
+ * (no overlap).  Workspace (osdp_zdp_ffn_split_mlp_workspace_bytes): TWO gathered slice buffers (the paper's
+ * size / slice_granularity, double-buffered) + in the backward two fp32 gradient staging slices + the ffn-split
+ * workspace of one slice.  osdp_zdp_schedule returns the steps of one call in enqueue order (pure host function; the
+ * calls walk exactly this list): gathers, slice computations, reduce-scatters, each with the slice, the buffer it uses
+ * and the bytes one rank contributes (slice = k: the b2 / db2 vector).  osdp_zdp_ffn_split_mlp_op_cost: cost-model
+ * factors of the ZDP execution: model_bytes = the WHOLE operator's model states (osdp_cost_eval divides them by N in
+ * ZDP mode), extra_transient = two gathered slices at k = 1 (sliceable: / k), extra_fixed / act_bytes as the ffn split.
+ * Status on one B200: the N = 1 path is parity-tested on the GPU; N > 1 is covered by a world_size-2 CPU run of the
+ * same schedule and layout (tests/test_zdp.py); no multi-GPU timing exists. */
+typedef struct osdp_zdp_desc {
+  osdp_mlp_desc mlp;   /* tokens = THIS rank's token batch; k = number of ffn slices */
+  int32_t world;       /* N >= 1 */
+  int32_t rank;        /* 0 <= rank < N */
+} osdp_zdp_desc;
+typedef struct osdp_zdp_slice {
+  int64_t lo, hi;               /* ffn columns of the slice */
+  int64_t w1_off, w1_elems;     /* element offset / count of the pieces inside a rank's shard */
+  int64_t b1_off, b1_elems;
+  int64_t w2_off, w2_elems;
+} osdp_zdp_slice;
+typedef struct osdp_comm {
+  void* ctx;
+  int (*all_gather)(void* ctx, const void* send, void* recv, size_t bytes_per_rank, void* stream);
+  int (*reduce_scatter_f32)(void* ctx, const void* send, void* recv, size_t floats_per_rank, void* stream);
+} osdp_comm;
+typedef enum osdp_zdp_op { OSDP_ZDP_GATHER = 0, OSDP_ZDP_COMPUTE = 1, OSDP_ZDP_REDUCE_SCATTER = 2 } osdp_zdp_op;
+typedef struct osdp_zdp_step {
+  int32_t op;                /* osdp_zdp_op */
+  int32_t slice;             /* 0..k-1; k = the b2 (forward gather) / db2 (backward reduce-scatter) vector */
+  int32_t buffer;            /* which of the two gathered (GATHER, COMPUTE) / gradient staging (REDUCE_SCATTER) buffers */
+  int32_t on_comm_stream;    /* 1: enqueued on comm_stream, 0: on compute_stream */
+  uint64_t bytes_per_rank;   /* collectives: bytes one rank contributes = bytes it receives from each peer; COMPUTE: 0 */
+} osdp_zdp_step;
+int osdp_zdp_shard_elems(const osdp_zdp_desc* desc, int64_t* elems);
+int osdp_zdp_slice_layout(const osdp_zdp_desc* desc, int32_t s, osdp_zdp_slice* out);
+int64_t osdp_zdp_schedule(const osdp_zdp_desc* desc, int pass, int64_t max_steps, osdp_zdp_step* steps);   /* count, or -status */
+int osdp_zdp_ffn_split_mlp_workspace_bytes(const osdp_zdp_desc* desc, int pass, size_t* bytes);
+int osdp_zdp_ffn_split_mlp_forward(const osdp_zdp_desc* desc, const void* param_shard, const void* X, void* Y,
+                                   void* workspace, size_t workspace_bytes, const osdp_comm* comm,
+                                   void* compute_stream, void* comm_stream);
+int osdp_zdp_ffn_split_mlp_backward(const osdp_zdp_desc* desc, const void* param_shard, const void* X, const void* dY,
+                                    void* dX, float* grad_shard, void* workspace, size_t workspace_bytes,
+                                    const osdp_comm* comm, void* compute_stream, void* comm_stream);
+int osdp_zdp_ffn_split_mlp_op_cost(const osdp_zdp_desc* desc, int pass, osdp_op_cost* out);
+
 #if defined(__GNUC__)
 #pragma GCC visibility pop
 #endif

@@ -35,6 +35,8 @@ EXPORTS = (
     "osdp_set_tuning", "osdp_get_tuning", "osdp_ffn_split_mlp_workspace_bytes", "osdp_ffn_split_mlp_forward",
     "osdp_ffn_split_mlp_backward", "osdp_ffn_split_mlp_op_cost", "osdp_cost_eval_mixed", "osdp_plan_mixed",
     "osdp_split_linear_workspace_bytes", "osdp_split_linear_forward", "osdp_split_linear_backward", "osdp_linear_op_cost",
+    "osdp_zdp_shard_elems", "osdp_zdp_slice_layout", "osdp_zdp_schedule", "osdp_zdp_ffn_split_mlp_workspace_bytes",
+    "osdp_zdp_ffn_split_mlp_forward", "osdp_zdp_ffn_split_mlp_backward", "osdp_zdp_ffn_split_mlp_op_cost",
 )
 
 
@@ -49,6 +51,31 @@ class osdp_linear_desc(C.Structure):
 
 
 OSDP_SPLIT_TOKENS, OSDP_SPLIT_CONTRACTION = 0, 1
+
+
+class osdp_zdp_desc(C.Structure):
+    _fields_ = [("mlp", osdp_mlp_desc), ("world", C.c_int32), ("rank", C.c_int32)]
+
+
+class osdp_zdp_slice(C.Structure):
+    _fields_ = [("lo", C.c_int64), ("hi", C.c_int64), ("w1_off", C.c_int64), ("w1_elems", C.c_int64),
+                ("b1_off", C.c_int64), ("b1_elems", C.c_int64), ("w2_off", C.c_int64), ("w2_elems", C.c_int64)]
+
+
+class osdp_zdp_step(C.Structure):
+    _fields_ = [("op", C.c_int32), ("slice", C.c_int32), ("buffer", C.c_int32), ("on_comm_stream", C.c_int32),
+                ("bytes_per_rank", C.c_uint64)]
+
+
+ALL_GATHER_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p)
+REDUCE_SCATTER_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p)
+
+
+class osdp_comm(C.Structure):
+    _fields_ = [("ctx", C.c_void_p), ("all_gather", ALL_GATHER_FN), ("reduce_scatter_f32", REDUCE_SCATTER_FN)]
+
+
+OSDP_ZDP_GATHER, OSDP_ZDP_COMPUTE, OSDP_ZDP_REDUCE_SCATTER = 0, 1, 2
 
 
 class osdp_op_cost(C.Structure):
@@ -108,6 +135,22 @@ _lib.osdp_split_linear_backward.restype = C.c_int
 _lib.osdp_split_linear_backward.argtypes = [C.POINTER(osdp_linear_desc)] + [C.c_void_p] * 7 + [C.c_size_t, C.c_void_p]
 _lib.osdp_linear_op_cost.restype = C.c_int
 _lib.osdp_linear_op_cost.argtypes = [C.POINTER(osdp_linear_desc), C.c_int, C.POINTER(osdp_op_cost)]
+_lib.osdp_zdp_shard_elems.restype = C.c_int
+_lib.osdp_zdp_shard_elems.argtypes = [C.POINTER(osdp_zdp_desc), C.POINTER(C.c_int64)]
+_lib.osdp_zdp_slice_layout.restype = C.c_int
+_lib.osdp_zdp_slice_layout.argtypes = [C.POINTER(osdp_zdp_desc), C.c_int32, C.POINTER(osdp_zdp_slice)]
+_lib.osdp_zdp_schedule.restype = C.c_int64
+_lib.osdp_zdp_schedule.argtypes = [C.POINTER(osdp_zdp_desc), C.c_int, C.c_int64, C.POINTER(osdp_zdp_step)]
+_lib.osdp_zdp_ffn_split_mlp_workspace_bytes.restype = C.c_int
+_lib.osdp_zdp_ffn_split_mlp_workspace_bytes.argtypes = [C.POINTER(osdp_zdp_desc), C.c_int, C.POINTER(C.c_size_t)]
+_lib.osdp_zdp_ffn_split_mlp_forward.restype = C.c_int
+_lib.osdp_zdp_ffn_split_mlp_forward.argtypes = [C.POINTER(osdp_zdp_desc)] + [C.c_void_p] * 4 + [C.c_size_t, C.POINTER(osdp_comm),
+                                                                                         C.c_void_p, C.c_void_p]
+_lib.osdp_zdp_ffn_split_mlp_backward.restype = C.c_int
+_lib.osdp_zdp_ffn_split_mlp_backward.argtypes = [C.POINTER(osdp_zdp_desc)] + [C.c_void_p] * 6 + [C.c_size_t, C.POINTER(osdp_comm),
+                                                                                          C.c_void_p, C.c_void_p]
+_lib.osdp_zdp_ffn_split_mlp_op_cost.restype = C.c_int
+_lib.osdp_zdp_ffn_split_mlp_op_cost.argtypes = [C.POINTER(osdp_zdp_desc), C.c_int, C.POINTER(osdp_op_cost)]
 _lib.osdp_trace_enable.restype = C.c_int
 _lib.osdp_trace_enable.argtypes = [C.c_int]
 _lib.osdp_set_tuning.restype = C.c_int
@@ -440,6 +483,160 @@ class SplitLinear:
                        db=torch.empty(W.shape[1], dtype=torch.float32, device=X.device) if self.desc.has_bias else None)
         osdp_split_linear_backward(self.desc, X, W, dY, out["dX"], out["dW"], out["db"], self.workspace, stream=stream)
         return out
+
+
+# ------------------------------------------------------------------ ZDP mode with weight-slice gathering
+def make_zdp_desc(tokens, hidden, ffn, dtype, k, world, rank) -> osdp_zdp_desc:
+    return osdp_zdp_desc(make_desc(tokens, hidden, ffn, dtype, k), int(world), int(rank))
+
+
+def osdp_zdp_shard_elems(desc: osdp_zdp_desc) -> int:
+    out = C.c_int64()
+    st = _lib.osdp_zdp_shard_elems(C.byref(desc), C.byref(out))
+    if st != OSDP_OK:
+        raise OsdpError(st, "osdp_zdp_shard_elems")
+    return int(out.value)
+
+
+def osdp_zdp_slice_layout(desc: osdp_zdp_desc, s: int) -> osdp_zdp_slice:
+    out = osdp_zdp_slice()
+    st = _lib.osdp_zdp_slice_layout(C.byref(desc), int(s), C.byref(out))
+    if st != OSDP_OK:
+        raise OsdpError(st, "osdp_zdp_slice_layout")
+    return out
+
+
+def osdp_zdp_schedule(desc: osdp_zdp_desc, pass_: int):
+    """[(op, slice, buffer, on_comm_stream, bytes_per_rank)] in enqueue order."""
+    n = int(_lib.osdp_zdp_schedule(C.byref(desc), int(pass_), 0, None))
+    if n < 0:
+        raise OsdpError(-n, "osdp_zdp_schedule")
+    arr = (osdp_zdp_step * n)()
+    _lib.osdp_zdp_schedule(C.byref(desc), int(pass_), n, arr)
+    return [(a.op, a.slice, a.buffer, a.on_comm_stream, int(a.bytes_per_rank)) for a in arr]
+
+
+def osdp_zdp_ffn_split_mlp_workspace_bytes(desc: osdp_zdp_desc, pass_: int) -> int:
+    out = C.c_size_t()
+    st = _lib.osdp_zdp_ffn_split_mlp_workspace_bytes(C.byref(desc), int(pass_), C.byref(out))
+    if st != OSDP_OK:
+        raise OsdpError(st, "osdp_zdp_ffn_split_mlp_workspace_bytes")
+    return int(out.value)
+
+
+def osdp_zdp_ffn_split_mlp_op_cost(desc: osdp_zdp_desc, pass_: int) -> osdp_op_cost:
+    out = osdp_op_cost()
+    st = _lib.osdp_zdp_ffn_split_mlp_op_cost(C.byref(desc), int(pass_), C.byref(out))
+    if st != OSDP_OK:
+        raise OsdpError(st, "osdp_zdp_ffn_split_mlp_op_cost")
+    return out
+
+
+def zdp_shard(desc: osdp_zdp_desc, W1, b1, W2, b2, rank=None):
+    """Rank `rank`'s dense shard (1-D tensor, dtype of W1) of the whole tensors, in the layout osdp_zdp_slice_layout
+    describes.  Pure data movement; also maps whole fp32 gradients to a gradient shard."""
+    d = osdp_zdp_desc(desc.mlp, desc.world, desc.rank if rank is None else int(rank))
+    N, r, h, k = d.world, d.rank, d.mlp.hidden, d.mlp.k
+    out = torch.empty(osdp_zdp_shard_elems(d), dtype=W1.dtype, device=W1.device)
+    for s in range(k):
+        sl = osdp_zdp_slice_layout(d, s)
+        fs = sl.hi - sl.lo
+        out[sl.w1_off:sl.w1_off + sl.w1_elems] = W1[r * h // N:(r + 1) * h // N, sl.lo:sl.hi].reshape(-1)
+        out[sl.b1_off:sl.b1_off + sl.b1_elems] = b1[sl.lo + r * fs // N:sl.lo + (r + 1) * fs // N]
+        out[sl.w2_off:sl.w2_off + sl.w2_elems] = W2[sl.lo + r * fs // N:sl.lo + (r + 1) * fs // N, :].reshape(-1)
+    sl = osdp_zdp_slice_layout(d, k)
+    out[sl.b1_off:sl.b1_off + sl.b1_elems] = b2[r * h // N:(r + 1) * h // N]
+    return out
+
+
+def zdp_unshard(desc: osdp_zdp_desc, shards):
+    """Inverse of zdp_shard over the list of every rank's shard: (W1, b1, W2, b2)-shaped whole tensors."""
+    N, h, f, k = desc.world, desc.mlp.hidden, desc.mlp.ffn, desc.mlp.k
+    t = shards[0]
+    W1, b1 = torch.empty((h, f), dtype=t.dtype, device=t.device), torch.empty(f, dtype=t.dtype, device=t.device)
+    W2, b2 = torch.empty((f, h), dtype=t.dtype, device=t.device), torch.empty(h, dtype=t.dtype, device=t.device)
+    for r, sh in enumerate(shards):
+        d = osdp_zdp_desc(desc.mlp, N, r)
+        for s in range(k):
+            sl = osdp_zdp_slice_layout(d, s)
+            fs = sl.hi - sl.lo
+            W1[r * h // N:(r + 1) * h // N, sl.lo:sl.hi] = sh[sl.w1_off:sl.w1_off + sl.w1_elems].reshape(h // N, fs)
+            b1[sl.lo + r * fs // N:sl.lo + (r + 1) * fs // N] = sh[sl.b1_off:sl.b1_off + sl.b1_elems]
+            W2[sl.lo + r * fs // N:sl.lo + (r + 1) * fs // N, :] = sh[sl.w2_off:sl.w2_off + sl.w2_elems].reshape(fs // N, h)
+        sl = osdp_zdp_slice_layout(d, k)
+        b2[r * h // N:(r + 1) * h // N] = sh[sl.b1_off:sl.b1_off + sl.b1_elems]
+    return W1, b1, W2, b2
+
+
+class _DevMem:
+    """A raw device range as a __cuda_array_interface__ object (so torch can wrap it without a copy)."""
+
+    def __init__(self, ptr, nbytes, typestr):
+        item = 4 if typestr == "<f4" else 1
+        self.__cuda_array_interface__ = {"shape": (nbytes // item,), "typestr": typestr, "data": (int(ptr), False),
+                                         "version": 2}
+
+
+class TorchDistComm:
+    """osdp_comm over torch.distributed (NCCL: ring / NVSwitch collectives over NVLink): the two collectives the paper
+    names.  The callbacks wrap the raw device ranges the library passes and enqueue the collective on the
+    stream it names.  Argument marshalling only."""
+
+    def __init__(self, group=None):
+        import torch.distributed as dist
+        self.dist, self.group = dist, group
+        self.world = dist.get_world_size(group)
+        self._ag = ALL_GATHER_FN(self._all_gather)
+        self._rs = REDUCE_SCATTER_FN(self._reduce_scatter)
+        self.struct = osdp_comm(None, self._ag, self._rs)
+        self.error = None
+
+    def _all_gather(self, ctx, send, recv, nbytes, stream):
+        try:
+            s = torch.as_tensor(_DevMem(send, nbytes, "|u1"), device="cuda")
+            r = torch.as_tensor(_DevMem(recv, nbytes * self.world, "|u1"), device="cuda")
+            with torch.cuda.stream(torch.cuda.ExternalStream(int(stream or 0))):
+                self.dist.all_gather_into_tensor(r, s, group=self.group)
+            return 0
+        except Exception as e:      # a Python exception must not unwind through C
+            self.error = e
+            return 1
+
+    def _reduce_scatter(self, ctx, send, recv, nfloats, stream):
+        try:
+            s = torch.as_tensor(_DevMem(send, nfloats * 4 * self.world, "<f4"), device="cuda")
+            r = torch.as_tensor(_DevMem(recv, nfloats * 4, "<f4"), device="cuda")
+            with torch.cuda.stream(torch.cuda.ExternalStream(int(stream or 0))):
+                self.dist.reduce_scatter_tensor(r, s, group=self.group)
+            return 0
+        except Exception as e:
+            self.error = e
+            return 1
+
+
+def osdp_zdp_ffn_split_mlp_forward(desc, param_shard, X, Y, workspace, comm=None, compute_stream=None, comm_stream=None,
+                                   check=True):
+    cs = _stream_ptr(compute_stream)
+    ms = cs if comm_stream is None else _stream_ptr(comm_stream)
+    st = _lib.osdp_zdp_ffn_split_mlp_forward(C.byref(desc), _ptr(param_shard), _ptr(X), _ptr(Y), _ptr(workspace),
+                                             workspace.numel() * workspace.element_size(),
+                                             C.byref(comm.struct) if comm is not None else None, cs, ms)
+    if check and st != OSDP_OK:
+        raise OsdpError(st, "osdp_zdp_ffn_split_mlp_forward", str(getattr(comm, "error", "") or ""))
+    return st
+
+
+def osdp_zdp_ffn_split_mlp_backward(desc, param_shard, X, dY, dX, grad_shard, workspace, comm=None, compute_stream=None,
+                                    comm_stream=None, check=True):
+    cs = _stream_ptr(compute_stream)
+    ms = cs if comm_stream is None else _stream_ptr(comm_stream)
+    st = _lib.osdp_zdp_ffn_split_mlp_backward(C.byref(desc), _ptr(param_shard), _ptr(X), _ptr(dY), _ptr(dX),
+                                              _ptr(grad_shard), _ptr(workspace),
+                                              workspace.numel() * workspace.element_size(),
+                                              C.byref(comm.struct) if comm is not None else None, cs, ms)
+    if check and st != OSDP_OK:
+        raise OsdpError(st, "osdp_zdp_ffn_split_mlp_backward", str(getattr(comm, "error", "") or ""))
+    return st
 
 
 # ---------------------------------------------------------------------------------------------- planner

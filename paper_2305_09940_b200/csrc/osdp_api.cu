@@ -240,6 +240,67 @@ inline int64_t tiles_256(int64_t m, int64_t n) { return ((m + 255) / 256) * ((n 
     if (_rc != OSDP_OK) return _rc; \
   } while (0)
 
+// ---- one slice of the ffn-axis split.  The slice's weights are given by pointer + leading
+// dimension, so the same code serves weights sliced in place (W1 + lo, ld = f) and gathered slice buffers (ZDP, ld = fs).
+struct FfnSliceW {
+  const void* W1s;   // W1[:, lo:hi]   [h x fs], leading dimension ldw1
+  int64_t ldw1;
+  const void* b1s;   // b1[lo:hi]
+  const void* W2s;   // W2[lo:hi, :]   [fs x h], leading dimension h
+};
+struct FfnSliceG {
+  float* dW1s;       // dW1[:, lo:hi]  [h x fs], leading dimension ldg1
+  int64_t ldg1;
+  float* db1s;       // db1[lo:hi]
+  float* dW2s;       // dW2[lo:hi, :]  [fs x h], leading dimension h
+};
+// H_s = gelu(X W1s + b1s); Y (+)= H_s W2s.  single = the operator has one slice (Y written directly, + b2).
+int ffn_slice_forward(int dt, int64_t T, int64_t h, int fs, const void* X, const FfnSliceW& w, const void* b2, void* Y,
+                      void* Hs, float* Yacc, bool single, bool first, cudaStream_t st) {
+  trace_set_step(1);
+  EpiParams e1 = {w.b1s, Hs, nullptr, nullptr, fs, 0};
+  OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_BIAS_GELU>(dt, X, h, w.W1s, w.ldw1, GemmShape{(int)T, fs, (int)h}, e1, st)));
+  // the paper's split: contraction axis sliced, partial products summed
+  trace_set_step(2);
+  if (single) {
+    EpiParams e2 = {b2, Y, nullptr, nullptr, h, 0};
+    OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_BIAS>(dt, Hs, fs, w.W2s, h, GemmShape{(int)T, (int)h, fs}, e2, st)));
+  } else {
+    EpiParams e2 = {nullptr, Yacc, nullptr, nullptr, h, first ? 0 : 1};
+    OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_ACCUM_F32>(dt, Hs, fs, w.W2s, h, GemmShape{(int)T, (int)h, fs}, e2, st)));
+  }
+  return OSDP_OK;
+}
+// Z_s, H_s recomputed; dZ_s; the slice's own parts of dW2, dW1, db1 (written once); dX (+)= dZ_s W1s^T.
+// db2 != nullptr: also db2 = colsum(dY) (once per call, with the first slice).
+int ffn_slice_backward(int dt, int64_t T, int64_t h, int fs, const void* X, const void* dY, const FfnSliceW& w,
+                       const FfnSliceG& g, void* Zs, void* Hs, void* dX, float* dXacc, float* scratch, float* db2,
+                       bool single, bool first, cudaStream_t st) {
+  trace_set_step(3);
+  EpiParams e3 = {w.b1s, Zs, Hs, nullptr, fs, 0};
+  OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_BIAS_GELU_DUAL>(dt, X, h, w.W1s, w.ldw1, GemmShape{(int)T, fs, (int)h}, e3, st)));
+  trace_set_step(4);
+  EpiParams e4 = {nullptr, Zs, nullptr, Zs, fs, 0};
+  OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_DGELU>(dt, dY, h, w.W2s, h, GemmShape{(int)T, fs, (int)h}, e4, st)));
+  trace_set_step(5);   // rows of dW2 belong to exactly one slice: written once, no accumulation
+  EpiParams e5 = {nullptr, g.dW2s, nullptr, nullptr, h, 0};
+  OSDP_TRY((gemm<MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32>(dt, Hs, fs, dY, h, GemmShape{fs, (int)h, (int)T}, e5, st)));
+  trace_set_step(8);
+  OSDP_TRY(colsum2(dt, dY, db2 ? (int)h : 0, db2, Zs, fs, g.db1s, (int)T, scratch, 0, st));
+  trace_set_step(6);   // columns of dW1 belong to exactly one slice
+  EpiParams e6 = {nullptr, g.dW1s, nullptr, nullptr, g.ldg1, 0};
+  OSDP_TRY((gemm<MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32>(dt, X, h, Zs, fs, GemmShape{(int)h, fs, (int)T}, e6, st)));
+  trace_set_step(7);   // the only result that spans slices
+  if (single) {
+    EpiParams e7 = {nullptr, dX, nullptr, nullptr, h, 0};
+    OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_PLAIN>(dt, Zs, fs, w.W1s, w.ldw1, GemmShape{(int)T, (int)h, fs}, e7, st)));
+  } else {
+    EpiParams e7 = {nullptr, dXacc, nullptr, nullptr, h, first ? 0 : 1};
+    OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_ACCUM_F32>(dt, Zs, fs, w.W1s, w.ldw1, GemmShape{(int)T, (int)h, fs}, e7, st)));
+  }
+  return OSDP_OK;
+}
+
 }  // namespace
 }  // namespace osdp
 
@@ -544,21 +605,9 @@ int osdp_ffn_split_mlp_forward(const osdp_mlp_desc* desc, const void* X, const v
     const int64_t lo = ffn_lo(desc, s), hi = ffn_lo(desc, s + 1);
     const int fs = (int)(hi - lo);
     if (fs == 0) continue;   // cannot happen for k <= units; kept for symmetry with the token split
-    // A1: H_s = gelu(X W1[:, lo:hi] + b1[lo:hi])                    [T x fs], compact
-    trace_set_step(1);
-    EpiParams e1 = {(const char*)b1 + (size_t)lo * e, Hs, nullptr, nullptr, fs, 0};
-    OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_BIAS_GELU>(dt, X, h, (const char*)W1 + (size_t)lo * e, desc->ffn,
-                                                     GemmShape{(int)T, fs, (int)h}, e1, st)));
-    // A2: Y (+)= H_s W2[lo:hi, :]   -- the paper's split: contraction axis sliced, partial products summed
-    trace_set_step(2);
-    const char* W2s = (const char*)W2 + (size_t)lo * h * e;
-    if (k == 1) {
-      EpiParams e2 = {b2, Y, nullptr, nullptr, h, 0};
-      OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_BIAS>(dt, Hs, fs, W2s, h, GemmShape{(int)T, (int)h, fs}, e2, st)));
-    } else {
-      EpiParams e2 = {nullptr, Yacc, nullptr, nullptr, h, s == 0 ? 0 : 1};
-      OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_ACCUM_F32>(dt, Hs, fs, W2s, h, GemmShape{(int)T, (int)h, fs}, e2, st)));
-    }
+    const FfnSliceW w = {(const char*)W1 + (size_t)lo * e, desc->ffn, (const char*)b1 + (size_t)lo * e,
+                         (const char*)W2 + (size_t)lo * h * e};
+    OSDP_TRY(ffn_slice_forward(dt, T, h, fs, X, w, b2, Y, Hs, Yacc, k == 1, s == 0, st));
   }
   if (k > 1) {   // Y = storage(Yacc + b2)
     trace_set_step(10);
@@ -595,36 +644,11 @@ int osdp_ffn_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const 
     const int64_t lo = ffn_lo(desc, s), hi = ffn_lo(desc, s + 1);
     const int fs = (int)(hi - lo);
     if (fs == 0) continue;
-    const char* W1s = (const char*)W1 + (size_t)lo * e;           // W1[:, lo:hi], leading dimension f
-    const char* W2s = (const char*)W2 + (size_t)lo * h * e;       // W2[lo:hi, :]
-    // A3: Z_s = X W1[:, lo:hi] + b1[lo:hi], H_s = gelu(Z_s)
-    trace_set_step(3);
-    EpiParams e3 = {(const char*)b1 + (size_t)lo * e, Zs, Hs, nullptr, fs, 0};
-    OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_BIAS_GELU_DUAL>(dt, X, h, W1s, f, GemmShape{(int)T, fs, (int)h}, e3, st)));
-    // A4: dZ_s = (dY W2[lo:hi, :]^T) (.) gelu'(Z_s), in place over Z_s
-    trace_set_step(4);
-    EpiParams e4 = {nullptr, Zs, nullptr, Zs, fs, 0};
-    OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_DGELU>(dt, dY, h, W2s, h, GemmShape{(int)T, fs, (int)h}, e4, st)));
-    // A5: dW2[lo:hi, :] = H_s^T dY       -- rows of dW2 belong to exactly one slice: written once, no accumulation
-    trace_set_step(5);
-    EpiParams e5 = {nullptr, dW2 + (size_t)lo * h, nullptr, nullptr, h, 0};
-    OSDP_TRY((gemm<MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32>(dt, Hs, fs, dY, h, GemmShape{fs, (int)h, (int)T}, e5, st)));
-    // A8: db1[lo:hi] = colsum(dZ_s); db2 = colsum(dY) once, with the first slice
-    trace_set_step(8);
-    OSDP_TRY(colsum2(dt, dY, s == 0 ? (int)h : 0, db2, Zs, fs, db1 + lo, (int)T, scratch, 0, st));
-    // A6: dW1[:, lo:hi] = X^T dZ_s       -- columns of dW1 belong to exactly one slice
-    trace_set_step(6);
-    EpiParams e6 = {nullptr, dW1 + lo, nullptr, nullptr, f, 0};
-    OSDP_TRY((gemm<MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32>(dt, X, h, Zs, fs, GemmShape{(int)h, fs, (int)T}, e6, st)));
-    // A7: dX (+)= dZ_s W1[:, lo:hi]^T    -- the only result that spans slices
-    trace_set_step(7);
-    if (k == 1) {
-      EpiParams e7 = {nullptr, dX, nullptr, nullptr, h, 0};
-      OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_PLAIN>(dt, Zs, fs, W1s, f, GemmShape{(int)T, (int)h, fs}, e7, st)));
-    } else {
-      EpiParams e7 = {nullptr, dXacc, nullptr, nullptr, h, s == 0 ? 0 : 1};
-      OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_ACCUM_F32>(dt, Zs, fs, W1s, f, GemmShape{(int)T, (int)h, fs}, e7, st)));
-    }
+    const FfnSliceW w = {(const char*)W1 + (size_t)lo * e, f, (const char*)b1 + (size_t)lo * e,
+                         (const char*)W2 + (size_t)lo * h * e};
+    const FfnSliceG g = {dW1 + lo, f, db1 + lo, dW2 + (size_t)lo * h};
+    OSDP_TRY(ffn_slice_backward(dt, T, h, fs, X, dY, w, g, Zs, Hs, dX, dXacc, scratch, s == 0 ? db2 : nullptr, k == 1,
+                                s == 0, st));
   }
   if (k > 1) {   // dX = storage(dXacc)
     trace_set_step(10);
@@ -638,3 +662,4 @@ int osdp_ffn_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const 
 }  // extern "C"
 
 #include "linear_api.inl"
+#include "zdp_api.inl"
