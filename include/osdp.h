@@ -73,9 +73,10 @@ const char* osdp_version(void);
 
 /* ---- A10: workspace accounting (PAPER.md:84-86 M_extra; PAPER.md:167 size/slice_granularity) ----------
  * Bytes of caller workspace one forward (OSDP_FWD) or backward (OSDP_BWD) call needs.  Pure host function.
- *   FWD: one [T_s x f] tensor (H_s);  BWD: two (Z_s, overwritten by dZ_s; H_s) + fixed fp32 column-sum scratch
- *   (32 x (hidden + ffn) floats);
- *   T_s = ceil(T/k); each tensor rounded up to 256 B.  Returns 0 on an invalid descriptor. */
+ *   FWD: one [T_s x f] tensor (H_s);  BWD: two (Z_s, overwritten by dZ_s; H_s) + the fp32 column-sum partials:
+ *   ceil(T_s / 32) x ffn floats (one row per 32-row band of dZ_s, written by the A4 epilogue: db1) and 32 x hidden
+ *   floats (db2);
+ *   T_s = ceil(T/k); each part rounded up to 256 B.  Returns 0 on an invalid descriptor. */
 size_t osdp_split_mlp_workspace_bytes(const osdp_mlp_desc* desc, int pass);
 
 /* ---- A0-A2: forward (DESIGN.md steps A1, A2) ---------------------------------------------
@@ -91,7 +92,9 @@ int osdp_split_mlp_forward(const osdp_mlp_desc* desc,
  *   Z_s = X_s W1 + b1, H_s = gelu(Z_s)                       (recomputed, workspace)
  *   dZ_s = (dY_s W2^T) (.) gelu'(Z_s)                        (overwrites Z_s)
  *   dW2 (+)= H_s^T dY_s;  dW1 (+)= X_s^T dZ_s                (fp32; "=" on slice 0, "+=" after: "summed")
- *   db1 (+)= colsum(dZ_s); db2 (+)= colsum(dY_s)             (fp32, fixed reduction order)
+ *   db1 (+)= colsum(dZ_s)                                    (fp32; 32-row band sums from the dZ_s epilogue, then a
+ *                                                             fixed-order sum over bands)
+ *   db2 = colsum(dY)                                         (fp32, fixed reduction order, once per call: dY is whole)
  *   dX_s = dZ_s W1^T                                         (rows of dX, storage dtype)
  * dX [T x h] storage dtype; dW1 [h x f], db1 [f], dW2 [f x h], db2 [h] fp32; all OVERWRITTEN (reading S11).
  * b2 is unused and may be NULL (reading S4). */
@@ -120,7 +123,8 @@ int osdp_split_mlp_backward(const osdp_mlp_desc* desc,
  *   - desc->k = number of ffn slices, 1 <= k <= ffn / (16 / sizeof(dtype));  lo_s = floor(s * units / k) * unit with
  *     unit = 16 bytes of elements and units = ffn / unit (slices are whole 16-byte column groups);
  *   - workspace (osdp_ffn_split_mlp_workspace_bytes): FWD one [tokens x f_max] tensor, BWD two, f_max = the widest
- *     slice; for k > 1 plus one fp32 [tokens x hidden] accumulator (Y or dX); BWD plus the column-sum scratch.
+ *     slice; for k > 1 plus one fp32 [tokens x hidden] accumulator (Y or dX); BWD plus the column-sum partials
+ *     (ceil(tokens / 32) x f_max floats for db1, 32 x hidden floats for db2).
  *     Each part rounded up to 256 B.
  *   - results: Y and dX differ across k only by fp32 re-association of the slice sums (then one rounding to the
  *     storage dtype); dW1, dW2, db1, db2 are bit-identical for every k.
@@ -185,7 +189,9 @@ int64_t osdp_last_launch_count(void);
  * MT = 2 when K >= OSDP_TUNE_MT2_MIN_K and either OSDP_TUNE_MT2_MIN_TILES = 0 and the 512 x 256 tiling idles at
  * most ~10 % more MMA slots than the 256 x 256 one (row padding, fill of the last wave), or it has at least
  * OSDP_TUNE_MT2_MIN_TILES > 0 such tiles.  OSDP_TUNE_WAVE_SYNC (MT = 2 launches of more than one wave): 0 off,
- * 1 at tile boundaries, q > 1 also every q k-blocks (64 contraction elements each) inside a tile.  OSDP_TUNE_BAND_MIB: L2 budget (MiB) for the A rows of one raster band.
+ * 1 at tile boundaries, q > 1 also every q k-blocks (64 contraction elements each) inside a tile.  OSDP_TUNE_BAND_MIB: 0 = raster bands that make one wave of
+ * resident CTA pairs cover a square-ish block of output tiles (least unique operand bytes per wave); n > 0 = bands whose A
+ * rows fit n MiB of L2 (round 1's rule).
  * OSDP_TUNE_CLUSTER_MIN_TILES: n > 0 = launches of at least n pair tiles run as 4-CTA clusters (two CTA pairs that
  * TMA-multicast the A rows they share); 0 = never (clusters of 4 CTAs can occupy only 132 of the 148 SMs).  Results do not depend on
  * any knob beyond fp32 summation order inside a tile (there is none: one owner per output tile).
@@ -194,7 +200,7 @@ typedef enum osdp_tune_key {
   OSDP_TUNE_MT2_MIN_K = 0,      /* default 4096 */
   OSDP_TUNE_MT2_MIN_TILES = 1,  /* default 0 (= efficiency rule) */
   OSDP_TUNE_WAVE_SYNC = 2,      /* default 1 */
-  OSDP_TUNE_BAND_MIB = 3,       /* default 32 */
+  OSDP_TUNE_BAND_MIB = 3,       /* default 0 */
   OSDP_TUNE_CLUSTER_MIN_TILES = 4, /* default 0 (multicast clusters off) */
   OSDP_TUNE_MT2_MIN_K_ACC = 5,     /* OSDP_TUNE_MT2_MIN_K for the fp32-accumulate launches (dW GEMMs, K = slice rows) */
   OSDP_TUNE_FORK_MAX_TILES = 6     /* default 256: in the token-split backward, the launches that only depend on dZ_s
@@ -234,18 +240,28 @@ typedef struct osdp_op_cost {
   double   delta;            /* seconds per extra slice (reading P2; 0 = the paper's model) */
 } osdp_op_cost;
 
-/* "Device information". */
+/* "Device information".  The last three fields describe activation checkpointing (PAPER.md:51,
+ * :251-253; reading P12) and may be left zero (= the paper's plain cost model): with checkpointing != 0
+ *   - a ZDP operator needs FOUR collectives: "the recomputation process before backward propagation requires an
+ *     additional round of gathering since each GPU does not maintain a full copy of model states";
+ *     DP operators keep their two - which is why OSDP "can leave operators with smaller memory overhead in DP mode";
+ *   - computation costs (1 + recompute_fraction) b gamma ("about 30% extra computation overhead");
+ *   - only act_keep_fraction of b M_act stays resident (the checkpoints). */
 typedef struct osdp_device {
   int32_t  N;                /* parallelism degree >= 1 */
   double   alpha;            /* network latency, seconds */
   double   beta;             /* transfer seconds per byte */
   uint64_t mem_limit_bytes;  /* M_limit */
+  int32_t  checkpointing;    /* 0 = off */
+  double   recompute_fraction;   /* >= 0; the paper's figure is ~0.3 */
+  double   act_keep_fraction;    /* in [0, 1] */
 } osdp_device;
 
 /* M_i and T_i of one operator (readings P1, P2):
  *   persist   = model/(N if ZDP else 1, rounded up) + batch*act + extra_fixed + ceil(extra_summed/k)
  *   transient = ceil(extra_transient/k)
  *   seconds   = c (N-1)(alpha + S beta/N) + batch*gamma + (k-1) delta,  c = 2 (DP) / 3 (ZDP)
+ * With dev->checkpointing: c = 2 / 4, batch*gamma*(1 + recompute_fraction), ceil(batch*act*act_keep_fraction).
  * Any output pointer may be NULL. */
 int osdp_cost_eval(const osdp_op_cost* op, int mode, int32_t k, int64_t batch, const osdp_device* dev,
                    uint64_t* persist_bytes, uint64_t* transient_bytes, double* seconds);

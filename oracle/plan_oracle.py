@@ -58,6 +58,12 @@ class Device:
     alpha: float = 0.0
     beta: float = 0.0
     mem_limit: int = 0
+    # Activation checkpointing ("about 30% extra computation overhead"; "the recomputation
+    # process before backward propagation requires an additional round of gathering"; reading P12).  Off = the paper's
+    # plain cost model.
+    checkpointing: bool = False
+    recompute_fraction: float = 0.0
+    act_keep_fraction: float = 1.0
 
 
 def ceil_div(a: int, b: int) -> int:
@@ -67,11 +73,21 @@ def ceil_div(a: int, b: int) -> int:
 def cost_eval(op: OpCost, mode: int, k: int, b: int, dev: Device):
     """(persistent_bytes, transient_bytes, seconds) of one operator under (mode, k, b)."""
     model = ceil_div(op.model, dev.N) if mode == ZDP else op.model
-    persist = model + b * op.act + op.extra_fixed + ceil_div(op.extra_summed, k)
+    persist = model + _act_bytes(op, b, dev) + op.extra_fixed + ceil_div(op.extra_summed, k)
     transient = ceil_div(op.extra_transient, k)
-    c = 3.0 if mode == ZDP else 2.0
-    t = c * (dev.N - 1) * (dev.alpha + op.S * dev.beta / dev.N) + b * op.gamma + (k - 1) * op.delta
+    c = (4.0 if dev.checkpointing else 3.0) if mode == ZDP else 2.0
+    t = c * (dev.N - 1) * (dev.alpha + op.S * dev.beta / dev.N) + _compute_seconds(op, b, dev) + (k - 1) * op.delta
     return persist, transient, t
+
+
+def _act_bytes(op: OpCost, b: int, dev: Device) -> int:
+    """b M_act, of which only the checkpoints stay resident under activation checkpointing."""
+    return math.ceil(b * op.act * dev.act_keep_fraction) if dev.checkpointing else b * op.act
+
+
+def _compute_seconds(op: OpCost, b: int, dev: Device) -> float:
+    """b gamma, plus the recomputation of the forward under activation checkpointing."""
+    return b * op.gamma * (1.0 + dev.recompute_fraction) if dev.checkpointing else b * op.gamma
 
 
 def to_ps(seconds: float) -> int:
@@ -118,10 +134,10 @@ def cost_eval_mixed(op: OpCost, k: int, z: int, b: int, dev: Device):
     assert 0 <= z <= k
     zdp_share = ceil_div(op.model * z, k)
     model = (op.model - zdp_share) + ceil_div(zdp_share, dev.N)
-    persist = model + b * op.act + op.extra_fixed + ceil_div(op.extra_summed, k)
+    persist = model + _act_bytes(op, b, dev) + op.extra_fixed + ceil_div(op.extra_summed, k)
     transient = ceil_div(op.extra_transient, k)
-    c = (2.0 * (k - z) + 3.0 * z) / k
-    t = c * (dev.N - 1) * (dev.alpha + op.S * dev.beta / dev.N) + b * op.gamma + (k - 1) * op.delta
+    c = (2.0 * (k - z) + (4.0 if dev.checkpointing else 3.0) * z) / k
+    t = c * (dev.N - 1) * (dev.alpha + op.S * dev.beta / dev.N) + _compute_seconds(op, b, dev) + (k - 1) * op.delta
     return persist, transient, t
 
 
@@ -167,20 +183,23 @@ def schedule_brute_force(ops, dev: Device, k_candidates, b_max: int = 1 << 20):
 # library source. -------------------------------------------------------------------------------------
 def mlp_workspace_bytes(T: int, h: int, f: int, e: int, k: int, backward: bool) -> int:
     """Bytes of caller workspace one call needs: per-slice T_s x f buffers (1 fwd: H_s; 2 bwd: Z_s/dZ_s
-    and H_s), each rounded up to 256 B, plus (bwd) the fixed column-sum scratch."""
+    and H_s), each rounded up to 256 B, plus (bwd) the column-sum scratch of one slice."""
     Ts = ceil_div(T, k)
     buf = ceil_div(Ts * f * e, 256) * 256
     if not backward:
         return buf
-    return 2 * buf + mlp_reduce_scratch_bytes(h, f)
+    return 2 * buf + mlp_reduce_scratch_bytes(Ts, h, f)
 
 
+BAND_ROWS = 32
 REDUCE_ROW_CHUNKS = 32
 
 
-def mlp_reduce_scratch_bytes(h: int, f: int) -> int:
-    """fp32 partial column sums for db2 and db1: REDUCE_ROW_CHUNKS x (h + f) floats, 256 B aligned."""
-    return ceil_div(REDUCE_ROW_CHUNKS * (h + f) * 4, 256) * 256
+def mlp_reduce_scratch_bytes(Ts: int, h: int, f: int) -> int:
+    """fp32 partial column sums: db1 keeps one partial row per BAND_ROWS-row band of the slice's
+    dZ_s (ceil(T_s / 32) x f floats, written by the A4 epilogue), db2 REDUCE_ROW_CHUNKS partial rows of dY (32 x h
+    floats); each part rounded up to 256 B."""
+    return ceil_div(ceil_div(Ts, BAND_ROWS) * f * 4, 256) * 256 + ceil_div(REDUCE_ROW_CHUNKS * h * 4, 256) * 256
 
 
 def mlp_persistent_bytes(T: int, h: int, f: int, e: int, backward: bool) -> int:

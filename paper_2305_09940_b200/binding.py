@@ -85,7 +85,8 @@ class osdp_op_cost(C.Structure):
 
 
 class osdp_device(C.Structure):
-    _fields_ = [("N", C.c_int32), ("alpha", C.c_double), ("beta", C.c_double), ("mem_limit_bytes", C.c_uint64)]
+    _fields_ = [("N", C.c_int32), ("alpha", C.c_double), ("beta", C.c_double), ("mem_limit_bytes", C.c_uint64),
+                ("checkpointing", C.c_int32), ("recompute_fraction", C.c_double), ("act_keep_fraction", C.c_double)]
 
 
 _lib.osdp_status_string.restype = C.c_char_p

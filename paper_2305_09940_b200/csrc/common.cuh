@@ -34,6 +34,10 @@ struct EpiParams {
   const void* aux;    // EPI_DGELU: Z_s
   int64_t ldo;        // leading dimension (elements) of out0/out1/aux
   int beta;           // EPI_ACCUM_F32: 0 = overwrite (first slice), 1 = accumulate
+  // EPI_DGELU (A4): the epilogue also leaves the column sums of every 32-row band of dZ_s here,
+  // colsum[(row / 32) * ld_colsum + col], for the fixed-order db1 reduction (reduce.cuh); nullptr = not wanted
+  float* colsum = nullptr;
+  int64_t ld_colsum = 0;
 };
 
 struct GemmShape {

@@ -31,6 +31,7 @@
 #include <cuda.h>
 
 #include <atomic>
+#include <cmath>
 #include <mutex>
 
 #include "common.cuh"
@@ -51,7 +52,7 @@ struct Tuning {
   std::atomic<int64_t> mt2_min_k_acc{4096}; // the same for the fp32-accumulate epilogue (dW GEMMs: K = slice rows)
   std::atomic<int64_t> mt2_min_tiles{0};    // 0: MT = 2 when it idles at most ~10 % more MMA slots than MT = 1; > 0: plain threshold
   std::atomic<int64_t> wave_sync{1};        // line the producers up at tile boundaries (MT = 2 launches)
-  std::atomic<int64_t> band_mib{32};        // L2 budget for the A rows of one raster band
+  std::atomic<int64_t> band_mib{0};         // 0: square-wave raster bands; > 0: band = tile rows whose A rows fit this many MiB of L2
   std::atomic<int64_t> cluster_min_tiles{0};   // > 0: multicast clusters for launches of at least this many pair tiles
   std::atomic<int64_t> fork_max_tiles{256};    // backward: A5 | A6 | A7 | column sums run concurrently when each GEMM has at most this many 256 x 256 tiles
 };
@@ -59,6 +60,7 @@ inline Tuning& tuning() {
   static Tuning t;
   return t;
 }
+constexpr int kPrefetchMaxK = 1024;   // fp32 accumulate launches with K up to this prefetch the old output tile into L2
 constexpr int kTmemCols = 512;
 constexpr int kThreads = 384;      // warps 0-3: TMA, MMA, TMEM alloc, (idle); warps 4-11: epilogue
 constexpr int kEpiWarp0 = 4;
@@ -202,6 +204,12 @@ __device__ __forceinline__ void tma_reduce_add_2d(const CUtensorMap* map, uint32
                ::"l"((uint64_t)map), "r"(src), "r"(c_inner), "r"(c_outer)
                : "memory");
 }
+// Bring the box at these coordinates into L2 (no shared-memory destination, nothing to wait for).
+__device__ __forceinline__ void tma_prefetch_l2_2d(const CUtensorMap* map, int c_inner, int c_outer) {
+  asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];"
+               ::"l"((uint64_t)map), "r"(c_inner), "r"(c_outer)
+               : "memory");
+}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
@@ -314,6 +322,10 @@ struct StorePipe {
   int lane;
   int cur = 0;      // buffer the next chunk goes to
   __device__ __forceinline__ uint32_t buf() const { return base + (uint32_t)cur * kStoreBufBytes; }
+  // the buffer the last commit() handed to TMA (still intact until the next begin() on it)
+  __device__ __forceinline__ uint32_t committed_buf() const {
+    return base + (uint32_t)(NBUF > 1 ? (cur == 0 ? NBUF - 1 : cur - 1) : 0) * kStoreBufBytes;
+  }
   __device__ __forceinline__ void begin() const {
     if (lane == 0) bulk_wait_read<NBUF - 1>();   // the store that last used this buffer has read it out
     __syncwarp();
@@ -625,6 +637,22 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
           bias_reg[ci] = c < shape.N ? __ldg(reinterpret_cast<const uint32_t*>(bias + c)) : 0u;   // N is even
         }
       }
+      if constexpr (Tr::kF32Out) {
+        // Cross-slice accumulation (beta = 1) is a reduce-add performed AT L2; on a miss L2 first fetches the old line
+        // from DRAM, and a warp's next chunk waits behind that (one staging buffer), so the drain of a tile runs at the
+        // DRAM latency: ~2.8 k cycles per 4 KiB chunk (ncu, C4).  With short slices (K = T_s <= 1024) the main loop is too
+        // short to hide that, so the warp asks for its chunks of the old dW tile while the main loop is still running and
+        // the reduce-adds hit in L2: +3.7 % per step at C4 k = 16.  For longer K the drain is hidden anyway and the
+        // prefetch only costs L2 space (-0.5 ... -1.5 % at K = 2048), so it is limited to short K.
+        if (ep.beta != 0 && shape.K <= kPrefetchMaxK && lane == 0) {
+#pragma unroll 1
+          for (int h = 0; h < MT; ++h) {
+            const int prow0 = (tc.m_blk * CM + pi) * kPairM + (int)rank * kCtaM + h * BLOCK_M + q * 32;
+            if (prow0 >= shape.M) continue;
+            for (int n = n0 + cg * kChunk; n < n_end; n += 2 * kChunk) tma_prefetch_l2_2d(&tmap_out0, n, prow0);
+          }
+        }
+      }
       mbar_wait(tfull_bar + 8 * as, aphase);
       tc_fence_after();
       bool released = false;   // the accumulator stage goes back to the MMA warp right after this warp's last tcgen05.ld
@@ -694,6 +722,27 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
               pipe.put(j, pack8(v));
             }
             pipe.commit(EPI == EPI_BIAS_GELU_DUAL ? &tmap_out1 : &tmap_out0, n, row0, false);
+            if constexpr (EPI == EPI_DGELU) {
+              // db1 (step A4 of SURVEY.md section 8(a)): column sums of this warp's 32 rows x 64 columns of dZ_s, taken
+              // from the staged bf16 values (exactly what is stored).  Lane l owns columns 2l and 2l + 1 and walks the
+              // 32 rows in order (word l of every 128-byte row: conflict-free under the 128B swizzle); rows outside M hold
+              // zeros (zero-filled operand rows).  One 256-byte store per chunk into the band-partials scratch; the
+              // fixed-order sum over bands is colsum_final_kernel's.
+              if (ep.colsum != nullptr) {
+                const uint32_t src = pipe.committed_buf() + ((lane & 3) << 2);
+                float s0 = 0.0f, s1 = 0.0f;
+#pragma unroll
+                for (int r = 0; r < 32; ++r) {
+                  uint32_t w;
+                  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(w) : "r"(src + r * 128 + ((((uint32_t)lane >> 2) ^ (r & 7)) << 4)));
+                  s0 += bf16_lo(w);
+                  s1 += bf16_hi(w);
+                }
+                const int c = n + 2 * lane;
+                if (c < shape.N)
+                  *reinterpret_cast<float2*>(ep.colsum + (int64_t)(row0 >> 5) * ep.ld_colsum + c) = make_float2(s0, s1);
+              }
+            }
           }
         }
       }   // h
@@ -854,10 +903,26 @@ inline int launch_gemm_bf16_cluster(const void* A, int64_t lda, const void* B, i
   const int num_m = (s.M + Cfg::kPairM - 1) / Cfg::kPairM, num_n = (s.N + BLOCK_N - 1) / BLOCK_N;   // pair tiles
   const int tiles = ((num_m + CM - 1) / CM) * ((num_n + CN - 1) / CN);                      // cluster tiles
   cfg.gridDim = dim3(kCluster * (tiles < max_clusters ? tiles : max_clusters));
-  // Raster band: as many cluster-tile rows as keep the band's A rows (band rows x K bf16) inside the L2 budget;
-  // DRAM reads are about |A| + |B| * (row bands), so taller is better while A stays resident.
-  const int64_t row_bytes = (int64_t)CM * Cfg::kPairM * s.K * 2;
-  int64_t group_m = (tuning().band_mib.load() << 20) / row_bytes;
+  // Raster band = group_m tile rows; inside a band tiles walk m fastest, then n, so one wave of P resident clusters
+  // covers group_m tile rows x P / group_m tile columns.  All clusters of a wave sweep K in step (wave sync, or simply
+  // equal work), so what a wave pulls from DRAM is its UNIQUE operand rows and columns, about
+  // (group_m * rows_per_tile + P / group_m * cols_per_tile) * K elements: least for a square-ish wave,
+  // group_m = sqrt(P * cols_per_tile / rows_per_tile), whatever K is.  (Round 1 sized the band so that its A rows fit an
+  // L2 budget; for long K that degenerates to one tile row per band and B is re-read per row: 1.24 GB instead of
+  // 0.67 GB for the A2 / A7 launches of C4 k = 4.  OSDP_TUNE_BAND_MIB > 0 brings that rule back.)
+  int64_t group_m;
+  const int64_t band_mib = tuning().band_mib.load();
+  if (band_mib > 0) {
+    const int64_t row_bytes = (int64_t)CM * Cfg::kPairM * s.K * 2;
+    group_m = (band_mib << 20) / row_bytes;
+  } else {
+    const int num_cm = (num_m + CM - 1) / CM;
+    const double ideal = std::sqrt((double)max_clusters * (CN * BLOCK_N) / (double)(CM * Cfg::kPairM));
+    int64_t g = (int64_t)(ideal + 0.5);
+    if (g < 1) g = 1;
+    const int64_t bands = (num_cm + g - 1) / g;          // equal bands: no thin last band
+    group_m = (num_cm + bands - 1) / bands;
+  }
   if (group_m < 1) group_m = 1;
   if (group_m > (1 << 20)) group_m = 1 << 20;
   // wave sync only when there is more than one wave, and only with a fully resident grid

@@ -137,7 +137,7 @@ int osdp_split_linear_backward(const osdp_linear_desc* desc, const void* X, cons
     // dX_s, dW (+)=, db (+)= only share inputs: side by side on small slices (helper streams, osdp_api.cu)
     const int64_t ts_max = (T + k - 1) / k;
     const int64_t fork_max = sm100::tuning().fork_max_tiles.load();
-    const bool fork = dt == OSDP_BF16 && fork_max > 0 && tiles_256(in, of) <= fork_max && tiles_256(ts_max, in) <= fork_max;
+    const bool fork = fork_max > 0 && tiles_256(in, of) <= fork_max && tiles_256(ts_max, in) <= fork_max;
     ForkCtx* fc = nullptr;
     if (fork) {
       OSDP_TRY(fork_ctx(&fc));
@@ -162,7 +162,7 @@ int osdp_split_linear_backward(const osdp_linear_desc* desc, const void* X, cons
                                                         fork ? fc->side[0] : st)));
       if (desc->has_bias) {
         trace_set_step(8);  // db (+)= colsum(dY_s)
-        OSDP_TRY(colsum2(dt, dYs, 0, db, dYs, (int)of, db, Ts, scratch, beta, fork ? fc->side[1] : st));
+        OSDP_TRY(colsum_rows(dt, dYs, (int)of, db, Ts, scratch, beta, fork ? fc->side[1] : st));
       }
     }
     if (fork) OSDP_TRY(join_into(fc, st));
@@ -171,7 +171,7 @@ int osdp_split_linear_backward(const osdp_linear_desc* desc, const void* X, cons
   // contraction axis: every slice writes its own columns of dX and rows of dW; db once
   if (desc->has_bias) {
     trace_set_step(8);
-    OSDP_TRY(colsum2(dt, dY, 0, db, dY, (int)of, db, (int)T, scratch, 0, st));
+    OSDP_TRY(colsum_rows(dt, dY, (int)of, db, (int)T, scratch, 0, st));
   }
   for (int s = 0; s < k; ++s) {
     const int64_t lo = lin_lo(desc, s), hi = lin_lo(desc, s + 1);

@@ -113,12 +113,16 @@ inline size_t slice_buf_bytes(const osdp_mlp_desc* d) {
   const int64_t ts = (d->tokens + d->k - 1) / d->k;
   return align_up((size_t)ts * (size_t)d->ffn * elem_size(d->dtype), 256);
 }
-inline size_t reduce_scratch_bytes(const osdp_mlp_desc* d) {
-  return align_up((size_t)kReduceRowChunks * (size_t)(d->hidden + d->ffn) * 4, 256);
+// Column-sum scratch: db1 = one fp32 partial row per 32-row band of the slice's dZ_s (written by
+// the A4 epilogue), db2 = kReduceRowChunks partial rows of dY.
+inline size_t db1_scratch_bytes(int64_t slice_rows, int64_t cols) {
+  return align_up((size_t)((slice_rows + kBandRows - 1) / kBandRows) * (size_t)cols * 4, 256);
 }
+inline size_t db2_scratch_bytes(int64_t h) { return align_up((size_t)kReduceRowChunks * (size_t)h * 4, 256); }
 size_t workspace_bytes(const osdp_mlp_desc* d, int pass) {
   if (pass == OSDP_FWD) return slice_buf_bytes(d);
-  return 2 * slice_buf_bytes(d) + reduce_scratch_bytes(d);
+  const int64_t ts = (d->tokens + d->k - 1) / d->k;
+  return 2 * slice_buf_bytes(d) + db1_scratch_bytes(ts, d->ffn) + db2_scratch_bytes(d->hidden);
 }
 
 // ---- ffn-axis split: slice s owns ffn columns [ffn_lo(s), ffn_lo(s + 1)), whole 16-byte units
@@ -149,7 +153,8 @@ inline size_t ffn_acc_bytes(const osdp_mlp_desc* d) {   // fp32 accumulator of Y
 }
 size_t ffn_workspace_bytes(const osdp_mlp_desc* d, int pass) {
   if (pass == OSDP_FWD) return ffn_slice_buf_bytes(d) + ffn_acc_bytes(d);
-  return 2 * ffn_slice_buf_bytes(d) + ffn_acc_bytes(d) + reduce_scratch_bytes(d);
+  return 2 * ffn_slice_buf_bytes(d) + ffn_acc_bytes(d) + db1_scratch_bytes(d->tokens, ffn_slice_max(d)) +
+         db2_scratch_bytes(d->hidden);
 }
 
 inline bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) != 0; }
@@ -177,13 +182,17 @@ int gemm(int dtype, const void* A, int64_t lda, const void* B, int64_t ldb, cons
   return launch_gemm_f32<EPI>(op, s, ep, st);
 }
 
-// db2 (+)= colsum(dY_s [rows x h]), db1 (+)= colsum(dZ_s [rows x f])
-int colsum2(int dtype, const void* dYs, int h, float* db2, const void* dZs, int f, float* db1, int rows, float* scratch,
-            int beta, cudaStream_t st) {
+// out (+)= colsum(src [rows x cols]) in kReduceRowChunks equal row chunks (db2, and the Linear operator's db)
+int colsum_rows(int dtype, const void* src, int cols, float* out, int rows, float* scratch, int beta, cudaStream_t st) {
+  if (dtype == OSDP_BF16) return launch_colsum<__nv_bfloat16>((const __nv_bfloat16*)src, cols, cols, out, rows, 0, scratch, beta, st);
+  return launch_colsum<float>((const float*)src, cols, cols, out, rows, 0, scratch, beta, st);
+}
+// db1 (+)= colsum(dZ_s [rows x cols]) from the 32-row band partials.  bf16: the A4 epilogue has already written them to
+// `scratch` (one launch here); fp32: the FFMA GEMM has no such epilogue, a kernel makes the same partials first.
+int db1_from_bands(int dtype, const void* dZs, int cols, float* out, int rows, float* scratch, int beta, cudaStream_t st) {
   if (dtype == OSDP_BF16)
-    return launch_colsum2<__nv_bfloat16>((const __nv_bfloat16*)dYs, h, h, db2, (const __nv_bfloat16*)dZs, f, f, db1, rows,
-                                         scratch, beta, st);
-  return launch_colsum2<float>((const float*)dYs, h, h, db2, (const float*)dZs, f, f, db1, rows, scratch, beta, st);
+    return launch_colsum_final(scratch, cols, (rows + kBandRows - 1) / kBandRows, out, 0, 0, nullptr, beta, st);
+  return launch_colsum<float>((const float*)dZs, cols, cols, out, rows, kBandRows, scratch, beta, st);
 }
 
 // ---- helper streams: independent launches of one slice side by side ------------------------------------------
@@ -274,19 +283,20 @@ int ffn_slice_forward(int dt, int64_t T, int64_t h, int fs, const void* X, const
 // Z_s, H_s recomputed; dZ_s; the slice's own parts of dW2, dW1, db1 (written once); dX (+)= dZ_s W1s^T.
 // db2 != nullptr: also db2 = colsum(dY) (once per call, with the first slice).
 int ffn_slice_backward(int dt, int64_t T, int64_t h, int fs, const void* X, const void* dY, const FfnSliceW& w,
-                       const FfnSliceG& g, void* Zs, void* Hs, void* dX, float* dXacc, float* scratch, float* db2,
-                       bool single, bool first, cudaStream_t st) {
+                       const FfnSliceG& g, void* Zs, void* Hs, void* dX, float* dXacc, float* scratch1, float* scratch2,
+                       float* db2, bool single, bool first, cudaStream_t st) {
   trace_set_step(3);
   EpiParams e3 = {w.b1s, Zs, Hs, nullptr, fs, 0};
   OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_BIAS_GELU_DUAL>(dt, X, h, w.W1s, w.ldw1, GemmShape{(int)T, fs, (int)h}, e3, st)));
-  trace_set_step(4);
-  EpiParams e4 = {nullptr, Zs, nullptr, Zs, fs, 0};
+  trace_set_step(4);   // the epilogue also leaves the 32-row band sums of dZ_s in scratch1 (db1)
+  EpiParams e4 = {nullptr, Zs, nullptr, Zs, fs, 0, scratch1, fs};
   OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_DGELU>(dt, dY, h, w.W2s, h, GemmShape{(int)T, fs, (int)h}, e4, st)));
   trace_set_step(5);   // rows of dW2 belong to exactly one slice: written once, no accumulation
   EpiParams e5 = {nullptr, g.dW2s, nullptr, nullptr, h, 0};
   OSDP_TRY((gemm<MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32>(dt, Hs, fs, dY, h, GemmShape{fs, (int)h, (int)T}, e5, st)));
   trace_set_step(8);
-  OSDP_TRY(colsum2(dt, dY, db2 ? (int)h : 0, db2, Zs, fs, g.db1s, (int)T, scratch, 0, st));
+  OSDP_TRY(db1_from_bands(dt, Zs, fs, g.db1s, (int)T, scratch1, 0, st));
+  if (db2) OSDP_TRY(colsum_rows(dt, dY, (int)h, db2, (int)T, scratch2, 0, st));
   trace_set_step(6);   // columns of dW1 belong to exactly one slice
   EpiParams e6 = {nullptr, g.dW1s, nullptr, nullptr, g.ldg1, 0};
   OSDP_TRY((gemm<MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32>(dt, X, h, Zs, fs, GemmShape{(int)h, fs, (int)T}, e6, st)));
@@ -346,7 +356,7 @@ int osdp_set_tuning(int key, int64_t value) {
       t.wave_sync = value;
       return OSDP_OK;
     case OSDP_TUNE_BAND_MIB:
-      if (value < 1 || value > 1024) return OSDP_ERR_ARG;
+      if (value < 0 || value > 1024) return OSDP_ERR_ARG;
       t.band_mib = value;
       return OSDP_OK;
     case OSDP_TUNE_CLUSTER_MIN_TILES:
@@ -445,8 +455,8 @@ int osdp_mlp_op_cost(const osdp_mlp_desc* desc, int pass, osdp_op_cost* out) {
   } else {
     c.model_bytes = (2 * h * f + f + h) * e + (2 * h * f + f + h) * 4;   // W, b; fp32 dW, db
     c.act_bytes = 3 * T * h * e;                                      // X, dY, dX
-    c.extra_transient = 2 * T * f * e;                                // Z/dZ and H
-    c.extra_fixed = reduce_scratch_bytes(desc);
+    c.extra_transient = 2 * T * f * e + (T * f * 4) / kBandRows;      // Z/dZ, H and the db1 band partials: all per slice
+    c.extra_fixed = db2_scratch_bytes(h);
   }
   *out = c;
   return OSDP_OK;
@@ -505,12 +515,17 @@ int osdp_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const void
   const size_t buf = slice_buf_bytes(desc);
   void* Zs = workspace;                                  // Z_s, then dZ_s in place
   void* Hs = (char*)workspace + buf;                     // H_s
-  float* scratch = (float*)((char*)workspace + 2 * buf);   // column-sum partials
+  const int64_t ts_max = (T + desc->k - 1) / desc->k;
+  float* scratch1 = (float*)((char*)workspace + 2 * buf);                                   // db1: band partials of dZ_s
+  float* scratch2 = (float*)((char*)workspace + 2 * buf + db1_scratch_bytes(ts_max, f));    // db2: chunk partials of dY
+
+  // db2 = colsum(dY): dY is whole in memory, so one fixed-order reduction per call (not per slice; bit-identical for every k)
+  trace_set_step(8);
+  OSDP_TRY(colsum_rows(dt, dY, (int)h, db2, (int)T, scratch2, 0, st));
 
   // Small slices: the three GEMMs and the column sums that only need dZ_s run side by side (helper streams above).
-  const int64_t ts_max = (T + desc->k - 1) / desc->k;
   const int64_t fork_max = sm100::tuning().fork_max_tiles.load();
-  const bool fork = dt == OSDP_BF16 && fork_max > 0 && tiles_256(f, h) <= fork_max && tiles_256(ts_max, h) <= fork_max;
+  const bool fork = fork_max > 0 && tiles_256(f, h) <= fork_max && tiles_256(ts_max, h) <= fork_max;
   ForkCtx* fc = nullptr;
   if (fork) OSDP_TRY(fork_ctx(&fc));
 
@@ -528,18 +543,18 @@ int osdp_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const void
     trace_set_step(3);
     EpiParams e3 = {b1, Zs, Hs, nullptr, f, 0};
     OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_BIAS_GELU_DUAL>(dt, Xs, h, W1, f, GemmShape{Ts, (int)f, (int)h}, e3, st)));
-    // A4: dZ_s = (dY_s W2^T) (.) gelu'(Z_s), in place over Z_s
+    // A4: dZ_s = (dY_s W2^T) (.) gelu'(Z_s), in place over Z_s; the epilogue also leaves the 32-row band sums (db1)
     trace_set_step(4);
-    EpiParams e4 = {nullptr, Zs, nullptr, Zs, f, 0};
+    EpiParams e4 = {nullptr, Zs, nullptr, Zs, f, 0, scratch1, f};
     OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_DGELU>(dt, dYs, h, W2, h, GemmShape{Ts, (int)f, (int)h}, e4, st)));
     if (fork) OSDP_TRY(fork_from(fc, st));
     // A5: dW2 (+)= H_s^T dY_s
     trace_set_step(5);
     EpiParams e5 = {nullptr, dW2, nullptr, nullptr, h, beta};
     OSDP_TRY((gemm<MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32>(dt, Hs, f, dYs, h, GemmShape{(int)f, (int)h, Ts}, e5, st)));
-    // A8: db2 (+)= colsum(dY_s);  db1 (+)= colsum(dZ_s)
+    // A8: db1 (+)= colsum(dZ_s), fixed-order sum of the band partials
     trace_set_step(8);
-    OSDP_TRY(colsum2(dt, dYs, (int)h, db2, Zs, (int)f, db1, Ts, scratch, beta, fork ? fc->side[2] : st));
+    OSDP_TRY(db1_from_bands(dt, Zs, (int)f, db1, Ts, scratch1, beta, fork ? fc->side[2] : st));
     // A6: dW1 (+)= X_s^T dZ_s
     trace_set_step(6);
     EpiParams e6 = {nullptr, dW1, nullptr, nullptr, f, beta};
@@ -577,8 +592,8 @@ int osdp_ffn_split_mlp_op_cost(const osdp_mlp_desc* desc, int pass, osdp_op_cost
   } else {
     c.model_bytes = (2 * h * f + f + h) * e + (2 * h * f + f + h) * 4;
     c.act_bytes = 3 * T * h * e;
-    c.extra_transient = 2 * T * f * e;
-    c.extra_fixed = acc + reduce_scratch_bytes(desc);
+    c.extra_transient = 2 * T * f * e + db1_scratch_bytes(T, f);     // db1 band partials of one slice: ceil(T / 32) x f / k floats
+    c.extra_fixed = acc + db2_scratch_bytes(h);
   }
   *out = c;
   return OSDP_OK;
@@ -638,7 +653,8 @@ int osdp_ffn_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const 
   void* Zs = workspace;                                  // Z_s, then dZ_s in place       [T x fs]
   void* Hs = (char*)workspace + buf;                     // H_s                           [T x fs]
   float* dXacc = (float*)((char*)workspace + 2 * buf);   // fp32 accumulator of dX        [T x h]   (k > 1)
-  float* scratch = (float*)((char*)workspace + 2 * buf + ffn_acc_bytes(desc));
+  float* scratch1 = (float*)((char*)workspace + 2 * buf + ffn_acc_bytes(desc));                      // db1 band partials
+  float* scratch2 = (float*)((char*)scratch1 + db1_scratch_bytes(T, ffn_slice_max(desc)));           // db2 chunk partials
 
   for (int s = 0; s < k; ++s) {
     const int64_t lo = ffn_lo(desc, s), hi = ffn_lo(desc, s + 1);
@@ -647,8 +663,8 @@ int osdp_ffn_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const 
     const FfnSliceW w = {(const char*)W1 + (size_t)lo * e, f, (const char*)b1 + (size_t)lo * e,
                          (const char*)W2 + (size_t)lo * h * e};
     const FfnSliceG g = {dW1 + lo, f, db1 + lo, dW2 + (size_t)lo * h};
-    OSDP_TRY(ffn_slice_backward(dt, T, h, fs, X, dY, w, g, Zs, Hs, dX, dXacc, scratch, s == 0 ? db2 : nullptr, k == 1,
-                                s == 0, st));
+    OSDP_TRY(ffn_slice_backward(dt, T, h, fs, X, dY, w, g, Zs, Hs, dX, dXacc, scratch1, scratch2, s == 0 ? db2 : nullptr,
+                                k == 1, s == 0, st));
   }
   if (k > 1) {   // dX = storage(dXacc)
     trace_set_step(10);

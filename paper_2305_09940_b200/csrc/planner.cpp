@@ -36,15 +36,19 @@ struct OptionCost {
 bool eval_mixed(const osdp_op_cost& op, int32_t k, int32_t z, int64_t batch, const osdp_device& dev,
                 uint64_t* persist, uint64_t* transient, double* seconds) {
   if (k < 1 || z < 0 || z > k || batch < 0 || dev.N < 1) return false;
+  const bool ckpt = dev.checkpointing != 0;   // PAPER.md:51, :251-253 (reading P12)
+  if (ckpt && (!(dev.recompute_fraction >= 0.0) || !(dev.act_keep_fraction >= 0.0) || !(dev.act_keep_fraction <= 1.0))) return false;
   const uint64_t zdp_share = (uint64_t)(((unsigned __int128)op.model_bytes * (uint64_t)z + (uint64_t)k - 1) / (uint64_t)k);
   const uint64_t model = (op.model_bytes - zdp_share) + ceil_div_u64(zdp_share, (uint64_t)dev.N);
-  if (persist)
-    *persist = model + (uint64_t)batch * op.act_bytes + op.extra_fixed + ceil_div_u64(op.extra_summed, (uint64_t)k);
+  uint64_t act = (uint64_t)batch * op.act_bytes;
+  if (ckpt) act = (uint64_t)std::ceil((double)act * dev.act_keep_fraction);   // only the checkpoints stay resident
+  if (persist) *persist = model + act + op.extra_fixed + ceil_div_u64(op.extra_summed, (uint64_t)k);
   if (transient) *transient = ceil_div_u64(op.extra_transient, (uint64_t)k);
   if (seconds) {
-    const double c = 2.0 + (double)z / (double)k;
-    *seconds = c * (double)(dev.N - 1) * (dev.alpha + op.S * dev.beta / (double)dev.N) +
-               (double)batch * op.gamma + (double)(k - 1) * op.delta;
+    // a ZDP slice: 3 collectives, 4 with checkpointing (one more gather round for the recomputation)
+    const double c = 2.0 + (ckpt ? 2.0 : 1.0) * (double)z / (double)k;
+    const double compute = (double)batch * op.gamma * (ckpt ? 1.0 + dev.recompute_fraction : 1.0);
+    *seconds = c * (double)(dev.N - 1) * (dev.alpha + op.S * dev.beta / (double)dev.N) + compute + (double)(k - 1) * op.delta;
   }
   return true;
 }

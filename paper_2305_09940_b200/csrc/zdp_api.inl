@@ -67,7 +67,7 @@ ZdpBuf zdp_buf(const ZdpGeom& g, size_t e) {
   return b;
 }
 struct ZdpWs {
-  size_t gbuf[2], b2g, rbuf[2], db2s, zs, hs, acc, scratch, total;
+  size_t gbuf[2], b2g, rbuf[2], db2s, zs, hs, acc, scratch1, scratch2, total;
 };
 ZdpWs zdp_ws(const ZdpGeom& g, int pass) {
   ZdpWs w = {};
@@ -88,7 +88,8 @@ ZdpWs zdp_ws(const ZdpGeom& g, int pass) {
     w.zs = off; off += slice_buf;
     w.hs = off; off += slice_buf;
     w.acc = off; off += acc;
-    w.scratch = off; off += align_up((size_t)kReduceRowChunks * (size_t)(g.h + g.f) * 4, 256);
+    w.scratch1 = off; off += db1_scratch_bytes(g.T, g.fs_max());
+    w.scratch2 = off; off += db2_scratch_bytes(g.h);
   }
   w.total = off;
   return w;
@@ -215,8 +216,9 @@ int osdp_zdp_ffn_split_mlp_op_cost(const osdp_zdp_desc* desc, int pass, osdp_op_
   // sliceable: two gathered parameter slices, in the backward also two fp32 gradient staging slices, and
   // the slice activations, all proportional to the slice width
   const uint64_t slice_params = 2 * h * f + f;
-  c.extra_transient = 2 * slice_params * e + (pass == OSDP_BWD ? 2 * slice_params * 4 : 0) + (pass == OSDP_FWD ? 1 : 2) * T * f * e;
-  c.extra_fixed = align_up((size_t)T * h * 4, 256) + (pass == OSDP_BWD ? reduce_scratch_bytes(&desc->mlp) + h * 4 : h * e);
+  c.extra_transient = 2 * slice_params * e + (pass == OSDP_BWD ? 2 * slice_params * 4 + db1_scratch_bytes(T, f) : 0) +
+                      (pass == OSDP_FWD ? 1 : 2) * T * f * e;
+  c.extra_fixed = align_up((size_t)T * h * 4, 256) + (pass == OSDP_BWD ? db2_scratch_bytes(h) + h * 4 : h * e);
   *out = c;
   return OSDP_OK;
 }
@@ -329,8 +331,8 @@ int osdp_zdp_ffn_split_mlp_backward(const osdp_zdp_desc* desc, const void* param
       const FfnSliceW sw = {G + gb.w1, fs, G + gb.b1, G + gb.w2};
       const FfnSliceG sg = {(float*)(R + rb.w1), fs, (float*)(R + rb.b1), (float*)(R + rb.w2)};
       OSDP_TRY(ffn_slice_backward(g.dt, g.T, g.h, fs, X, dY, sw, sg, ws + w.zs, ws + w.hs, dX, (float*)(ws + w.acc),
-                                  (float*)(ws + w.scratch), stp.slice == 0 ? (float*)(ws + w.db2s) : nullptr, g.k == 1,
-                                  stp.slice == 0, cs));
+                                  (float*)(ws + w.scratch1), (float*)(ws + w.scratch2),
+                                  stp.slice == 0 ? (float*)(ws + w.db2s) : nullptr, g.k == 1, stp.slice == 0, cs));
       if (two) {
         OSDP_CUDA_TRY(cudaEventRecord(ev->freed[b], cs));
         OSDP_CUDA_TRY(cudaEventRecord(ev->grads[b], cs));

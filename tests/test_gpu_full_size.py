@@ -18,22 +18,29 @@ def rel(got, ref):
     return float(np.max(np.abs(got - ref))) / (s if s > 0 else 1.0)
 
 
-def sample_indices(T, k, f, seed=0):
+def sample_indices(T, k, f, seed=0, every_tile=False):
     rng = np.random.default_rng(seed)
     b = O.slice_bounds(T, k)
     rows = {0, T - 1, b[0][1] - 1, b[-1][0], b[k // 2][0], b[k // 2][1] - 1}       # first/last rows of slices
     rows |= set(int(r) for r in rng.integers(0, T, 6))
     cols = {0, f - 1, 255, 256} | set(int(c) for c in rng.integers(0, f, 4))         # across n-tile edges
+    if every_tile:
+        # one token row in every 512-row block (every m-tile of the token-major GEMMs A1-A4, A7, whichever slice and wave
+        # it falls in) and one ffn column in every 256-column block (every n-tile of A1/A3/A4, every m-tile of dW2 = A5
+        # and every n-tile of dW1 = A6); a sampled row covers all of Y / dX along hidden, a sampled column all of
+        # dW2[j, :] and dW1[:, j], so every output tile of every GEMM of every wave has a checked element
+        rows |= {min(T - 1, r0 + int(rng.integers(0, 512))) for r0 in range(0, T, 512)}
+        cols |= {min(f - 1, c0 + int(rng.integers(0, 256))) for c0 in range(0, f, 256)}
     return sorted(rows), sorted(cols)
 
 
-def check_sampled(lib, inp, x64, ks, what, refs=None, axis="tokens"):
+def check_sampled(lib, inp, x64, ks, what, refs=None, axis="tokens", every_tile=False):
     T, h = inp.X.shape
     f = inp.W1.shape[1]
     d = inp.to("cuda")
     cache = {}
     for k in ks:
-        rows, cols = sample_indices(T, k, f)
+        rows, cols = sample_indices(T, k, f, every_tile=every_tile)
         if axis == "ffn":      # first/last columns of ffn slices as well
             fb = O.ffn_slice_bounds(f, k, 8)
             cols = sorted(set(cols) | {fb[0][1] - 1, fb[-1][0], fb[k // 2][0], fb[k // 2][1] - 1})
@@ -64,13 +71,13 @@ def check_sampled(lib, inp, x64, ks, what, refs=None, axis="tokens"):
 def test_c3_sampled_oracle_k_1_4_16(lib):
     c = I.CONFIGS["C3"]
     inp = I.mlp_inputs(c["tokens"], c["hidden"], c["ffn"], torch.bfloat16, seed=c["seed"])
-    check_sampled(lib, inp, inp.as_f64(), c["ks"], "C3")
+    check_sampled(lib, inp, inp.as_f64(), c["ks"], "C3", every_tile=True)
 
 
 def test_c4_sampled_oracle_bench_config_and_extremes(lib):
     c = I.CONFIGS["C4"]
     inp = I.mlp_inputs(c["tokens"], c["hidden"], c["ffn"], torch.bfloat16, seed=c["seed"])
-    check_sampled(lib, inp, inp.as_f64(), (4, 1, 32), "C4")          # k = 4 is what bench.py times
+    check_sampled(lib, inp, inp.as_f64(), (4, 1, 32), "C4", every_tile=True)          # k = 4 is what bench.py times
 
 
 def test_c4_ffn_split_sampled_oracle(lib):
@@ -91,25 +98,30 @@ def test_large_token_count_offsets_beyond_2_gib(lib):
     check_sampled(lib, inp, x64, (2,), "2^30-element intermediate, ffn split", axis="ffn")
 
 
-def test_c4_token_downscaled_full_oracle(lib):
-    """Full oracle on a token-downscaled copy (T/8) of the largest config: every output element checked."""
-    c = I.CONFIGS["C4"]
+@pytest.mark.parametrize("cfg,k", [("C4", 4), ("C3", 4), ("C5", 2)])
+def test_token_downscaled_full_oracle(lib, cfg, k):
+    """Full oracle on a token-downscaled copy (T/8) of each large config: every output element
+    checked, for the token split and the ffn-axis split."""
+    c = I.CONFIGS[cfg]
     T = c["tokens"] // 8
     inp = I.mlp_inputs(T, c["hidden"], c["ffn"], torch.bfloat16, seed=3)
     ref = O.mlp_forward_backward(**inp.as_f64())
     d = inp.to("cuda")
-    op = lib.SplitMlp(T, c["hidden"], c["ffn"], torch.bfloat16, 4)
-    out = {"Y": op.forward(d.X, d.W1, d.b1, d.W2, d.b2)}
-    out.update(op.backward(d.X, d.W1, d.b1, d.W2, d.dY))
-    torch.cuda.synchronize()
-    errs = {n: rel(out[n].double().cpu().numpy(), ref[n]) for n in ref}
-    assert all(e <= TOL for e in errs.values()), errs
+    for axis in ("tokens", "ffn"):
+        op = lib.SplitMlp(T, c["hidden"], c["ffn"], torch.bfloat16, k, axis=axis)
+        out = {"Y": op.forward(d.X, d.W1, d.b1, d.W2, d.b2)}
+        out.update(op.backward(d.X, d.W1, d.b1, d.W2, d.dY))
+        torch.cuda.synchronize()
+        errs = {n: rel(out[n].double().cpu().numpy(), ref[n]) for n in ref}
+        assert all(e <= TOL for e in errs.values()), (cfg, axis, errs)
+        del op, out
+        torch.cuda.empty_cache()
 
 
 def test_c5_stack_planned_k_teacher_forced(lib):
     """24-layer chain, per-layer k from osdp_plan under the 24 GiB activation cap (pure-sum accounting at
     8 B per T x f element, SURVEY.md §8 note), forward through all layers then backward; parity per layer,
-    teacher-forced on the GPU's own bf16 X_l and dY_l (reading S13), on sampled outputs for 3 layers."""
+    teacher-forced on the GPU's own bf16 X_l and dY_l (reading S13), on sampled outputs of ALL 24 layers."""
     c = I.CONFIGS["C5"]
     T, h, f, L = c["tokens"], c["hidden"], c["ffn"], c["layers"]
     desc1 = lib.make_desc(T, h, f, torch.bfloat16, 1)
@@ -146,7 +158,7 @@ def test_c5_stack_planned_k_teacher_forced(lib):
         W1, b1, W2, b2 = dev_w[l]
         Xs.append(opsl[l].forward(Xs[l], W1, b1, W2, b2))
     dY = dYL.cuda()
-    checked = {0, L // 2, L - 1}
+    checked = set(range(L))
     rows, cols = sample_indices(T, 4, f, seed=5)
     ri, ci = torch.tensor(rows, device="cuda"), torch.tensor(cols, device="cuda")
     for l in reversed(range(L)):
@@ -197,6 +209,7 @@ def test_ffn_split_peak_bytes_within_5pct_of_cost_model(lib, cfg, ks):
             fs = -(-(f // 8) // k) * 8
             bufs = (2 if name == "bwd" else 1) * ((T * fs * 2 + 255) // 256 * 256)
             acc = 0 if k == 1 else (T * h * 4 + 255) // 256 * 256
-            scratch = P.mlp_reduce_scratch_bytes(h, f) if name == "bwd" else 0
+            # db1 band partials of one slice (all T rows x the widest ffn slice) + db2 partials
+            scratch = P.mlp_reduce_scratch_bytes(T, h, fs) if name == "bwd" else 0
             assert pk[name]["workspace"] == bufs + acc + scratch
 

@@ -136,8 +136,9 @@ def test_bf16_tile_shapes_and_wave_sync_agree_bitwise(lib, force_big_tiles):
     T, h, f = 5200, 1288, 5144
     inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=10)
     outs = []
-    for min_k, sync, band, cluster in ((1, 1, 32, 0), (1, 0, 32, 0), (1, 4, 32, 0), (1, 1, 1, 0), (1 << 40, 1, 32, 0),
+    for min_k, sync, band, cluster in ((1, 1, 0, 0), (1, 0, 32, 0), (1, 4, 32, 0), (1, 1, 1, 0), (1 << 40, 1, 0, 0),
                                        (1, 1, 32, 1), (1 << 40, 1, 32, 1)):        # last two: 4-CTA multicast clusters
+        # band 0 = the default square-wave raster, > 0 = round 1's L2-budget bands
         lib.osdp_set_tuning(lib.OSDP_TUNE_MT2_MIN_K, min_k)
         lib.osdp_set_tuning(lib.OSDP_TUNE_WAVE_SYNC, sync)
         lib.osdp_set_tuning(lib.OSDP_TUNE_BAND_MIB, band)
@@ -209,8 +210,10 @@ def test_trace_records_every_launch_with_its_step(lib):
     """osdp_trace_*: one (step id, milliseconds) entry per kernel launch, in launch order, both split axes."""
     T, h, f, k = 600, 128, 512, 3
     d = I.mlp_inputs(T, h, f, torch.bfloat16, seed=17).to("cuda")
-    for axis, fwd_steps, bwd_steps in (("tokens", [1, 2] * k, [3, 4, 5, 8, 8, 6, 7] * k),
-                                       ("ffn", [1, 2] * k + [10], [3, 4, 5, 8, 8, 6, 7] * k + [10])):
+    # step 8 = column sums: db2 takes two launches once per call (partials of dY, fixed-order sum); db1 one per slice
+    # (the band partials come out of the A4 epilogue, only their fixed-order sum is a launch)
+    for axis, fwd_steps, bwd_steps in (("tokens", [1, 2] * k, [8, 8] + [3, 4, 5, 8, 6, 7] * k),
+                                       ("ffn", [1, 2] * k + [10], [3, 4, 5, 8, 8, 8, 6, 7] + [3, 4, 5, 8, 6, 7] * (k - 1) + [10])):
         op = lib.SplitMlp(T, h, f, torch.bfloat16, k, axis=axis)
         op.forward(d.X, d.W1, d.b1, d.W2, d.b2)                      # warm-up, untraced
         lib.osdp_trace_enable(True)
@@ -231,7 +234,7 @@ def test_tuning_rejects_bad_arguments(lib):
     assert lib.osdp_set_tuning(99, 1, check=False) == lib.OSDP_ERR_ARG
     assert lib.osdp_set_tuning(lib.OSDP_TUNE_WAVE_SYNC, -1, check=False) == lib.OSDP_ERR_ARG
     assert lib.osdp_set_tuning(lib.OSDP_TUNE_MT2_MIN_K, 0, check=False) == lib.OSDP_ERR_ARG
-    assert lib.osdp_set_tuning(lib.OSDP_TUNE_BAND_MIB, 0, check=False) == lib.OSDP_ERR_ARG
+    assert lib.osdp_set_tuning(lib.OSDP_TUNE_BAND_MIB, -1, check=False) == lib.OSDP_ERR_ARG
     assert lib.osdp_get_tuning(99) == -1
     assert lib.osdp_get_tuning(lib.OSDP_TUNE_MT2_MIN_K) == 4096 and lib.osdp_get_tuning(lib.OSDP_TUNE_WAVE_SYNC) == 1
 
@@ -301,7 +304,8 @@ def test_ffn_split_error_codes_and_workspace(lib):
     inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=1).to("cuda")
     desc = lib.make_desc(T, h, f, torch.bfloat16, 4)
     fwd, bwd = (lib.osdp_ffn_split_mlp_workspace_bytes(desc, p) for p in (lib.OSDP_FWD, lib.OSDP_BWD))
-    assert fwd == T * 32 * 2 + T * h * 4 and bwd == 2 * T * 32 * 2 + T * h * 4 + 32 * (h + f) * 4
+    # bwd: two slice buffers, the fp32 dX accumulator, db1 band partials (T / 32 rows x 32 columns) and db2 partials (32 x h)
+    assert fwd == T * 32 * 2 + T * h * 4 and bwd == 2 * T * 32 * 2 + T * h * 4 + (T // 32) * 32 * 4 + 32 * h * 4
     assert lib.osdp_ffn_split_mlp_workspace_bytes(lib.make_desc(T, h, f, torch.bfloat16, 1), lib.OSDP_FWD) == T * f * 2
     assert lib.osdp_ffn_split_mlp_workspace_bytes(lib.make_desc(T, h, f, torch.bfloat16, f // 8 + 1), lib.OSDP_FWD) == 0
     ws = torch.empty(bwd, dtype=torch.uint8, device="cuda")
@@ -380,7 +384,7 @@ def test_backward_overwrites_and_accepts_null_b2(lib):
     torch.cuda.synchronize()
     for n in ("dX", "dW1", "db1", "dW2", "db2"):
         assert rel_err(out[n].double().cpu().numpy(), ref[n]) <= 2e-2, n
-    assert lib.osdp_last_launch_count() == 3 * 7          # k slices x (5 GEMMs + 2 reduction kernels for db1 and db2)
+    assert lib.osdp_last_launch_count() == 2 + 3 * 6      # db2 (2 launches per call) + k slices x (5 GEMMs + the db1 sum)
 
 
 def test_runs_on_a_side_stream(lib):

@@ -197,15 +197,17 @@ def _golden_peak_rows():
 
 def test_oracle_byte_calculators_reproduce_the_worked_peak_bytes():
     """mlp_persistent_bytes + mlp_workspace_bytes against the figures SURVEY.md section 8(d) works out by hand (MiB;
-    tests/golden/peak_bytes_mib.txt).  The printed figures leave out the bias vectors and the fixed column-sum scratch:
-    the scratch is stated separately (REDUCE_ROW_CHUNKS x (h + f) fp32 partial sums) and the biases
-    are (f + h) e bytes forward, (f + h)(e + 4) backward (db1, db2 are fp32)."""
+    tests/golden/peak_bytes_mib.txt).  The printed figures leave out the bias vectors and the column-sum scratch:
+    the scratch is stated separately (one fp32 partial row of f columns per 32-row band of the slice for db1, 32 partial
+    rows of h columns for db2) and the biases are (f + h) e bytes forward, (f + h)(e + 4) backward
+    (db1, db2 are fp32)."""
     rows = _golden_peak_rows()
     assert len(rows) == 9
     MiB = 1 << 20
     for c, T, h, f, e, k, fwd, bwd in rows:
-        scratch = P.mlp_reduce_scratch_bytes(h, f)
-        assert scratch == -(-32 * (h + f) * 4 // 256) * 256
+        Ts = -(-T // k)
+        scratch = P.mlp_reduce_scratch_bytes(Ts, h, f)
+        assert scratch == -(-(-(-Ts // 32)) * f * 4 // 256) * 256 + -(-32 * h * 4 // 256) * 256
         got_f = P.mlp_persistent_bytes(T, h, f, e, False) + P.mlp_workspace_bytes(T, h, f, e, k, False)
         got_b = P.mlp_persistent_bytes(T, h, f, e, True) + P.mlp_workspace_bytes(T, h, f, e, k, True) - scratch
         assert got_f - (f + h) * e == fwd * MiB, (c, k)
@@ -213,10 +215,59 @@ def test_oracle_byte_calculators_reproduce_the_worked_peak_bytes():
     # size / slice_granularity: the workspace is the only term that moves with k
     for T, h, f, e in ((8192, 8192, 32768, 2), (512, 256, 1024, 4)):
         for bw in (False, True):
-            fixed = P.mlp_reduce_scratch_bytes(h, f) if bw else 0
+            fixed = -(-32 * h * 4 // 256) * 256 if bw else 0             # the db2 partials do not depend on k
             w1 = P.mlp_workspace_bytes(T, h, f, e, 1, bw) - fixed
             for k in (2, 4, 8):
                 assert (P.mlp_workspace_bytes(T, h, f, e, k, bw) - fixed) * k == w1
+
+
+def test_oracle_checkpointing_interplay_closed_forms():
+    """recomputation costs 'about 30% extra computation'; with ZeRO 'the recomputation process
+    before backward propagation requires an additional round of gathering' - a fourth collective for a ZDP operator,
+    while a DP operator keeps its two, so ZDP / DP communication becomes 4 / 2."""
+    op = P.OpCost(S=3.0e8, model=16 * 10 ** 9, act=1000, extra_fixed=77, gamma=0.25, delta=0.01)
+    for N in (2, 8, 64):
+        plain = P.Device(N=N, alpha=3e-5, beta=1.0 / 12e9)
+        ck = P.Device(N=N, alpha=3e-5, beta=1.0 / 12e9, checkpointing=True, recompute_fraction=0.3, act_keep_fraction=0.125)
+        comm = (N - 1) * (plain.alpha + op.S * plain.beta / N)
+        b = 4
+        pd, _, td = P.cost_eval(op, P.DP, 1, b, ck)
+        pz, _, tz = P.cost_eval(op, P.ZDP, 1, b, ck)
+        assert math.isclose(td, 2 * comm + 1.3 * b * op.gamma, rel_tol=1e-12)
+        assert math.isclose(tz, 4 * comm + 1.3 * b * op.gamma, rel_tol=1e-12)
+        assert math.isclose((tz - 1.3 * b * op.gamma) / (td - 1.3 * b * op.gamma), 2.0, rel_tol=1e-12)
+        assert pd == op.model + 500 + 77 and pz == -(-op.model // N) + 500 + 77     # 1/8 of 4 x 1000 bytes of activations kept
+        # the extra cost of turning an operator to ZDP doubles (2 comm instead of 1): OSDP keeps more operators in DP
+        assert math.isclose(tz - td, 2 * (P.cost_eval(op, P.ZDP, 1, b, plain)[2] - P.cost_eval(op, P.DP, 1, b, plain)[2]), rel_tol=1e-12)
+        # mixed slices interpolate: 4 slices with 1 in ZDP = (3 x 2 + 1 x 4) / 4 = 2.5 collectives
+        assert math.isclose(P.cost_eval_mixed(op, 4, 1, 0, ck)[2] - 3 * op.delta, 2.5 * comm, rel_tol=1e-12)
+    off = P.Device(N=8, alpha=1e-5, beta=1e-10, checkpointing=False, recompute_fraction=0.3, act_keep_fraction=0.1)
+    assert P.cost_eval(op, P.ZDP, 2, 3, off) == P.cost_eval(op, P.ZDP, 2, 3, P.Device(N=8, alpha=1e-5, beta=1e-10))
+
+
+def test_checkpointing_cost_model_and_plans_match_oracle(lib):
+    rng = random.Random(8)
+    for op in _ops(10, 6):
+        d = P.Device(N=rng.choice([2, 8]), alpha=rng.random() * 1e-3, beta=rng.random() * 1e-9, checkpointing=True,
+                     recompute_fraction=0.3, act_keep_fraction=rng.choice([0.0, 0.25, 1.0]))
+        for mode in (0, 1):
+            assert lib.osdp_cost_eval(_to_lib(lib, op), mode, 2, 3, _dev(lib, d)) == P.cost_eval(op, mode, 2, 3, d)
+        assert lib.osdp_cost_eval_mixed(_to_lib(lib, op), 4, 1, 3, _dev(lib, d)) == P.cost_eval_mixed(op, 4, 1, 3, d)
+    ops = _ops(4, 12)
+    base = dict(N=8, alpha=2e-4, beta=1e-9)
+    lo = P.plan_memory_time(ops, [1] * 4, [4] * 4, 1, P.Device(**base))[0]
+    hi = P.plan_memory_time(ops, [0] * 4, [1] * 4, 1, P.Device(**base))[0]
+    zdp_ops = {}
+    for ck in (False, True):
+        d = P.Device(mem_limit=(lo + 3 * hi) // 4, checkpointing=ck, recompute_fraction=0.3, act_keep_fraction=1.0, **base)
+        ref = P.plan_brute_force(ops, d, 1, [1, 4])
+        st, ks, modes, sec, peak = lib.osdp_plan([_to_lib(lib, o) for o in ops], _dev(lib, d), 1, [1, 4])
+        assert st == lib.OSDP_OK and (modes, ks, peak) == (ref[0], ref[1], ref[3]) and round(sec * 1e12) == ref[2]
+        zdp_ops[ck] = sum(modes)
+    assert zdp_ops[True] <= zdp_ops[False]          # ZDP got dearer: never more operators in ZDP at the same limit
+    bad = lib.osdp_device(2, 0.0, 0.0, 1 << 40, 1, 0.3, 1.5)
+    with pytest.raises(lib.OsdpError):
+        lib.osdp_cost_eval(_to_lib(lib, ops[0]), 0, 1, 1, bad)
 
 
 # ------------------------------------------------------------------ library == oracle
@@ -226,7 +277,8 @@ def _to_lib(lib, op):
 
 
 def _dev(lib, d):
-    return lib.osdp_device(d.N, d.alpha, d.beta, d.mem_limit)
+    return lib.osdp_device(d.N, d.alpha, d.beta, d.mem_limit, 1 if d.checkpointing else 0, d.recompute_fraction,
+                           d.act_keep_fraction)
 
 
 def test_library_exports_every_declared_symbol(lib):
@@ -424,13 +476,14 @@ def test_workspace_and_mlp_factors_match_cost_model(lib, T, h, f, dt, e):
             c = lib.osdp_mlp_op_cost(desc, pass_)
             assert c.model_bytes + c.act_bytes == P.mlp_persistent_bytes(T, h, f, e, bwd)
             assert c.act_bytes == (3 if bwd else 2) * T * h * e          # only the T x h tensors scale with the batch
-            assert c.extra_fixed == (P.mlp_reduce_scratch_bytes(h, f) if bwd else 0)
-            assert c.extra_transient == (2 if bwd else 1) * T * f * e
-            # cost model predicts the workspace: sliceable/k + fixed, up to 256 B padding per buffer and
-            # (ragged T/k) one extra row per buffer
+            assert c.extra_fixed == (-(-32 * h * 4 // 256) * 256 if bwd else 0)              # db2 partials
+            assert c.extra_transient == ((2 * T * f * e + T * f * 4 // 32) if bwd else T * f * e)   # slice buffers (+ db1 band partials)
+            # cost model predicts the workspace: sliceable/k + fixed, up to 256 B padding per buffer,
+            # (ragged T/k) one extra row per buffer and (T_s % 32) one extra band of partials
             pred = -(-c.extra_transient // k) + c.extra_fixed
-            slack = (2 if bwd else 1) * (256 + (f * e if T % k else 0))
-            assert 0 <= ws - pred <= slack
+            Ts = -(-T // k)
+            slack = (2 if bwd else 1) * (256 + (f * e if T % k else 0)) + (256 + f * 4 if bwd else 0)
+            assert 0 <= ws - pred <= slack, (ws, pred, slack)
 
 
 def test_mlp_factors_zdp_shards_only_the_model_states(lib):
