@@ -195,6 +195,12 @@ int db1_from_bands(int dtype, const void* dZs, int cols, float* out, int rows, f
   return launch_colsum<float>((const float*)dZs, cols, cols, out, rows, kBandRows, scratch, beta, st);
 }
 
+#define OSDP_TRY(expr)            \
+  do {                            \
+    int _rc = (expr);             \
+    if (_rc != OSDP_OK) return _rc; \
+  } while (0)
+
 // ---- helper streams: independent launches of one slice side by side ------------------------------------------
 // Once dZ_s exists, dW2 (+)= H_s^T dY_s, dW1 (+)= X_s^T dZ_s, dX_s = dZ_s W1^T and the two column sums are independent
 // (SURVEY.md section 7 "co-scheduling").  On small slices each of them fills a fraction of the machine for a few
@@ -243,11 +249,6 @@ int join_into(ForkCtx* c, cudaStream_t st) {
 }
 inline int64_t tiles_256(int64_t m, int64_t n) { return ((m + 255) / 256) * ((n + 255) / 256); }
 
-#define OSDP_TRY(expr)            \
-  do {                            \
-    int _rc = (expr);             \
-    if (_rc != OSDP_OK) return _rc; \
-  } while (0)
 
 // ---- one slice of the ffn-axis split.  The slice's weights are given by pointer + leading
 // dimension, so the same code serves weights sliced in place (W1 + lo, ld = f) and gathered slice buffers (ZDP, ld = fs).
@@ -285,29 +286,37 @@ int ffn_slice_forward(int dt, int64_t T, int64_t h, int fs, const void* X, const
 int ffn_slice_backward(int dt, int64_t T, int64_t h, int fs, const void* X, const void* dY, const FfnSliceW& w,
                        const FfnSliceG& g, void* Zs, void* Hs, void* dX, float* dXacc, float* scratch1, float* scratch2,
                        float* db2, bool single, bool first, cudaStream_t st) {
+  // dW2, dW1, dX (+)= and the column sums only need dZ_s: side by side on small slices (helper streams above)
+  const int64_t fork_max = sm100::tuning().fork_max_tiles.load();
+  const bool fork = fork_max > 0 && tiles_256(fs, h) <= fork_max && tiles_256(T, h) <= fork_max;
+  ForkCtx* fc = nullptr;
+  if (fork) OSDP_TRY(fork_ctx(&fc));
   trace_set_step(3);
   EpiParams e3 = {w.b1s, Zs, Hs, nullptr, fs, 0};
   OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_BIAS_GELU_DUAL>(dt, X, h, w.W1s, w.ldw1, GemmShape{(int)T, fs, (int)h}, e3, st)));
   trace_set_step(4);   // the epilogue also leaves the 32-row band sums of dZ_s in scratch1 (db1)
   EpiParams e4 = {nullptr, Zs, nullptr, Zs, fs, 0, scratch1, fs};
   OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_DGELU>(dt, dY, h, w.W2s, h, GemmShape{(int)T, fs, (int)h}, e4, st)));
+  if (fork) OSDP_TRY(fork_from(fc, st));
+  cudaStream_t s1 = fork ? fc->side[0] : st, s2 = fork ? fc->side[1] : st, s3 = fork ? fc->side[2] : st;
   trace_set_step(5);   // rows of dW2 belong to exactly one slice: written once, no accumulation
   EpiParams e5 = {nullptr, g.dW2s, nullptr, nullptr, h, 0};
   OSDP_TRY((gemm<MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32>(dt, Hs, fs, dY, h, GemmShape{fs, (int)h, (int)T}, e5, st)));
   trace_set_step(8);
-  OSDP_TRY(db1_from_bands(dt, Zs, fs, g.db1s, (int)T, scratch1, 0, st));
-  if (db2) OSDP_TRY(colsum_rows(dt, dY, (int)h, db2, (int)T, scratch2, 0, st));
+  OSDP_TRY(db1_from_bands(dt, Zs, fs, g.db1s, (int)T, scratch1, 0, s3));
+  if (db2) OSDP_TRY(colsum_rows(dt, dY, (int)h, db2, (int)T, scratch2, 0, s3));
   trace_set_step(6);   // columns of dW1 belong to exactly one slice
   EpiParams e6 = {nullptr, g.dW1s, nullptr, nullptr, g.ldg1, 0};
-  OSDP_TRY((gemm<MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32>(dt, X, h, Zs, fs, GemmShape{(int)h, fs, (int)T}, e6, st)));
+  OSDP_TRY((gemm<MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32>(dt, X, h, Zs, fs, GemmShape{(int)h, fs, (int)T}, e6, s1)));
   trace_set_step(7);   // the only result that spans slices
   if (single) {
     EpiParams e7 = {nullptr, dX, nullptr, nullptr, h, 0};
-    OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_PLAIN>(dt, Zs, fs, w.W1s, w.ldw1, GemmShape{(int)T, (int)h, fs}, e7, st)));
+    OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_PLAIN>(dt, Zs, fs, w.W1s, w.ldw1, GemmShape{(int)T, (int)h, fs}, e7, s2)));
   } else {
     EpiParams e7 = {nullptr, dXacc, nullptr, nullptr, h, first ? 0 : 1};
-    OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_ACCUM_F32>(dt, Zs, fs, w.W1s, w.ldw1, GemmShape{(int)T, (int)h, fs}, e7, st)));
+    OSDP_TRY((gemm<MAJOR_K, MAJOR_K, EPI_ACCUM_F32>(dt, Zs, fs, w.W1s, w.ldw1, GemmShape{(int)T, (int)h, fs}, e7, s2)));
   }
+  if (fork) OSDP_TRY(join_into(fc, st));   // the next slice overwrites Z_s / H_s
   return OSDP_OK;
 }
 
