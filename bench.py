@@ -612,6 +612,67 @@ def stack_bench(args, lib, cfg):
     return 0
 
 
+def zdp_bench(args, lib, cfg):
+    """ZDP mode with weight-slice gathering: every rank owns its token batch
+    and 1/N of the model states; each step = osdp_zdp_ffn_split_mlp_forward + backward with the slice all-gathers and
+    reduce-scatters (NCCL through torch.distributed) on a second stream beside the GEMMs.  Works at N = 1 (single-rank
+    NCCL group: the collectives are real but move nothing between GPUs); N > 1 has never been run (one-GPU lease).
+    One JSON line; `value` = executed TFLOP/s summed over ranks, max-over-ranks device time."""
+    import torch.distributed as dist
+    from paper_2305_09940_b200 import dist as D
+    from paper_2305_09940_b200 import inputs as I
+    world, rank, local = D.init("nccl")
+    if not dist.is_initialized():        # single process: a one-rank group so that the collectives are real NCCL calls
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29517")
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+    T, h, f, k = cfg["tokens"], cfg["hidden"], cfg["ffn"], args.zdp
+    dt = I.torch_dtype(cfg["dtype"])
+    whole = I.mlp_inputs(1, h, f, dt, seed=cfg["seed"])                  # the same weights on every rank
+    mine = I.mlp_inputs(T, h, 8, dt, seed=D.rank_seed(cfg["seed"], rank) + 1000)   # this rank's tokens (X, dY)
+    desc = lib.make_zdp_desc(T, h, f, dt, k, world, rank)
+    shard = lib.zdp_shard(desc, whole.W1, whole.b1, whole.W2, whole.b2).cuda()
+    X, dY = mine.X.cuda(), mine.dY.cuda()
+    Y, dX = torch.empty_like(X), torch.empty_like(X)
+    gshard = torch.empty(shard.numel(), dtype=torch.float32, device="cuda")
+    ws = torch.empty(max(lib.osdp_zdp_ffn_split_mlp_workspace_bytes(desc, p) for p in (lib.OSDP_FWD, lib.OSDP_BWD)),
+                     dtype=torch.uint8, device="cuda")
+    comm, cs = lib.TorchDistComm(), torch.cuda.Stream()
+    launches = [0]
+
+    def step():
+        lib.osdp_zdp_ffn_split_mlp_forward(desc, shard, X, Y, ws, comm=comm, comm_stream=cs)
+        n = lib.osdp_last_launch_count()
+        lib.osdp_zdp_ffn_split_mlp_backward(desc, shard, X, dY, dX, gshard, ws, comm=comm, comm_stream=cs)
+        launches[0] = n + lib.osdp_last_launch_count()
+
+    for _ in range(args.warmup):
+        step()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ms_sum, _ = timed_steps(step, args.steps, world, None)
+    clocks = sampler.stop()
+    ms = max_over_ranks(ms_sum / args.steps, world)
+    flops = executed_flops(T, h, f)
+    e = 2 if cfg["dtype"] == "bf16" else 4
+    S = (2 * h * f + f + h) * e
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": world * flops / (ms * 1e-3) / 1e12, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": cfg["dtype"], "data": "synthetic",
+            "config": {"workload": f"{args.config}: ZDP ffn-split MLP tokens/GPU={T} hidden={h} ffn={f}, k={k} ffn slices, "
+                                   f"model states sharded over {world} ranks, slice gathers / reduce-scatters on a second stream",
+                       "parallelism": f"zdp{world}", "collective_bytes_per_rank_per_step":
+                           {"all_gather_contributed": (2 * S - h * e) // world, "reduce_scatter_contributed": (S // e) * 4 // world},
+                       "workspace_bytes": int(ws.numel()), "param_shard_bytes": int(shard.numel() * e)},
+            "clocks": clocks, "gpu_launches": launches[0] * args.steps,
+            "note": "N > 1 has not been run on hardware by the builder (one-GPU lease); at N = 1 the NCCL collectives are "
+                    "single-rank copies"}), flush=True)
+    D.finalize()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -633,6 +694,9 @@ def main():
                          "hidden sizes (ffn = 4 hidden, --sweep-tokens tokens), both split axes - the shape of the "
                          "paper's operator-splitting experiment (PAPER.md:231-247, Fig. 7)")
     ap.add_argument("--sweep-tokens", type=int, default=8192)
+    ap.add_argument("--zdp", type=int, default=0, metavar="K",
+                    help="instead of the bench line: ZDP mode with weight-slice gathering over the ranks torchrun started "
+                         "(or one rank), K ffn slices (osdp_zdp_ffn_split_mlp_*, DESIGN.md section 11)")
     ap.add_argument("--stack", action="store_true",
                     help="with --config C5: instead of the bench line, run the 24-layer MLP stack with the split count "
                          "per layer chosen by osdp_plan from gamma/delta calibrated on this GPU (BASELINE.json config 5)")
@@ -654,6 +718,8 @@ def main():
         return granularity_sweep(args, lib)
     if args.stack:
         return stack_bench(args, lib, cfg)
+    if args.zdp:
+        return zdp_bench(args, lib, cfg)
     from paper_2305_09940_b200 import dist as D
     world, rank, local = D.init("nccl")
     peaks = load_peaks()
