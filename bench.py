@@ -393,6 +393,7 @@ def measure_peak_bytes(lib, cfg, k, axis="tokens"):
         torch.cuda.synchronize()
         torch.cuda.empty_cache()
         base = torch.cuda.memory_allocated()
+        free0, _ = torch.cuda.mem_get_info()            # the device's own view (cudaMemGetInfo), not the allocator's
         torch.cuda.reset_peak_memory_stats()
         desc = lib.make_desc(T, h, f, dt, k)
         mk = lambda *s, d=dt: torch.empty(s, dtype=d, device="cuda")
@@ -414,13 +415,15 @@ def measure_peak_bytes(lib, cfg, k, axis="tokens"):
                 desc, X, W1, b1, W2, b2, dY, dX, dW1, db1, dW2, db2, ws)
         torch.cuda.synchronize()
         measured = torch.cuda.max_memory_allocated() - base
+        free1, _ = torch.cuda.mem_get_info()            # all call tensors still alive here: used-memory delta of the device
         c = (lib.osdp_ffn_split_mlp_op_cost if ffn else lib.osdp_mlp_op_cost)(desc, pass_)
         dev = lib.osdp_device(1, 0.0, 0.0, 1 << 62)
         p, tr, _ = lib.osdp_cost_eval(c, lib.OSDP_DP, k, 1, dev)
         model = int(p + tr)
         if ffn and k == 1:       # the variant's cost factors describe k > 1; at k = 1 there is no fp32 accumulator
             model -= (T * h * 4 + 255) // 256 * 256
-        out[name] = {"measured": int(measured), "model": model, "workspace": int(ws.numel())}
+        out[name] = {"measured": int(measured), "model": model, "workspace": int(ws.numel()),
+                     "device_used_delta": int(free0 - free1)}   # >= measured by the allocator's 2 MiB segment rounding; the library allocates nothing itself
         del X, W1, b1, W2, b2, ws
         if pass_ == lib.OSDP_FWD:
             del Y
@@ -791,9 +794,19 @@ def main():
         elif tj.get(key) is not None:
             traffic = tj.get(key)
             traffic_detail = {"source": tj.get("source")}
+    operand_path = None
+    if os.path.exists(tpath) and args.axis == "tokens":
+        l2b = json.load(open(tpath)).get(f"{args.config}:k{args.k}:A{dom}:l2_to_sm")
+        if l2b and clocks.get("sm_mhz"):
+            # what actually binds the 256 x 256-tile dW GEMMs: operand delivery L2 -> SM, whose
+            # measured chip-wide ceiling is about 6300 B/clk (B300_MICROARCH.md "LTS throughput cap")
+            bpc = l2b / (dom_avg * 1e-3 * clocks["sm_mhz"] * 1e6)
+            operand_path = {"l2_to_sm_bytes_per_launch": l2b, "achieved_B_per_clk": bpc, "ceiling_B_per_clk": 6300.0,
+                            "frac": bpc / 6300.0, "clock_mhz": clocks["sm_mhz"],
+                            "how": "ncu lts__t_sectors_srcunit_tex_op_read x 32 B (profiles/r02_ncu_full.md) / (avg launch ms x SM clock sampled in this run)"}
     roofline = {"bound": "tensor", "kernel": f"gemm_bf16_sm100_kernel [{lib.osdp_step_name(dom)}]",
                 "achieved": achieved, "peak": peak, "unit": UNIT, "frac": (achieved / peak) if peak else None,
-                "traffic": traffic, "traffic_detail": traffic_detail, "peak_source": f"{peaks['source']} (bf16_tflops_sustained: kernel timed inside a long step)",
+                "traffic": traffic, "traffic_detail": traffic_detail, "operand_path": operand_path, "peak_source": f"{peaks['source']} (bf16_tflops_sustained: kernel timed inside a long step)",
                 "frac_of_burst": achieved / peaks["bf16_tflops"], "frac_of_nominal": achieved / NOMINAL_BF16_TFLOPS,
                 "flops_per_launch": gemm_flops, "avg_launch_ms": dom_avg,
                 "how": "per-launch CUDA events recorded by the library on the call's stream over K traced steps"}
