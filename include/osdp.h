@@ -203,12 +203,19 @@ typedef enum osdp_tune_key {
   OSDP_TUNE_BAND_MIB = 3,       /* default 0 */
   OSDP_TUNE_CLUSTER_MIN_TILES = 4, /* default 0 (multicast clusters off) */
   OSDP_TUNE_MT2_MIN_K_ACC = 5,     /* OSDP_TUNE_MT2_MIN_K for the fp32-accumulate launches (dW GEMMs, K = slice rows) */
-  OSDP_TUNE_FORK_MAX_TILES = 6     /* default 256: in the token-split backward, the launches that only depend on dZ_s
+  OSDP_TUNE_FORK_MAX_TILES = 6,    /* default 256: in the token-split backward, the launches that only depend on dZ_s
                                       (dW2, dW1, dX, column sums) are enqueued side by side on helper streams that fork
                                       from and join `stream` when each GEMM has at most this many 256 x 256 output tiles
                                       (small slices: every launch is a wave or two; measured +4-8 % at C2, +5 % at the
                                       C5 layer shape, neutral to -1 % at C3 / C4, which the default excludes); 0 = always
                                       in sequence */
+  OSDP_TUNE_SLICE_KERNEL_MAX_TILES = 7
+                                   /* token split, bf16: when every GEMM of a slice has at most this many 256 x 256
+                                      output tiles, the whole slice runs as ONE persistent kernel (forward A1 -> A2;
+                                      backward A3 -> A4 -> A7 | A5 | A6 and the db1 sum): CTA pairs claim tiles of all
+                                      GEMMs from one list and a tile waits only for the producer tiles it reads
+                                      (csrc/slice_sm100.cuh).  Results are bit-identical to the
+                                      launch-per-GEMM path.  0 = never */
 } osdp_tune_key;
 int osdp_set_tuning(int key, int64_t value);
 int64_t osdp_get_tuning(int key);

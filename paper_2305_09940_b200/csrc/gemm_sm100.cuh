@@ -55,6 +55,7 @@ struct Tuning {
   std::atomic<int64_t> band_mib{0};         // 0: square-wave raster bands; > 0: band = tile rows whose A rows fit this many MiB of L2
   std::atomic<int64_t> cluster_min_tiles{0};   // > 0: multicast clusters for launches of at least this many pair tiles
   std::atomic<int64_t> fork_max_tiles{256};    // backward: A5 | A6 | A7 | column sums run concurrently when each GEMM has at most this many 256 x 256 tiles
+  std::atomic<int64_t> slice_kernel_max_tiles{0};   // token split: one persistent kernel per slice (slice_sm100.cuh) when every GEMM of the slice has at most this many 256 x 256 tiles; 0 = never
 };
 inline Tuning& tuning() {
   static Tuning t;
@@ -656,6 +657,10 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
       mbar_wait(tfull_bar + 8 * as, aphase);
       tc_fence_after();
       bool released = false;   // the accumulator stage goes back to the MMA warp right after this warp's last tcgen05.ld
+      // ... if a later tile of this cluster will wait for it.  A hand-back that nobody consumes is a remote arrive that
+      // may still be in flight when the leader CTA has exited (the teardown rendezvous is relaxed): it would then land
+      // in the barriers of the NEXT kernel's CTA on that SM as a spurious arrival (seen in slice_sm100.cuh).
+      const bool hand_back = t + kAccStages * num_clusters < num_tiles;
 #pragma unroll 1
       for (int h = 0; h < MT; ++h) {
         const int row0 = (tc.m_blk * CM + pi) * kPairM + (int)rank * kCtaM + h * BLOCK_M + q * 32;   // this warp's 32-row band
@@ -682,7 +687,7 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
           if (h == MT - 1 && n + 2 * kChunk >= n_end) {   // this warp's last read of the accumulator stage
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(tempty_leader + 8 * as);
+            if (lane == 0 && hand_back) mbar_arrive_cluster(tempty_leader + 8 * as);
             released = true;
           }
           [[maybe_unused]] const uint32_t bias_cur = (n - n0) >= 2 * kChunk ? bias_reg[1] : bias_reg[0];
@@ -749,7 +754,7 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
       if (!released) {
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive_cluster(tempty_leader + 8 * as);
+        if (lane == 0 && hand_back) mbar_arrive_cluster(tempty_leader + 8 * as);
       }
     }
     if (lane == 0) bulk_wait<0>();   // all of this warp's stores have completed before the CTA's smem goes away

@@ -12,6 +12,7 @@
 #include "gemm_f32.cuh"
 #include "gemm_sm100.cuh"
 #include "reduce.cuh"
+#include "slice_sm100.cuh"
 
 namespace osdp {
 
@@ -250,6 +251,34 @@ int join_into(ForkCtx* c, cudaStream_t st) {
 inline int64_t tiles_256(int64_t m, int64_t n) { return ((m + 255) / 256) * ((n + 255) / 256); }
 
 
+// ---- one persistent kernel per slice (slice_sm100.cuh) ----------------------------------------------------------
+// Taken for bf16 when every GEMM of a slice has at most OSDP_TUNE_SLICE_KERNEL_MAX_TILES tiles of 256 x 256 and the
+// call's completion counters fit the per-call block.  A2 / A7 (long contraction, few output tiles) take 128-column
+// tiles when that still fits one wave of CTA pairs, so they spread over twice as many SMs.
+struct SlicePlan {
+  bool use = false;
+  int bn_narrow = 256;   // tile width of A2 / A7
+  int words_per_slice = 0, words = 0;
+};
+int slice_plan(const osdp_mlp_desc* d, int pass, SlicePlan* out) {
+  *out = SlicePlan{};
+  const int64_t max_tiles = sm100::tuning().slice_kernel_max_tiles.load();
+  if (d->dtype != OSDP_BF16 || max_tiles <= 0) return OSDP_OK;
+  sm100::DeviceInfo dev;
+  OSDP_TRY(sm100::current_device(&dev));
+  const int64_t ts = (d->tokens + d->k - 1) / d->k;
+  const int64_t t_tf = tiles_256(ts, d->ffn), t_th = tiles_256(ts, d->hidden), t_fh = tiles_256(d->ffn, d->hidden);
+  if (t_tf > max_tiles || t_th > max_tiles || t_fh > max_tiles) return OSDP_OK;
+  out->bn_narrow = 2 * t_th <= dev.sms / 2 ? 128 : 256;
+  const int64_t t_narrow = ((ts + 255) / 256) * ((d->hidden + out->bn_narrow - 1) / out->bn_narrow);
+  const int64_t per_slice = sm100::kSliceFlags0 + 2 * (pass == OSDP_FWD ? t_tf + t_narrow : 2 * t_tf + t_narrow + 2 * t_fh);
+  if (per_slice * d->k > sm100::kSliceSyncWords) return OSDP_OK;
+  out->use = true;
+  out->words_per_slice = (int)per_slice;
+  out->words = (int)(per_slice * d->k);
+  return OSDP_OK;
+}
+
 // ---- one slice of the ffn-axis split.  The slice's weights are given by pointer + leading
 // dimension, so the same code serves weights sliced in place (W1 + lo, ld = f) and gathered slice buffers (ZDP, ld = fs).
 struct FfnSliceW {
@@ -380,6 +409,10 @@ int osdp_set_tuning(int key, int64_t value) {
       if (value < 0) return OSDP_ERR_ARG;
       t.fork_max_tiles = value;
       return OSDP_OK;
+    case OSDP_TUNE_SLICE_KERNEL_MAX_TILES:
+      if (value < 0) return OSDP_ERR_ARG;
+      t.slice_kernel_max_tiles = value;
+      return OSDP_OK;
     default: return OSDP_ERR_ARG;
   }
 }
@@ -394,6 +427,7 @@ int64_t osdp_get_tuning(int key) {
     case OSDP_TUNE_CLUSTER_MIN_TILES: return t.cluster_min_tiles;
     case OSDP_TUNE_MT2_MIN_K_ACC: return t.mt2_min_k_acc;
     case OSDP_TUNE_FORK_MAX_TILES: return t.fork_max_tiles;
+    case OSDP_TUNE_SLICE_KERNEL_MAX_TILES: return t.slice_kernel_max_tiles;
     default: return -1;
   }
 }
@@ -438,6 +472,8 @@ const char* osdp_step_name(int step_id) {
     case 11: return "Linear fwd Y = X W + b";
     case 12: return "Linear bwd dX = dY W^T";
     case 13: return "Linear bwd dW += X^T dY";
+    case 21: return "slice kernel fwd (A1 -> A2 in one launch)";
+    case 22: return "slice kernel bwd (A3 -> A4 -> A7 | A5 | A6 + db1 in one launch)";
     default: return "unknown";
   }
 }
@@ -487,12 +523,28 @@ int osdp_split_mlp_forward(const osdp_mlp_desc* desc, const void* X, const void*
   const int dt = desc->dtype;
   void* Hs = workspace;
 
+  SlicePlan sp;
+  OSDP_TRY(slice_plan(desc, OSDP_FWD, &sp));
+  unsigned int* sync = nullptr;
+  unsigned int epoch0 = 0;
+  if (sp.use) OSDP_TRY(sm100::slice_sync_acquire(sp.words, desc->k, &sync, &epoch0));
+
   for (int s = 0; s < desc->k; ++s) {
     const int64_t lo = (int64_t)s * T / desc->k, hi = (int64_t)(s + 1) * T / desc->k;
     const int Ts = (int)(hi - lo);
     if (Ts == 0) continue;
     const char* Xs = (const char*)X + (size_t)lo * h * e;
     char* Ys = (char*)Y + (size_t)lo * h * e;
+    if (sp.use) {   // A1 -> A2 in one launch: an A2 tile starts when its 256 rows of H_s are complete
+      trace_set_step(21);
+      sm100::SliceGemm g[2] = {};
+      g[0] = {Xs, h, W1, f, MAJOR_K, MAJOR_MN, EPI_BIAS_GELU, GemmShape{Ts, (int)f, (int)h},
+              EpiParams{b1, Hs, nullptr, nullptr, f, 0}, sm100::DEP_NONE, 0, 256, 1, 0};
+      g[1] = {Hs, f, W2, h, MAJOR_K, MAJOR_MN, EPI_BIAS, GemmShape{Ts, (int)h, (int)f},
+              EpiParams{b2, Ys, nullptr, nullptr, h, 0}, sm100::DEP_ROW, 0, sp.bn_narrow, 0, 0};
+      OSDP_TRY(sm100::launch_mlp_slice(g, 2, sync + (size_t)s * sp.words_per_slice, epoch0 + (unsigned int)s, nullptr, st));
+      continue;
+    }
     // A1: H_s = gelu(X_s W1 + b1)
     trace_set_step(1);
     EpiParams e1 = {b1, Hs, nullptr, nullptr, f, 0};
@@ -536,7 +588,12 @@ int osdp_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const void
   const int64_t fork_max = sm100::tuning().fork_max_tiles.load();
   const bool fork = fork_max > 0 && tiles_256(f, h) <= fork_max && tiles_256(ts_max, h) <= fork_max;
   ForkCtx* fc = nullptr;
-  if (fork) OSDP_TRY(fork_ctx(&fc));
+  SlicePlan sp;
+  OSDP_TRY(slice_plan(desc, OSDP_BWD, &sp));
+  unsigned int* sync = nullptr;
+  unsigned int epoch0 = 0;
+  if (sp.use) OSDP_TRY(sm100::slice_sync_acquire(sp.words, desc->k, &sync, &epoch0));
+  if (fork && !sp.use) OSDP_TRY(fork_ctx(&fc));
 
   int first = 1;
   for (int s = 0; s < desc->k; ++s) {
@@ -548,6 +605,24 @@ int osdp_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const void
     const char* Xs = (const char*)X + (size_t)lo * h * e;
     const char* dYs = (const char*)dY + (size_t)lo * h * e;
     char* dXs = (char*)dX + (size_t)lo * h * e;
+    if (sp.use) {
+      // A3 -> A4 -> A7 | A5 | A6 (+ db1) in one launch.  List order: the long-contraction dX tiles before the dW tiles.
+      trace_set_step(22);
+      sm100::SliceGemm g[5] = {};
+      g[0] = {Xs, h, W1, f, MAJOR_K, MAJOR_MN, EPI_BIAS_GELU_DUAL, GemmShape{Ts, (int)f, (int)h},
+              EpiParams{b1, Zs, Hs, nullptr, f, 0}, sm100::DEP_NONE, 0, 256, 1, 0};
+      g[1] = {dYs, h, W2, h, MAJOR_K, MAJOR_K, EPI_DGELU, GemmShape{Ts, (int)f, (int)h},
+              EpiParams{nullptr, Zs, nullptr, Zs, f, 0, scratch1, f}, sm100::DEP_SAME, 0, 256, 1, 0};
+      g[2] = {Zs, f, W1, f, MAJOR_K, MAJOR_K, EPI_PLAIN, GemmShape{Ts, (int)h, (int)f},
+              EpiParams{nullptr, dXs, nullptr, nullptr, h, 0}, sm100::DEP_ROW, 1, sp.bn_narrow, 0, 0};
+      g[3] = {Hs, f, dYs, h, MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32, GemmShape{(int)f, (int)h, Ts},
+              EpiParams{nullptr, dW2, nullptr, nullptr, h, beta}, sm100::DEP_COL_AS_M, 0, 256, 0, 0};
+      g[4] = {Xs, h, Zs, f, MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32, GemmShape{(int)h, (int)f, Ts},
+              EpiParams{nullptr, dW1, nullptr, nullptr, f, beta}, sm100::DEP_COL_AS_N, 1, 256, 0, 1};
+      const sm100::SliceDb1 dj = {scratch1, f, db1, (Ts + kBandRows - 1) / kBandRows, beta};
+      OSDP_TRY(sm100::launch_mlp_slice(g, 5, sync + (size_t)s * sp.words_per_slice, epoch0 + (unsigned int)s, &dj, st));
+      continue;
+    }
     // A3: Z_s = X_s W1 + b1, H_s = gelu(Z_s)
     trace_set_step(3);
     EpiParams e3 = {b1, Zs, Hs, nullptr, f, 0};

@@ -1,0 +1,155 @@
+"""The one-kernel-per-slice path of the token split (csrc/slice_sm100.cuh, OSDP_TUNE_SLICE_KERNEL_MAX_TILES): parity
+with the fp64 oracle, bit-identity with the launch-per-GEMM path, concurrency on two streams, CUDA-graph capture.
+GPU only (-m gpu)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import mlp_oracle as O
+from paper_2305_09940_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+NAMES = ("Y", "dX", "dW1", "db1", "dW2", "db2")
+
+
+def run_gpu(lib, inp, k, stream=None):
+    T, h = inp.X.shape
+    f = inp.W1.shape[1]
+    d = inp.to("cuda")
+    op = lib.SplitMlp(T, h, f, torch.bfloat16, k)
+    Y = op.forward(d.X, d.W1, d.b1, d.W2, d.b2)
+    g = op.backward(d.X, d.W1, d.b1, d.W2, d.dY)
+    torch.cuda.synchronize()
+    out = {"Y": Y}
+    out.update(g)
+    return {n: out[n].to(torch.float64).cpu().numpy() for n in NAMES}
+
+
+def rel_err(got, ref):
+    scale = float(np.max(np.abs(ref)))
+    return float(np.max(np.abs(got - ref))) / (scale if scale > 0 else 1.0)
+
+
+@pytest.fixture
+def slice_kernel(lib):
+    """Slice kernel for every eligible shape (the default threshold only takes small slices)."""
+    old = lib.osdp_get_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES)
+    lib.osdp_set_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES, 1 << 20)
+    yield
+    lib.osdp_set_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES, old)
+
+
+def per_gemm(lib, fn):
+    old = lib.osdp_get_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES)
+    lib.osdp_set_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES, 0)
+    try:
+        return fn()
+    finally:
+        lib.osdp_set_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES, old)
+
+
+@pytest.mark.parametrize("T,h,f,k", [
+    (256, 256, 512, 1),       # exact tiles, one tile row
+    (384, 128, 512, 2),
+    (333, 136, 520, 3),       # ragged everywhere
+    (130, 72, 264, 1),
+    (1000, 320, 1032, 4),
+    (64, 8, 8, 4),            # minimum hidden / ffn
+    (5, 64, 128, 5),          # one token per slice
+    (1, 16, 24, 1),
+    (1536, 1024, 2048, 2),    # several tile rows and columns: every dependency kind spans several tiles
+    (2100, 520, 1288, 3),     # the same, ragged; hidden wider than 256: 128-column tiles for A2 / A7
+])
+def test_slice_kernel_matches_oracle_and_the_per_gemm_path_bitwise(lib, slice_kernel, T, h, f, k):
+    inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=31)
+    ref = O.mlp_forward_backward(**inp.as_f64())
+    got = run_gpu(lib, inp, k)
+    n_fwd_bwd = lib.osdp_last_launch_count()
+    errs = {n: rel_err(got[n], ref[n]) for n in NAMES}
+    assert all(e <= 2e-2 for e in errs.values()), errs
+    assert n_fwd_bwd == 2 + k, "backward = db2 (two launches) + one slice kernel per slice"
+    want = per_gemm(lib, lambda: run_gpu(lib, inp, k))
+    for n in NAMES:
+        assert np.array_equal(got[n], want[n]), f"{n}: slice kernel and launch-per-GEMM path differ"
+
+
+def test_slice_kernel_is_reproducible_and_rows_do_not_depend_on_k(lib, slice_kernel):
+    inp = I.mlp_inputs(2048, 512, 1024, torch.bfloat16, seed=32)
+    a = run_gpu(lib, inp, 4)
+    b = run_gpu(lib, inp, 4)
+    c = run_gpu(lib, inp, 8)
+    for n in NAMES:
+        assert np.array_equal(a[n], b[n]), n
+    assert np.array_equal(a["Y"], c["Y"]) and np.array_equal(a["dX"], c["dX"]) and np.array_equal(a["db2"], c["db2"])
+
+
+def test_two_streams_of_slice_kernels_do_not_deadlock(lib, slice_kernel):
+    """Two slice kernels in flight on different streams can each hold SMs the other's missing CTAs would use; tiles are
+    claimed dynamically by the CTAs that run, so neither launch ever waits for a CTA that is not resident."""
+    T, h, f, k = 4096, 1024, 4096, 2
+    inps = [I.mlp_inputs(T, h, f, torch.bfloat16, seed=s) for s in (40, 41)]
+    want = [run_gpu(lib, inp, k) for inp in inps]
+    devs = [inp.to("cuda") for inp in inps]
+    ops = [lib.SplitMlp(T, h, f, torch.bfloat16, k) for _ in inps]
+    streams = [torch.cuda.Stream() for _ in inps]
+    torch.cuda.synchronize()
+    outs = [None, None]
+    for _ in range(4):
+        for i, (d, op, st) in enumerate(zip(devs, ops, streams)):
+            with torch.cuda.stream(st):
+                Y = op.forward(d.X, d.W1, d.b1, d.W2, d.b2, stream=st)
+                g = op.backward(d.X, d.W1, d.b1, d.W2, d.dY, stream=st)
+            outs[i] = dict(Y=Y, **g)
+    torch.cuda.synchronize()
+    for o, w in zip(outs, want):
+        for n in NAMES:
+            assert np.array_equal(o[n].double().cpu().numpy(), w[n]), n
+
+
+def test_slice_kernel_step_can_be_captured_in_a_cuda_graph(lib, slice_kernel):
+    T, h, f, k = 1000, 320, 1032, 4
+    inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=33)
+    want = run_gpu(lib, inp, k)
+    d = inp.to("cuda")
+    op = lib.SplitMlp(T, h, f, torch.bfloat16, k)
+    Y = torch.empty_like(d.X)
+    g = dict(dX=torch.empty_like(d.X), dW1=torch.empty(h, f, device="cuda"), db1=torch.empty(f, device="cuda"),
+             dW2=torch.empty(f, h, device="cuda"), db2=torch.empty(h, device="cuda"))
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        op.forward(d.X, d.W1, d.b1, d.W2, d.b2, Y=Y, stream=s)
+        op.backward(d.X, d.W1, d.b1, d.W2, d.dY, out=g, stream=s)
+        s.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=s):
+            op.forward(d.X, d.W1, d.b1, d.W2, d.b2, Y=Y, stream=s)
+            op.backward(d.X, d.W1, d.b1, d.W2, d.dY, out=g, stream=s)
+    for t in (Y, *g.values()):
+        t.fill_(7.0)
+    graph.replay()
+    graph.replay()
+    torch.cuda.synchronize()
+    got = dict(Y=Y, **g)
+    for n in NAMES:
+        assert np.array_equal(got[n].double().cpu().numpy(), want[n]), n
+
+
+def test_slice_kernel_trace_and_fallback(lib, slice_kernel):
+    """One traced launch per slice (steps 21 / 22); fp32 and over-sized calls keep the launch-per-GEMM path."""
+    T, h, f, k = 600, 128, 512, 3
+    d = I.mlp_inputs(T, h, f, torch.bfloat16, seed=34).to("cuda")
+    op = lib.SplitMlp(T, h, f, torch.bfloat16, k)
+    op.forward(d.X, d.W1, d.b1, d.W2, d.b2)
+    lib.osdp_trace_enable(True)
+    op.forward(d.X, d.W1, d.b1, d.W2, d.b2)
+    op.backward(d.X, d.W1, d.b1, d.W2, d.dY)
+    tr = lib.osdp_trace_read()
+    lib.osdp_trace_enable(False)
+    assert [s for s, _ in tr] == [21] * k + [8, 8] + [22] * k
+    assert "slice kernel" in lib.osdp_step_name(21) and "slice kernel" in lib.osdp_step_name(22)
+    d32 = I.mlp_inputs(96, 32, 64, torch.float32, seed=35).to("cuda")
+    op32 = lib.SplitMlp(96, 32, 64, torch.float32, 2)
+    op32.forward(d32.X, d32.W1, d32.b1, d32.W2, d32.b2)
+    assert lib.osdp_last_launch_count() == 2 * 2               # fp32: one launch per GEMM
