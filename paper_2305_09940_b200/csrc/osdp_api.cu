@@ -528,6 +528,7 @@ int osdp_split_mlp_forward(const osdp_mlp_desc* desc, const void* X, const void*
   unsigned int* sync = nullptr;
   unsigned int epoch0 = 0;
   if (sp.use) OSDP_TRY(sm100::slice_sync_acquire(sp.words, desc->k, &sync, &epoch0));
+  bool first_launch = true;
 
   for (int s = 0; s < desc->k; ++s) {
     const int64_t lo = (int64_t)s * T / desc->k, hi = (int64_t)(s + 1) * T / desc->k;
@@ -536,13 +537,20 @@ int osdp_split_mlp_forward(const osdp_mlp_desc* desc, const void* X, const void*
     const char* Xs = (const char*)X + (size_t)lo * h * e;
     char* Ys = (char*)Y + (size_t)lo * h * e;
     if (sp.use) {   // A1 -> A2 in one launch: an A2 tile starts when its 256 rows of H_s are complete
+      // A workspace with room for two H_s buffers (the backward's is: callers that train pass the same workspace to both
+      // passes) lets consecutive slices alternate buffers, and slice s then need not wait for slice s - 1 at all (see
+      // late_wait in slice_sm100.cuh); with the forward's own minimum the slices run one after another as the paper says.
+      const bool two_bufs = workspace_bytes_given >= 2 * slice_buf_bytes(desc);
+      void* Hb = two_bufs ? (char*)workspace + (size_t)(s & 1) * slice_buf_bytes(desc) : Hs;
       trace_set_step(21);
       sm100::SliceGemm g[2] = {};
       g[0] = {Xs, h, W1, f, MAJOR_K, MAJOR_MN, EPI_BIAS_GELU, GemmShape{Ts, (int)f, (int)h},
-              EpiParams{b1, Hs, nullptr, nullptr, f, 0}, sm100::DEP_NONE, 0, 256, 1, 0};
-      g[1] = {Hs, f, W2, h, MAJOR_K, MAJOR_MN, EPI_BIAS, GemmShape{Ts, (int)h, (int)f},
+              EpiParams{b1, Hb, nullptr, nullptr, f, 0}, sm100::DEP_NONE, 0, 256, 1, 0};
+      g[1] = {Hb, f, W2, h, MAJOR_K, MAJOR_MN, EPI_BIAS, GemmShape{Ts, (int)h, (int)f},
               EpiParams{b2, Ys, nullptr, nullptr, h, 0}, sm100::DEP_ROW, 0, sp.bn_narrow, 0, 0};
-      OSDP_TRY(sm100::launch_mlp_slice(g, 2, sync + (size_t)s * sp.words_per_slice, epoch0 + (unsigned int)s, nullptr, st));
+      OSDP_TRY(sm100::launch_mlp_slice(g, 2, sync + (size_t)s * sp.words_per_slice, epoch0 + (unsigned int)s, nullptr,
+                                       two_bufs && !first_launch, st));
+      first_launch = false;
       continue;
     }
     // A1: H_s = gelu(X_s W1 + b1)
@@ -606,21 +614,23 @@ int osdp_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const void
     const char* dYs = (const char*)dY + (size_t)lo * h * e;
     char* dXs = (char*)dX + (size_t)lo * h * e;
     if (sp.use) {
-      // A3 -> A4 -> A7 | A5 | A6 (+ db1) in one launch.  List order: the long-contraction dX tiles before the dW tiles.
+      // A3 | A4 -> A5 | A7 | A6 (+ db1) in one launch.  List order = claim order: a pair that has claimed a tile waits
+      // for it, so tiles come in the order in which their inputs become ready (H_s columns for A5 after A3, then the
+      // dZ_s rows for the long-contraction dX tiles and the dZ_s columns for A6 after A4).
       trace_set_step(22);
       sm100::SliceGemm g[5] = {};
       g[0] = {Xs, h, W1, f, MAJOR_K, MAJOR_MN, EPI_BIAS_GELU_DUAL, GemmShape{Ts, (int)f, (int)h},
               EpiParams{b1, Zs, Hs, nullptr, f, 0}, sm100::DEP_NONE, 0, 256, 1, 0};
       g[1] = {dYs, h, W2, h, MAJOR_K, MAJOR_K, EPI_DGELU, GemmShape{Ts, (int)f, (int)h},
               EpiParams{nullptr, Zs, nullptr, Zs, f, 0, scratch1, f}, sm100::DEP_SAME, 0, 256, 1, 0};
-      g[2] = {Zs, f, W1, f, MAJOR_K, MAJOR_K, EPI_PLAIN, GemmShape{Ts, (int)h, (int)f},
-              EpiParams{nullptr, dXs, nullptr, nullptr, h, 0}, sm100::DEP_ROW, 1, sp.bn_narrow, 0, 0};
-      g[3] = {Hs, f, dYs, h, MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32, GemmShape{(int)f, (int)h, Ts},
+      g[2] = {Hs, f, dYs, h, MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32, GemmShape{(int)f, (int)h, Ts},
               EpiParams{nullptr, dW2, nullptr, nullptr, h, beta}, sm100::DEP_COL_AS_M, 0, 256, 0, 0};
+      g[3] = {Zs, f, W1, f, MAJOR_K, MAJOR_K, EPI_PLAIN, GemmShape{Ts, (int)h, (int)f},
+              EpiParams{nullptr, dXs, nullptr, nullptr, h, 0}, sm100::DEP_ROW, 1, sp.bn_narrow, 0, 0};
       g[4] = {Xs, h, Zs, f, MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32, GemmShape{(int)h, (int)f, Ts},
               EpiParams{nullptr, dW1, nullptr, nullptr, f, beta}, sm100::DEP_COL_AS_N, 1, 256, 0, 1};
       const sm100::SliceDb1 dj = {scratch1, f, db1, (Ts + kBandRows - 1) / kBandRows, beta};
-      OSDP_TRY(sm100::launch_mlp_slice(g, 5, sync + (size_t)s * sp.words_per_slice, epoch0 + (unsigned int)s, &dj, st));
+      OSDP_TRY(sm100::launch_mlp_slice(g, 5, sync + (size_t)s * sp.words_per_slice, epoch0 + (unsigned int)s, &dj, false, st));
       continue;
     }
     // A3: Z_s = X_s W1 + b1, H_s = gelu(Z_s)

@@ -47,7 +47,8 @@ constexpr int kSliceFlags0 = 4;             // first flag word of a launch's par
 // What a tile waits for before its first operand load (tiles of phase dep_phase, which precedes it in the list):
 enum SliceDep : int {
   DEP_NONE = 0,
-  DEP_SAME = 1,       // the tile with the same coordinates (A4's epilogue reads the Z_s tile A3 stored)
+  DEP_SAME = 1,       // the tile with the same coordinates, needed by the EPILOGUE only (A4's epilogue reads the Z_s tile
+                      // A3 stored; its operands dY_s, W2 are inputs, so its main loop runs beside A3's)
   DEP_ROW = 2,        // every tile of the same tile ROW (A operand = the producer's output rows: A2 <- A1, A7 <- A4)
   DEP_COL_AS_M = 3,   // every tile of producer COLUMN band = this tile's row band (A5: rows of dW2 are columns of H_s)
   DEP_COL_AS_N = 4    // every tile of producer COLUMN band = this tile's column band (A6: columns of dW1 are columns of dZ_s)
@@ -69,6 +70,7 @@ struct SliceParams {
   unsigned int* sync;  // [0]: next list index to claim; [1]: pairs that have drawn their sentinel; [2]: CTAs that have left;
                        // [kSliceFlags0 + 2 t + r]: epoch once CTA r of the owning pair has published tile t
   unsigned int epoch;  // this launch's flag value (never 0; no two launches that can see the same flags share one)
+  int late_wait;       // 1: this launch does not depend on the previous kernel of the stream (see the kernel)
   // db1 (+)= sum over bands of band[r * ld_band + c] (the A4 epilogue's 32-row band sums of dZ_s)
   const float* band;
   int64_t ld_band;
@@ -182,8 +184,9 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
   const uint32_t qfull_bar = tempty_bar + 8 * kAccStages;       // [kSliceQueue] (each CTA): slot holds a tile index
   const uint32_t qempty_bar = qfull_bar + 8 * kSliceQueue;      // [kSliceQueue] (pair leader): every reader has read it
   const uint32_t tile_q = qempty_bar + 8 * kSliceQueue;         // [kSliceQueue] uint32
-  const uint32_t tmem_slot = tile_q + 4 * kSliceQueue;
-  static_assert(16 * kStages + 16 * kAccStages + 20 * kSliceQueue + 4 <= 256, "barrier area");
+  const uint32_t req_bar = tile_q + 4 * kSliceQueue;            // (pair leader): the producer wants its next tile
+  const uint32_t tmem_slot = req_bar + 8;
+  static_assert(16 * kStages + 16 * kAccStages + 20 * kSliceQueue + 8 + 4 <= 256, "barrier area");
   uint32_t* tmem_slot_ptr = reinterpret_cast<uint32_t*>(smem_raw + (tmem_slot - smem_u32(smem_raw)));
 
   const int warp = threadIdx.x / 32, lane = threadIdx.x % 32;
@@ -213,6 +216,7 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
       mbar_init(qfull_bar + 8 * i, 1);
       mbar_init(qempty_bar + 8 * i, kQueueReaders);
     }
+    mbar_init(req_bar, 1);
     fence_barrier_init();
   }
   if (warp == 2) {
@@ -223,8 +227,23 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
   cluster_sync();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot_ptr;
-  asm volatile("griddepcontrol.wait;" ::: "memory");
-  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  // Programmatic dependent launch.  Normally every thread waits for the previous kernel of the stream to complete
+  // before it touches memory, and then lets the next kernel start its set-up.  late_wait (forward slices s > 0 when the
+  // caller's workspace holds two H_s buffers): nothing this launch reads or writes is touched by the previous kernel
+  // (slice s - 1 uses the other buffer, other rows of Y), and the kernel before that (slice s - 2, the last user of this
+  // launch's buffer) had completed before the previous kernel let this one start.  So only one thread per CTA waits, off
+  // the critical path, and only then lets the NEXT kernel (slice s + 1, which reuses slice s - 1's buffer) start: the
+  // A1 tiles of this slice run beside the long-contraction A2 tiles of the previous one, which occupy few SMs.
+  if (!P.late_wait) {
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  } else if (warp == 2) {
+    if (lane == 0) {
+      asm volatile("griddepcontrol.wait;" ::: "memory");
+      asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    }
+    __syncwarp();
+  }
 
   unsigned int* const flags = P.sync + kSliceFlags0;   // two words per tile (one per CTA of the owning pair)
   const unsigned int epoch = P.epoch;
@@ -245,9 +264,7 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
   auto wait_deps = [&](const SlicePhase& S, const SliceTile& tl) {
     const SlicePhase& D = P.ph[S.dep_phase];
     const unsigned int* df = flags + 2 * D.tile_begin;
-    if (S.dep_kind == DEP_SAME) {
-      if (lane < 2) flag_wait(df + 2 * (tl.m_blk * D.num_n + tl.n_blk) + lane, epoch);
-    } else if (S.dep_kind == DEP_ROW) {
+    if (S.dep_kind == DEP_ROW) {
       for (int i = lane; i < 2 * D.num_n; i += 32) flag_wait(df + 2 * (tl.m_blk * D.num_n) + i, epoch);
     } else {
       const int col = S.dep_kind == DEP_COL_AS_M ? tl.m_blk : tl.n_blk;
@@ -264,6 +281,10 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
       const uint32_t tq_peer = mapa(tile_q, 1);
       for (int it = 0;; ++it) {
         const int slot = it % kSliceQueue;
+        // Claim on demand: tile it + 1 is drawn when the producer is close to the end of tile it's loads (the claim's
+        // latency hides behind the shared-memory ring), not as far ahead as the queue has room: tiles claimed early are
+        // tiles other pairs cannot take, and a pair in a long tile would sit on work the idle ones should do.
+        if (it > 0) mbar_wait(req_bar, (uint32_t)(it - 1) & 1u);
         mbar_wait(qempty_bar + 8 * slot, ((uint32_t)(it / kSliceQueue) & 1u) ^ 1u);
         unsigned int t = 0;
         if (lane == 0) {
@@ -296,7 +317,7 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
       const SlicePhase& S = P.ph[tl.phase];
       const CUtensorMap* map_a = &maps.m[tl.phase][0];
       const CUtensorMap* map_b = &maps.m[tl.phase][1];
-      if (S.dep_kind != DEP_NONE) {
+      if (S.dep_kind > DEP_SAME) {
         wait_deps(S, tl);
         fence_proxy_async_global();   // what the producers' TMA stores wrote -> visible to this thread's TMA loads
       }
@@ -305,7 +326,9 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
       const int n0 = tl.n_blk * S.bn + (int)rank * half_n;
       const int num_kb = (S.K + BLOCK_K - 1) / BLOCK_K;
       const uint32_t tx_bytes = 2u * (kAStageBytes + (uint32_t)half_n * (BLOCK_K * 2));
+      const int req_kb = num_kb > kStages + 2 ? num_kb - (kStages + 2) : 0;   // when to ask for the next tile
       for (int kb = 0; kb < num_kb; ++kb) {
+        if (kb == req_kb && leader && lane == 0) mbar_arrive(req_bar);
         mbar_wait(empty_bar + 8 * stage, phase ^ 1);
         if (lane == 0) {
           const uint32_t fb_local = full_bar + 8 * stage;
@@ -613,7 +636,7 @@ inline int slice_sync_acquire(int words, int launches, unsigned int** out, unsig
 }
 
 inline int launch_mlp_slice(const SliceGemm* g, int n, unsigned int* sync, unsigned int epoch, const SliceDb1* db1,
-                            cudaStream_t st) {
+                            bool late_wait, cudaStream_t st) {
   using Cfg = TileCfg<1, 1>;
   if (n < 1 || n > kSliceMaxPhases) return OSDP_ERR_ARG;
   SliceMaps maps;
@@ -621,6 +644,7 @@ inline int launch_mlp_slice(const SliceGemm* g, int n, unsigned int* sync, unsig
   P.num_phases = n;
   P.sync = sync;
   P.epoch = epoch;
+  P.late_wait = late_wait ? 1 : 0;
   if (db1) {
     P.band = db1->band;
     P.ld_band = db1->ld_band;
