@@ -614,23 +614,23 @@ int osdp_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const void
     const char* dYs = (const char*)dY + (size_t)lo * h * e;
     char* dXs = (char*)dX + (size_t)lo * h * e;
     if (sp.use) {
-      // A3 | A4 -> A5 | A7 | A6 (+ db1) in one launch.  List order = claim order: a pair that has claimed a tile waits
-      // for it, so tiles come in the order in which their inputs become ready (H_s columns for A5 after A3, then the
-      // dZ_s rows for the long-contraction dX tiles and the dZ_s columns for A6 after A4).
+      // (A3 + A4) -> A5 | A7 | A6 (+ db1) in one launch.  A3 and A4 share their output tile grid, so one tile runs both
+      // contractions into the two TMEM accumulators and one epilogue makes H_s and dZ_s (Z_s never goes to memory).
+      // List order = claim order: a pair that has claimed a tile waits for it, so the dW2 tiles come first (they need
+      // H_s columns), then the long-contraction dX tiles (dZ_s rows), then dW1 (dZ_s columns).
       trace_set_step(22);
-      sm100::SliceGemm g[5] = {};
-      g[0] = {Xs, h, W1, f, MAJOR_K, MAJOR_MN, EPI_BIAS_GELU_DUAL, GemmShape{Ts, (int)f, (int)h},
-              EpiParams{b1, Zs, Hs, nullptr, f, 0}, sm100::DEP_NONE, 0, 256, 1, 0};
-      g[1] = {dYs, h, W2, h, MAJOR_K, MAJOR_K, EPI_DGELU, GemmShape{Ts, (int)f, (int)h},
-              EpiParams{nullptr, Zs, nullptr, Zs, f, 0, scratch1, f}, sm100::DEP_SAME, 0, 256, 1, 0};
-      g[2] = {Hs, f, dYs, h, MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32, GemmShape{(int)f, (int)h, Ts},
+      sm100::SliceGemm g[4] = {};
+      g[0] = {Xs, h, W1, f, MAJOR_K, MAJOR_MN, sm100::kEpiFusedA34, GemmShape{Ts, (int)f, (int)h},
+              EpiParams{b1, Zs, Hs, nullptr, f, 0, scratch1, f}, sm100::DEP_NONE, 0, 256, 1, 0,
+              dYs, h, W2, h, MAJOR_K, MAJOR_K, (int)h};
+      g[1] = {Hs, f, dYs, h, MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32, GemmShape{(int)f, (int)h, Ts},
               EpiParams{nullptr, dW2, nullptr, nullptr, h, beta}, sm100::DEP_COL_AS_M, 0, 256, 0, 0};
-      g[3] = {Zs, f, W1, f, MAJOR_K, MAJOR_K, EPI_PLAIN, GemmShape{Ts, (int)h, (int)f},
-              EpiParams{nullptr, dXs, nullptr, nullptr, h, 0}, sm100::DEP_ROW, 1, sp.bn_narrow, 0, 0};
-      g[4] = {Xs, h, Zs, f, MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32, GemmShape{(int)h, (int)f, Ts},
-              EpiParams{nullptr, dW1, nullptr, nullptr, f, beta}, sm100::DEP_COL_AS_N, 1, 256, 0, 1};
+      g[2] = {Zs, f, W1, f, MAJOR_K, MAJOR_K, EPI_PLAIN, GemmShape{Ts, (int)h, (int)f},
+              EpiParams{nullptr, dXs, nullptr, nullptr, h, 0}, sm100::DEP_ROW, 0, sp.bn_narrow, 0, 0};
+      g[3] = {Xs, h, Zs, f, MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32, GemmShape{(int)h, (int)f, Ts},
+              EpiParams{nullptr, dW1, nullptr, nullptr, f, beta}, sm100::DEP_COL_AS_N, 0, 256, 0, 1};
       const sm100::SliceDb1 dj = {scratch1, f, db1, (Ts + kBandRows - 1) / kBandRows, beta};
-      OSDP_TRY(sm100::launch_mlp_slice(g, 5, sync + (size_t)s * sp.words_per_slice, epoch0 + (unsigned int)s, &dj, false, st));
+      OSDP_TRY(sm100::launch_mlp_slice(g, 4, sync + (size_t)s * sp.words_per_slice, epoch0 + (unsigned int)s, &dj, false, st));
       continue;
     }
     // A3: Z_s = X_s W1 + b1, H_s = gelu(Z_s)

@@ -43,6 +43,11 @@ constexpr int kSliceCallSlots = 32;         // calls in flight on one device tha
 constexpr int kSliceSyncWords = 16384;      // words per call: k x (2 + 2 x tiles of a slice) must fit
 constexpr unsigned int kPublishersPerTile = 2 * kNumEpiWarps;   // arrivals that hand a TMEM stage back
 constexpr int kSliceFlags0 = 4;             // first flag word of a launch's part of the array
+// A3 and A4 of the backward in one tile (they have the same output tile grid): accumulator 0 = X_s W1, accumulator 1 =
+// dY_s W2^T; the epilogue forms z = acc0 + b1 once, stores H_s = gelu(z) (out1) and dZ_s = acc1 * gelu'(bf16(z)) (out0)
+// and the 32-row band sums of dZ_s: the arithmetic of EPI_BIAS_GELU_DUAL followed by EPI_DGELU, without Z_s ever going
+// to memory and without a tile-to-tile dependency.
+constexpr int kEpiFusedA34 = 6;
 
 // What a tile waits for before its first operand load (tiles of phase dep_phase, which precedes it in the list):
 enum SliceDep : int {
@@ -63,6 +68,9 @@ struct SlicePhase {
   int dep_kind, dep_phase;
   int publish;         // a later phase waits for this phase's tiles
   int db1;             // A6: tiles of tile row 0 also reduce the db1 band partials of their columns
+  // Fused phase (epi == kEpiFusedA34): a tile runs TWO contractions into the two TMEM accumulator stages, first
+  // A x B (K), then A2 x B2 (K2), and one epilogue combines them.  A2 / B2's tensor maps sit in phase slot `aux`.
+  int fused, a2_major, b2_major, K2, aux;
   EpiParams ep;
 };
 struct SliceParams {
@@ -200,7 +208,11 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
       tma_prefetch_desc(&maps.m[p][0]);
       tma_prefetch_desc(&maps.m[p][1]);
       tma_prefetch_desc(&maps.m[p][2]);
-      if (P.ph[p].epi == EPI_BIAS_GELU_DUAL) tma_prefetch_desc(&maps.m[p][3]);
+      if (P.ph[p].epi == EPI_BIAS_GELU_DUAL || P.ph[p].fused) tma_prefetch_desc(&maps.m[p][3]);
+      if (P.ph[p].fused) {
+        tma_prefetch_desc(&maps.m[P.ph[p].aux][0]);
+        tma_prefetch_desc(&maps.m[P.ph[p].aux][1]);
+      }
     }
   }
   if (warp == 1 && lane == 0) {
@@ -324,9 +336,17 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
       const int half_n = S.bn / 2;
       const int m0 = tl.m_blk * UMMA_M + (int)rank * BLOCK_M;
       const int n0 = tl.n_blk * S.bn + (int)rank * half_n;
-      const int num_kb = (S.K + BLOCK_K - 1) / BLOCK_K;
       const uint32_t tx_bytes = 2u * (kAStageBytes + (uint32_t)half_n * (BLOCK_K * 2));
-      const int req_kb = num_kb > kStages + 2 ? num_kb - (kStages + 2) : 0;   // when to ask for the next tile
+      const int nseg = S.fused ? 2 : 1;
+      for (int seg = 0; seg < nseg; ++seg) {
+      const int a_major = seg ? S.a2_major : S.a_major, b_major = seg ? S.b2_major : S.b_major;
+      if (seg) {
+        map_a = &maps.m[S.aux][0];
+        map_b = &maps.m[S.aux][1];
+      }
+      const int num_kb = ((seg ? S.K2 : S.K) + BLOCK_K - 1) / BLOCK_K;
+      // when to ask for the next tile: a ring's worth of k-blocks before the end of this tile's loads
+      const int req_kb = seg + 1 < nseg ? -1 : (num_kb > kStages + 2 ? num_kb - (kStages + 2) : 0);
       for (int kb = 0; kb < num_kb; ++kb) {
         if (kb == req_kb && leader && lane == 0) mbar_arrive(req_bar);
         mbar_wait(empty_bar + 8 * stage, phase ^ 1);
@@ -336,13 +356,13 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
           const uint32_t sa = smem_a + stage * kAStageBytes, sb = smem_b + stage * kBStageBytes;
           const int k0 = kb * BLOCK_K;
           if (leader) mbar_expect_tx(fb_local, tx_bytes);
-          if (S.a_major == MAJOR_K) {
+          if (a_major == MAJOR_K) {
             tma_load_2d(sa, map_a, fb, k0, m0, pol);
           } else {
 #pragma unroll
             for (int c = 0; c < BLOCK_M / 64; ++c) tma_load_2d(sa + c * (BLOCK_K * 128), map_a, fb, m0 + 64 * c, k0, pol);
           }
-          if (S.b_major == MAJOR_K) {
+          if (b_major == MAJOR_K) {
             tma_load_2d(sb, map_b, fb, k0, n0, pol);
           } else {
             for (int c = 0; c < half_n / 64; ++c) tma_load_2d(sb + c * (BLOCK_K * 128), map_b, fb, n0 + 64 * c, k0, pol);
@@ -351,22 +371,26 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
         __syncwarp();
         if (++stage == kStages) { stage = 0; phase ^= 1; }
       }
+      }   // seg
     }
   } else if (warp == 1) {
     // ================================================================== MMA issuer (pair leader)
     if (leader) {
       int stage = 0;
       uint32_t phase = 0;
+      uint32_t acc = 0;   // accumulator stages handed out so far (a fused tile takes two)
       for (int it = 0;; ++it) {
         const int t = next_tile(it);
         if (t >= P.total_tiles) break;
         const SliceTile tl = slice_tile(P, t);
         const SlicePhase& S = P.ph[tl.phase];
-        const uint32_t idesc = make_idesc_rt(S.a_major, S.b_major, S.bn);
-        const int a_major = S.a_major, b_major = S.b_major;
-        const int num_kb = (S.K + BLOCK_K - 1) / BLOCK_K;
-        const int as = it % kAccStages;
-        mbar_wait(tempty_bar + 8 * as, (((uint32_t)(it / kAccStages)) & 1u) ^ 1u);
+        const int nseg = S.fused ? 2 : 1;
+        for (int seg = 0; seg < nseg; ++seg, ++acc) {
+        const int a_major = seg ? S.a2_major : S.a_major, b_major = seg ? S.b2_major : S.b_major;
+        const uint32_t idesc = make_idesc_rt(a_major, b_major, S.bn);
+        const int num_kb = ((seg ? S.K2 : S.K) + BLOCK_K - 1) / BLOCK_K;
+        const int as = (int)(acc % kAccStages);
+        mbar_wait(tempty_bar + 8 * as, ((acc / kAccStages) & 1u) ^ 1u);
         tc_fence_after();
         const uint32_t tmem_d = tmem_base + as * BLOCK_N;
         for (int kb = 0; kb < num_kb; ++kb) {
@@ -383,6 +407,7 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
           __syncwarp();
           if (++stage == kStages) { stage = 0; phase ^= 1; }
         }
+        }   // seg
       }
     }
   } else if (warp >= kEpiWarp0) {
@@ -391,6 +416,7 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
     const int cg = (warp - kEpiWarp0) / 4;
     StorePipe<1> pipe{smem_store + (uint32_t)(warp - kEpiWarp0) * kStoreBufBytes, lane};
     const uint32_t tempty_leader = mapa(tempty_bar, 0);
+    uint32_t acc_used = 0;   // accumulator stages consumed so far (mirrors the MMA warp's count)
     for (int it = 0;; ++it) {
       const int t = next_tile(it);
       if (t >= P.total_tiles) break;
@@ -399,8 +425,9 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
       const CUtensorMap* map0 = &maps.m[tl.phase][2];
       const CUtensorMap* map1 = &maps.m[tl.phase][3];
       const EpiParams& ep = S.ep;
-      const int as = it % kAccStages;
-      const uint32_t aphase = ((uint32_t)(it / kAccStages)) & 1u;
+      const int as = (int)(acc_used % kAccStages);
+      const uint32_t aphase = (acc_used / kAccStages) & 1u;
+      acc_used += S.fused ? 2u : 1u;
       const int M = S.M, N = S.N;
       const int n0 = tl.n_blk * S.bn;
       const int n_end = min(n0 + S.bn, N);
@@ -535,7 +562,121 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
           if (lane == 0) mbar_arrive_cluster(tempty_leader + 8 * as);
         }
       };
+
+      // ---- fused A3 + A4 tile: accumulator 0 in stage `as`, accumulator 1 in the other stage
+      auto run_fused = [&]() {
+        const int as1 = as ^ 1;
+        const uint32_t aphase1 = ((acc_used - 1u) / kAccStages) & 1u;
+        const uint32_t taddr1 = tmem_base + ((uint32_t)(q * 32) << 16) + as1 * BLOCK_N;
+        const __nv_bfloat16* bias = reinterpret_cast<const __nv_bfloat16*>(ep.bias);
+        uint32_t bias_reg[2];
+#pragma unroll
+        for (int ci = 0; ci < 2; ++ci) {
+          const int c = n0 + (cg + 2 * ci) * 64 + 2 * lane;
+          bias_reg[ci] = c < N ? __ldg(reinterpret_cast<const uint32_t*>(bias + c)) : 0u;
+        }
+        // z (fp32) = accumulator 0 + b1 for 8 consecutive columns; j = index of the 8-column group inside the chunk
+        auto z8 = [&](const uint32_t* a, uint32_t bias_cur, int j, float (&v)[8]) {
+#pragma unroll
+          for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(a[i]);
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const uint32_t bw = __shfl_sync(0xFFFFFFFFu, bias_cur, 4 * j + i);
+            v[2 * i] += bf16_lo(bw);
+            v[2 * i + 1] += bf16_hi(bw);
+          }
+        };
+        auto pack8 = [](const float (&v)[8]) {
+          return make_uint4(pack_bf16x2(v[0], v[1]), pack_bf16x2(v[2], v[3]), pack_bf16x2(v[4], v[5]), pack_bf16x2(v[6], v[7]));
+        };
+        // pass 1 (needs only X_s W1, which finishes first): H_s = gelu(z)
+        mbar_wait(tfull_bar + 8 * as, aphase);
+        tc_fence_after();
+        if (row0 < M) {
+#pragma unroll 1
+          for (int n = n0 + cg * 64; n < n_end; n += 128) {
+            uint32_t a0[64];
+            tmem_ld_32x32(taddr + (n - n0), *reinterpret_cast<uint32_t(*)[32]>(&a0[0]));
+            tmem_ld_32x32(taddr + (n - n0) + 32, *reinterpret_cast<uint32_t(*)[32]>(&a0[32]));
+            tmem_ld_wait();
+            const uint32_t bias_cur = (n - n0) >= 128 ? bias_reg[1] : bias_reg[0];
+            pipe.begin();
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              float v[8];
+              z8(&a0[8 * j], bias_cur, j, v);
+#pragma unroll
+              for (int i = 0; i < 8; ++i) v[i] = gelu_fwd<false>(v[i]);
+              pipe.put(j, pack8(v));
+            }
+            pipe.commit(map1, n, row0, false);
+          }
+        }
+        // pass 2: dZ_s = (dY_s W2^T) * gelu'(Z_s), Z_s = z rounded to bf16 exactly as EPI_BIAS_GELU_DUAL would store it
+        mbar_wait(tfull_bar + 8 * as1, aphase1);
+        tc_fence_after();
+        bool released = false;
+        if (row0 < M) {
+#pragma unroll 1
+          for (int n = n0 + cg * 64; n < n_end; n += 128) {
+            const uint32_t bias_cur = (n - n0) >= 128 ? bias_reg[1] : bias_reg[0];
+            pipe.begin();
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+              uint32_t a0[32], a1[32];
+              tmem_ld_32x32(taddr + (n - n0) + 32 * half, a0);
+              tmem_ld_32x32(taddr1 + (n - n0) + 32 * half, a1);
+              tmem_ld_wait();
+              if (half == 1 && n + 128 >= n_end) {   // this warp's last read of both accumulator stages
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) {
+                  mbar_arrive_cluster(tempty_leader + 8 * as);
+                  mbar_arrive_cluster(tempty_leader + 8 * as1);
+                }
+                released = true;
+              }
+#pragma unroll
+              for (int jj = 0; jj < 4; ++jj) {
+                const int j = 4 * half + jj;
+                float z[8], d[8];
+                z8(&a0[8 * jj], bias_cur, j, z);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                  const uint32_t zw = pack_bf16x2(z[2 * i], z[2 * i + 1]);
+                  d[2 * i] = __uint_as_float(a1[8 * jj + 2 * i]) * gelu_bwd<false>(bf16_lo(zw));
+                  d[2 * i + 1] = __uint_as_float(a1[8 * jj + 2 * i + 1]) * gelu_bwd<false>(bf16_hi(zw));
+                }
+                pipe.put(j, pack8(d));
+              }
+            }
+            pipe.commit(map0, n, row0, false);
+            if (ep.colsum != nullptr) {   // db1 band sums from the staged bf16 values (step A4)
+              const uint32_t src = pipe.committed_buf() + ((lane & 3) << 2);
+              float s0 = 0.0f, s1 = 0.0f;
+#pragma unroll
+              for (int r = 0; r < 32; ++r) {
+                uint32_t w;
+                asm volatile("ld.shared.b32 %0, [%1];" : "=r"(w) : "r"(src + r * 128 + ((((uint32_t)lane >> 2) ^ (r & 7)) << 4)));
+                s0 += bf16_lo(w);
+                s1 += bf16_hi(w);
+              }
+              const int c = n + 2 * lane;
+              if (c < N) *reinterpret_cast<float2*>(ep.colsum + (int64_t)(row0 >> 5) * ep.ld_colsum + c) = make_float2(s0, s1);
+            }
+          }
+        }
+        if (!released) {
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) {
+            mbar_arrive_cluster(tempty_leader + 8 * as);
+            mbar_arrive_cluster(tempty_leader + 8 * as1);
+          }
+        }
+      };
       switch (S.epi) {
+        case kEpiFusedA34: run_fused(); break;
         case EPI_BIAS_GELU: run(std::integral_constant<int, EPI_BIAS_GELU>{}); break;
         case EPI_BIAS: run(std::integral_constant<int, EPI_BIAS>{}); break;
         case EPI_BIAS_GELU_DUAL: run(std::integral_constant<int, EPI_BIAS_GELU_DUAL>{}); break;
@@ -604,6 +745,12 @@ struct SliceGemm {   // one phase as the scheduler states it (operands as in lau
   int bn;        // 256 or 128
   int publish;
   int db1;
+  // fused phase (epi == kEpiFusedA34): the second contraction A2 [M x K2] x B2 [K2 x N]
+  const void* A2 = nullptr;
+  int64_t lda2 = 0;
+  const void* B2 = nullptr;
+  int64_t ldb2 = 0;
+  int a2_major = 0, b2_major = 0, K2 = 0;
 };
 struct SliceDb1 {
   const float* band;
@@ -664,6 +811,7 @@ inline int launch_mlp_slice(const SliceGemm* g, int n, unsigned int* sync, unsig
     S.tile_begin = tiles;
     S.dep_kind = G.dep_kind; S.dep_phase = G.dep_phase;
     S.publish = G.publish; S.db1 = G.db1;
+    S.fused = G.epi == kEpiFusedA34 ? 1 : 0;
     S.ep = G.ep;
     tiles += S.num_m * S.num_n;
     int rc;
@@ -677,13 +825,23 @@ inline int launch_mlp_slice(const SliceGemm* g, int n, unsigned int* sync, unsig
     rc = make_tmap(&maps.m[p][2], G.ep.out0, G.s.N, G.s.M, G.ep.ldo, f32out ? 32 : 64, 32, f32out);
     if (rc != OSDP_OK) return rc;
     maps.m[p][3] = maps.m[p][2];
-    if (G.epi == EPI_BIAS_GELU_DUAL) {
+    if (S.fused) {   // the second contraction's operand maps go to the first phase slot this launch does not use
+      if (n >= kSliceMaxPhases || G.bn != BLOCK_N) return OSDP_ERR_ARG;
+      S.a2_major = G.a2_major; S.b2_major = G.b2_major; S.K2 = G.K2; S.aux = n;
+      if (G.a2_major == MAJOR_K) rc = make_tmap(&maps.m[n][0], G.A2, G.K2, G.s.M, G.lda2, BLOCK_K, BLOCK_M);
+      else                       rc = make_tmap(&maps.m[n][0], G.A2, G.s.M, G.K2, G.lda2, 64, BLOCK_K);
+      if (rc != OSDP_OK) return rc;
+      if (G.b2_major == MAJOR_K) rc = make_tmap(&maps.m[n][1], G.B2, G.K2, G.s.N, G.ldb2, BLOCK_K, G.bn / 2);
+      else                       rc = make_tmap(&maps.m[n][1], G.B2, G.s.N, G.K2, G.ldb2, 64, BLOCK_K);
+      if (rc != OSDP_OK) return rc;
+    }
+    if (G.epi == EPI_BIAS_GELU_DUAL || S.fused) {
       rc = make_tmap(&maps.m[p][3], G.ep.out1, G.s.N, G.s.M, G.ep.ldo, 64, 32, false);
       if (rc != OSDP_OK) return rc;
     }
   }
   for (int p = n; p < kSliceMaxPhases; ++p)
-    for (int i = 0; i < 4; ++i) maps.m[p][i] = maps.m[0][i];
+    for (int i = (p == n && P.ph[0].fused ? 2 : 0); i < 4; ++i) maps.m[p][i] = maps.m[0][i];
   P.total_tiles = tiles;
 
   DeviceInfo dev;
