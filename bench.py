@@ -35,6 +35,9 @@ import torch  # noqa: E402
 METRIC = "split_mlp_fwd_bwd_tflops"
 UNIT = "TFLOP/s"
 NOMINAL_BF16_TFLOPS = 2250.0      # dense bf16, B200 (B200_PROFILING.md; context only)
+# GEMMs (of 2 T_s h f flops each) per traced launch: steps A1-A7 are one GEMM; the one-kernel-per-slice launches (small
+# slices, csrc/slice_sm100.cuh) hold the forward's two (step 21) / the backward's five (step 22)
+GEMMS_PER_LAUNCH = {1: 1, 2: 1, 3: 1, 4: 1, 5: 1, 6: 1, 7: 1, 21: 2, 22: 5}
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 L2_BYTES = 126 << 20
 
@@ -771,11 +774,12 @@ def main():
         avg = sum(v) / len(v)
         ent = {"step": lib.osdp_step_name(sid), "launches_per_step": len(v) // args.steps, "avg_ms": avg,
                "share": sum(v) / total_traced}
-        if sid <= 7:
-            ent["tflops"] = gemm_flops / (avg * 1e-3) / 1e12
-        kernels[f"A{sid}" if sid <= 8 else "acc_to_out"] = ent
-    dom = max((s for s in per if s <= 7), key=lambda s: sum(per[s]))
+        if sid in GEMMS_PER_LAUNCH:
+            ent["tflops"] = GEMMS_PER_LAUNCH[sid] * gemm_flops / (avg * 1e-3) / 1e12
+        kernels[{21: "slice_fwd", 22: "slice_bwd", 10: "acc_to_out"}.get(sid, f"A{sid}")] = ent
+    dom = max((s for s in per if s in GEMMS_PER_LAUNCH), key=lambda s: sum(per[s]))
     dom_avg = sum(per[dom]) / len(per[dom])
+    gemm_flops *= GEMMS_PER_LAUNCH[dom]            # flops of one launch of the dominant kernel
     achieved = gemm_flops / (dom_avg * 1e-3) / 1e12
     peak = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]) if cfg["dtype"] == "bf16" else None
     # DRAM bytes of the dominant kernel per launch, from the committed ncu --set full capture (profiles/traffic.json; its
@@ -804,7 +808,7 @@ def main():
             operand_path = {"l2_to_sm_bytes_per_launch": l2b, "achieved_B_per_clk": bpc, "ceiling_B_per_clk": 6300.0,
                             "frac": bpc / 6300.0, "clock_mhz": clocks["sm_mhz"],
                             "how": "ncu lts__t_sectors_srcunit_tex_op_read x 32 B (profiles/r02_ncu_full.md) / (avg launch ms x SM clock sampled in this run)"}
-    roofline = {"bound": "tensor", "kernel": f"gemm_bf16_sm100_kernel [{lib.osdp_step_name(dom)}]",
+    roofline = {"bound": "tensor", "kernel": f"{'mlp_slice_kernel' if dom >= 21 else 'gemm_bf16_sm100_kernel'} [{lib.osdp_step_name(dom)}]",
                 "achieved": achieved, "peak": peak, "unit": UNIT, "frac": (achieved / peak) if peak else None,
                 "traffic": traffic, "traffic_detail": traffic_detail, "operand_path": operand_path, "peak_source": f"{peaks['source']} (bf16_tflops_sustained: kernel timed inside a long step)",
                 "frac_of_burst": achieved / peaks["bf16_tflops"], "frac_of_nominal": achieved / NOMINAL_BF16_TFLOPS,

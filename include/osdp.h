@@ -210,12 +210,15 @@ typedef enum osdp_tune_key {
                                       C5 layer shape, neutral to -1 % at C3 / C4, which the default excludes); 0 = always
                                       in sequence */
   OSDP_TUNE_SLICE_KERNEL_MAX_TILES = 7
-                                   /* token split, bf16: when every GEMM of a slice has at most this many 256 x 256
-                                      output tiles, the whole slice runs as ONE persistent kernel (forward A1 -> A2;
-                                      backward A3 -> A4 -> A7 | A5 | A6 and the db1 sum): CTA pairs claim tiles of all
-                                      GEMMs from one list and a tile waits only for the producer tiles it reads
-                                      (csrc/slice_sm100.cuh).  Results are bit-identical to the
-                                      launch-per-GEMM path.  0 = never */
+                                   /* default 96.  Token split, bf16: when the [T_s x ffn] GEMMs of a slice have at most
+                                      this many 256 x 256 output tiles (small slices: about one wave), the whole slice
+                                      runs as ONE persistent kernel (forward A1 -> A2; backward (A3 + A4 fused per tile)
+                                      -> A7 | A5 | A6 and the db1 sum): CTA pairs claim tiles of all GEMMs from one list
+                                      and a tile waits only for the producer tiles it reads (csrc/slice_sm100.cuh,
+                                      DESIGN.md section 6.5).  Results are bit-identical to the launch-per-GEMM path.
+                                      If the workspace passed to the forward has room for two slice buffers (the
+                                      backward's size), consecutive forward slices alternate buffers and overlap.
+                                      0 = never */
 } osdp_tune_key;
 int osdp_set_tuning(int key, int64_t value);
 int64_t osdp_get_tuning(int key);

@@ -252,9 +252,11 @@ inline int64_t tiles_256(int64_t m, int64_t n) { return ((m + 255) / 256) * ((n 
 
 
 // ---- one persistent kernel per slice (slice_sm100.cuh) ----------------------------------------------------------
-// Taken for bf16 when every GEMM of a slice has at most OSDP_TUNE_SLICE_KERNEL_MAX_TILES tiles of 256 x 256 and the
-// call's completion counters fit the per-call block.  A2 / A7 (long contraction, few output tiles) take 128-column
-// tiles when that still fits one wave of CTA pairs, so they spread over twice as many SMs.
+// Taken for bf16 when the slice is small in TOKENS: its [T_s x ffn] GEMMs (A1, A3, A4) have at most
+// OSDP_TUNE_SLICE_KERNEL_MAX_TILES tiles of 256 x 256, i.e. about one wave, which is where a launch per GEMM is mostly
+// fill and drain (measured crossover: C2 k = 4 / C5 layer k = 16 at 128 tiles break even, 64 tiles gain 8-26 %; the dW
+// GEMMs' tile count does not matter), and the call's flags fit the per-call block.  A2 / A7 (long contraction, few
+// output tiles) take 128-column tiles when that still fits one wave of CTA pairs, so they spread over twice as many SMs.
 struct SlicePlan {
   bool use = false;
   int bn_narrow = 256;   // tile width of A2 / A7
@@ -268,7 +270,7 @@ int slice_plan(const osdp_mlp_desc* d, int pass, SlicePlan* out) {
   OSDP_TRY(sm100::current_device(&dev));
   const int64_t ts = (d->tokens + d->k - 1) / d->k;
   const int64_t t_tf = tiles_256(ts, d->ffn), t_th = tiles_256(ts, d->hidden), t_fh = tiles_256(d->ffn, d->hidden);
-  if (t_tf > max_tiles || t_th > max_tiles || t_fh > max_tiles) return OSDP_OK;
+  if (t_tf > max_tiles) return OSDP_OK;
   out->bn_narrow = 2 * t_th <= dev.sms / 2 ? 128 : 256;
   const int64_t t_narrow = ((ts + 255) / 256) * ((d->hidden + out->bn_narrow - 1) / out->bn_narrow);
   const int64_t per_slice = sm100::kSliceFlags0 + 2 * (pass == OSDP_FWD ? t_tf + t_narrow : 2 * t_tf + t_narrow + 2 * t_fh);
@@ -473,7 +475,7 @@ const char* osdp_step_name(int step_id) {
     case 12: return "Linear bwd dX = dY W^T";
     case 13: return "Linear bwd dW += X^T dY";
     case 21: return "slice kernel fwd (A1 -> A2 in one launch)";
-    case 22: return "slice kernel bwd (A3 -> A4 -> A7 | A5 | A6 + db1 in one launch)";
+    case 22: return "slice kernel bwd ((A3 + A4 fused) -> A7 | A5 | A6 + db1 in one launch)";
     default: return "unknown";
   }
 }
@@ -616,17 +618,17 @@ int osdp_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const void
     if (sp.use) {
       // (A3 + A4) -> A5 | A7 | A6 (+ db1) in one launch.  A3 and A4 share their output tile grid, so one tile runs both
       // contractions into the two TMEM accumulators and one epilogue makes H_s and dZ_s (Z_s never goes to memory).
-      // List order = claim order: a pair that has claimed a tile waits for it, so the dW2 tiles come first (they need
-      // H_s columns), then the long-contraction dX tiles (dZ_s rows), then dW1 (dZ_s columns).
+      // List order = claim order; everything after the fused tiles becomes ready at about the same time, so the
+      // long-contraction dX tiles (few tiles, four times the k-blocks of the others) go first and the dW tiles fill in.
       trace_set_step(22);
       sm100::SliceGemm g[4] = {};
       g[0] = {Xs, h, W1, f, MAJOR_K, MAJOR_MN, sm100::kEpiFusedA34, GemmShape{Ts, (int)f, (int)h},
               EpiParams{b1, Zs, Hs, nullptr, f, 0, scratch1, f}, sm100::DEP_NONE, 0, 256, 1, 0,
               dYs, h, W2, h, MAJOR_K, MAJOR_K, (int)h};
-      g[1] = {Hs, f, dYs, h, MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32, GemmShape{(int)f, (int)h, Ts},
-              EpiParams{nullptr, dW2, nullptr, nullptr, h, beta}, sm100::DEP_COL_AS_M, 0, 256, 0, 0};
-      g[2] = {Zs, f, W1, f, MAJOR_K, MAJOR_K, EPI_PLAIN, GemmShape{Ts, (int)h, (int)f},
+      g[1] = {Zs, f, W1, f, MAJOR_K, MAJOR_K, EPI_PLAIN, GemmShape{Ts, (int)h, (int)f},
               EpiParams{nullptr, dXs, nullptr, nullptr, h, 0}, sm100::DEP_ROW, 0, sp.bn_narrow, 0, 0};
+      g[2] = {Hs, f, dYs, h, MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32, GemmShape{(int)f, (int)h, Ts},
+              EpiParams{nullptr, dW2, nullptr, nullptr, h, beta}, sm100::DEP_COL_AS_M, 0, 256, 0, 0};
       g[3] = {Xs, h, Zs, f, MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32, GemmShape{(int)h, (int)f, Ts},
               EpiParams{nullptr, dW1, nullptr, nullptr, f, beta}, sm100::DEP_COL_AS_N, 0, 256, 0, 1};
       const sm100::SliceDb1 dj = {scratch1, f, db1, (Ts + kBandRows - 1) / kBandRows, beta};

@@ -1,22 +1,24 @@
-// slice_sm100.cuh — one persistent kernel per SLICE of the token-split MLP (small and medium slices).
+// slice_sm100.cuh — one persistent kernel per SLICE of the token-split MLP (small slices).
 //
 // A slice of the operator-split MLP (slices "executed sequentially") is a short chain of GEMMs:
-// forward A1 -> A2, backward A3 -> A4 -> {A7, A5, A6}.  When a slice is small each GEMM is a fraction of a wave and a
+// forward A1 -> A2, backward (A3, A4) -> {A7, A5, A6}.  When a slice is small each GEMM is a fraction of a wave and a
 // few microseconds of tensor time, and one launch per GEMM spends more time filling and draining the machine than
-// computing (C2 at k = 8 ran at 0.36 of the sustained peak, cuBLAS launch by launch would reach
-// 0.53).  This kernel runs ALL GEMMs of one slice in ONE launch: the tiles of every GEMM ("phase") form one list,
-// CTA pairs claim tiles from it in order through a global counter, and a tile that reads another phase's output
-// waits for exactly the producer tiles it needs (per-tile completion counters in global memory), so the machine
-// drains only once per slice and independent GEMMs (A7 | A5 | A6) fill each other's partial waves.
+// computing.  This kernel runs ALL GEMMs of one slice in ONE launch: the tiles of every GEMM
+// ("phase") form one list, CTA pairs claim tiles from it in order through a global counter, and a tile that reads
+// another phase's output waits for exactly the producer tiles it needs (per-tile flags in global memory), so the
+// machine drains once per slice and independent GEMMs (A7 | A5 | A6) fill each other's partial waves.
 //
 //   * Tile pipeline, warp roles, shared-memory ring, TMEM double buffering, epilogue math: those of the MT = 1
 //     configuration of gemm_sm100.cuh (256 x 256 pair tiles, tcgen05.mma.cta_group::2, TMA loads / stores), with
 //     operand majorness, epilogue kind and tile width (256 or 128 columns) read per phase at run time.
-//   * Dynamic tile claiming (warp 3 of each pair's leader CTA: atomicAdd on the launch's tile counter, the index is
-//     handed to both CTAs of the pair through a small shared-memory queue): a tile only ever waits for tiles with a
-//     SMALLER list index, and those were claimed by pairs that are already running.  So the kernel cannot deadlock
-//     however few of its CTAs are resident (two such launches on two streams each holding SMs the other wants are
-//     fine), which a static tile-to-pair assignment could not promise.
+//   * A3 and A4 share their output tile grid and are ONE phase: a tile runs X_s W1 into TMEM accumulator 0 and
+//     dY_s W2^T into accumulator 1, and one epilogue makes H_s and dZ_s from the same z (kEpiFusedA34 below).
+//   * Tile claiming on demand (warp 3 of each pair's leader CTA: atomicAdd on the launch's tile counter when the
+//     producer nears the end of its current tile; the index reaches both CTAs of the pair through a small shared-memory
+//     queue): a tile only ever waits for tiles with a SMALLER list index, and those were claimed by pairs that are
+//     already running.  So the kernel cannot deadlock however few of its CTAs are resident (two such launches on two
+//     streams each holding SMs the other wants are fine), which a static tile-to-pair assignment could not promise,
+//     and a pair inside a long tile does not sit on tiles the idle pairs could take.
 //   * Publication: every epilogue warp waits for its TMA stores of the tile to complete (cp.async.bulk.wait_group 0)
 //     and fences the async proxy, the 8 epilogue warps of the CTA meet at a named barrier, and one thread stores the
 //     launch's EPOCH (release, gpu scope) into the tile's flag of this CTA; a tile is complete when both CTAs' flags
@@ -25,8 +27,13 @@
 //     sentinel puts the tile counter back to zero and the last CTA to leave clears the flags (so a captured launch can
 //     be replayed); the per-launch epoch only guards against flags an earlier launch could not clear.  Every launch in
 //     flight owns its own part of the array (osdp_api.cu).
-//   * db1: the A6 tiles of the first tile row also add up the 32-row band sums that the A4 epilogue left in the
+//   * Forward slices pipeline: with room for two H_s buffers in the caller's workspace, slice s does not wait for
+//     slice s - 1 (late_wait below), so its A1 tiles run beside the few long A2 tiles of the slice before.
+//   * db1: the A6 tiles of the first tile row also add up the 32-row band sums that the fused epilogue left in the
 //     scratch (bands in ascending order, one thread per column: the arithmetic of colsum_final_kernel).
+//   * No remote mbarrier arrive is left unconsumed at exit, and the teardown is a release / acquire cluster barrier: a
+//     remote arrive still in flight when the peer CTA has exited lands in the NEXT kernel's CTA on that SM (found the
+//     hard way: a queue slot refilled before its slowest reader had read it).
 // Results are bit-identical to the launch-per-GEMM path: same tile shape per output element, same ascending-k
 // accumulation, same epilogue arithmetic, same db1 order (tests/test_gpu_slice_kernel.py).
 #pragma once
@@ -52,11 +59,9 @@ constexpr int kEpiFusedA34 = 6;
 // What a tile waits for before its first operand load (tiles of phase dep_phase, which precedes it in the list):
 enum SliceDep : int {
   DEP_NONE = 0,
-  DEP_SAME = 1,       // the tile with the same coordinates, needed by the EPILOGUE only (A4's epilogue reads the Z_s tile
-                      // A3 stored; its operands dY_s, W2 are inputs, so its main loop runs beside A3's)
-  DEP_ROW = 2,        // every tile of the same tile ROW (A operand = the producer's output rows: A2 <- A1, A7 <- A4)
-  DEP_COL_AS_M = 3,   // every tile of producer COLUMN band = this tile's row band (A5: rows of dW2 are columns of H_s)
-  DEP_COL_AS_N = 4    // every tile of producer COLUMN band = this tile's column band (A6: columns of dW1 are columns of dZ_s)
+  DEP_ROW = 1,        // every tile of the same tile ROW (A operand = the producer's output rows: A2 <- A1, A7 <- A4)
+  DEP_COL_AS_M = 2,   // every tile of producer COLUMN band = this tile's row band (A5: rows of dW2 are columns of H_s)
+  DEP_COL_AS_N = 3    // every tile of producer COLUMN band = this tile's column band (A6: columns of dW1 are columns of dZ_s)
 };
 
 struct SlicePhase {
@@ -329,7 +334,7 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
       const SlicePhase& S = P.ph[tl.phase];
       const CUtensorMap* map_a = &maps.m[tl.phase][0];
       const CUtensorMap* map_b = &maps.m[tl.phase][1];
-      if (S.dep_kind > DEP_SAME) {
+      if (S.dep_kind != DEP_NONE) {
         wait_deps(S, tl);
         fence_proxy_async_global();   // what the producers' TMA stores wrote -> visible to this thread's TMA loads
       }
@@ -432,15 +437,14 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
       const int n0 = tl.n_blk * S.bn;
       const int n_end = min(n0 + S.bn, N);
       const int row0 = tl.m_blk * UMMA_M + (int)rank * BLOCK_M + q * 32;   // this warp's 32-row band
-      const int64_t row = row0 + lane;
-      const bool row_ok = row < M;
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + as * BLOCK_N;
 
+      // ---- one contraction per tile: bias + GeLU (A1), bias (A2), plain (A7), fp32 store / reduce-add (A5, A6)
       auto run = [&](auto tag) {
         constexpr int EPI = decltype(tag)::value;
         using Tr = EpiTraits<EPI>;
         constexpr int kChunk = Tr::kChunkCols;
-        constexpr bool kHasBias = (EPI == EPI_BIAS_GELU || EPI == EPI_BIAS || EPI == EPI_BIAS_GELU_DUAL);
+        constexpr bool kHasBias = (EPI == EPI_BIAS_GELU || EPI == EPI_BIAS);
         uint32_t bias_reg[2] = {0u, 0u};
         if constexpr (kHasBias) {
           const __nv_bfloat16* bias = reinterpret_cast<const __nv_bfloat16*>(ep.bias);
@@ -470,11 +474,6 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
             for (int n = n0 + cg * kChunk; n < n_end; n += 2 * kChunk) tma_prefetch_l2_2d(map0, n, row0);
           }
         }
-        if constexpr (EPI == EPI_DGELU) {   // the stored Z_s tile (phase dep_phase, same coordinates) is complete
-          const SlicePhase& D = P.ph[S.dep_phase];
-          if (lane < 2) flag_wait(flags + 2 * (D.tile_begin + tl.m_blk * D.num_n + tl.n_blk) + lane, epoch);
-          __syncwarp();
-        }
         mbar_wait(tfull_bar + 8 * as, aphase);
         tc_fence_after();
         bool released = false;
@@ -482,15 +481,6 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
 #pragma unroll 1
           for (int n = n0 + cg * kChunk; n < n_end; n += 2 * kChunk) {
             uint32_t acc[kChunk];
-            [[maybe_unused]] uint4 zraw[8];
-            if constexpr (EPI == EPI_DGELU) {
-#pragma unroll
-              for (int j = 0; j < 8; ++j) {
-                zraw[j] = make_uint4(0, 0, 0, 0);
-                if (row_ok && n + 8 * j < N)
-                  zraw[j] = __ldcg(reinterpret_cast<const uint4*>((const __nv_bfloat16*)ep.aux + row * ep.ldo + n + 8 * j));
-              }
-            }
 #pragma unroll
             for (int i = 0; i < kChunk / 32; ++i)
               tmem_ld_32x32(taddr + (n - n0) + 32 * i, *reinterpret_cast<uint32_t(*)[32]>(&acc[32 * i]));
@@ -502,57 +492,23 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
               released = true;
             }
             [[maybe_unused]] const uint32_t bias_cur = (n - n0) >= 2 * kChunk ? bias_reg[1] : bias_reg[0];
+            pipe.begin();
             if constexpr (Tr::kF32Out) {
-              pipe.begin();
 #pragma unroll
               for (int j = 0; j < 8; ++j) pipe.put(j, make_uint4(acc[4 * j], acc[4 * j + 1], acc[4 * j + 2], acc[4 * j + 3]));
               pipe.commit(map0, n, row0, ep.beta != 0);
             } else {
-              if constexpr (EPI == EPI_BIAS_GELU_DUAL) {
-                pipe.begin();
-#pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                  float v[8];
-                  load8(&acc[8 * j], bias_cur, j, v);
-                  pipe.put(j, pack8(v));
-                }
-                pipe.commit(map0, n, row0, false);
-              }
-              pipe.begin();
 #pragma unroll
               for (int j = 0; j < 8; ++j) {
                 float v[8];
                 load8(&acc[8 * j], bias_cur, j, v);
-                if constexpr (EPI == EPI_BIAS_GELU || EPI == EPI_BIAS_GELU_DUAL) {
+                if constexpr (EPI == EPI_BIAS_GELU) {
 #pragma unroll
                   for (int i = 0; i < 8; ++i) v[i] = gelu_fwd<false>(v[i]);
                 }
-                if constexpr (EPI == EPI_DGELU) {
-                  const uint32_t zw[4] = {zraw[j].x, zraw[j].y, zraw[j].z, zraw[j].w};
-#pragma unroll
-                  for (int i = 0; i < 4; ++i) {
-                    v[2 * i] *= gelu_bwd<false>(bf16_lo(zw[i]));
-                    v[2 * i + 1] *= gelu_bwd<false>(bf16_hi(zw[i]));
-                  }
-                }
                 pipe.put(j, pack8(v));
               }
-              pipe.commit(EPI == EPI_BIAS_GELU_DUAL ? map1 : map0, n, row0, false);
-              if constexpr (EPI == EPI_DGELU) {
-                if (ep.colsum != nullptr) {   // db1 band sums from the staged bf16 values (gemm_sm100.cuh, step A4)
-                  const uint32_t src = pipe.committed_buf() + ((lane & 3) << 2);
-                  float s0 = 0.0f, s1 = 0.0f;
-#pragma unroll
-                  for (int r = 0; r < 32; ++r) {
-                    uint32_t w;
-                    asm volatile("ld.shared.b32 %0, [%1];" : "=r"(w) : "r"(src + r * 128 + ((((uint32_t)lane >> 2) ^ (r & 7)) << 4)));
-                    s0 += bf16_lo(w);
-                    s1 += bf16_hi(w);
-                  }
-                  const int c = n + 2 * lane;
-                  if (c < N) *reinterpret_cast<float2*>(ep.colsum + (int64_t)(row0 >> 5) * ep.ld_colsum + c) = make_float2(s0, s1);
-                }
-              }
+              pipe.commit(map0, n, row0, false);
             }
           }
         }
@@ -679,8 +635,6 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
         case kEpiFusedA34: run_fused(); break;
         case EPI_BIAS_GELU: run(std::integral_constant<int, EPI_BIAS_GELU>{}); break;
         case EPI_BIAS: run(std::integral_constant<int, EPI_BIAS>{}); break;
-        case EPI_BIAS_GELU_DUAL: run(std::integral_constant<int, EPI_BIAS_GELU_DUAL>{}); break;
-        case EPI_DGELU: run(std::integral_constant<int, EPI_DGELU>{}); break;
         case EPI_ACCUM_F32: run(std::integral_constant<int, EPI_ACCUM_F32>{}); break;
         default: run(std::integral_constant<int, EPI_PLAIN>{}); break;
       }

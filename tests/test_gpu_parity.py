@@ -94,10 +94,11 @@ def force_big_tiles(lib):
     """512 x 256 pair tiles (MT = 2) for every launch, whatever K and the tile count: the default build takes them
     only for long-K GEMMs that fill the machine (full-size tests), so the ragged small shapes would never see them."""
     keys = (lib.OSDP_TUNE_MT2_MIN_K, lib.OSDP_TUNE_MT2_MIN_TILES, lib.OSDP_TUNE_WAVE_SYNC, lib.OSDP_TUNE_BAND_MIB,
-            lib.OSDP_TUNE_CLUSTER_MIN_TILES)
+            lib.OSDP_TUNE_CLUSTER_MIN_TILES, lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES)
     old = {k: lib.osdp_get_tuning(k) for k in keys}
     lib.osdp_set_tuning(lib.OSDP_TUNE_MT2_MIN_K, 1)
     lib.osdp_set_tuning(lib.OSDP_TUNE_MT2_MIN_TILES, 1)
+    lib.osdp_set_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES, 0)   # small slices would take the one-kernel-per-slice path
     yield
     for k, v in old.items():
         lib.osdp_set_tuning(k, v)
@@ -206,7 +207,17 @@ def test_forward_backward_can_be_captured_in_a_cuda_graph(lib):
             assert np.array_equal(got[n].double().cpu().numpy(), want[axis][n]), (axis, n)
 
 
-def test_trace_records_every_launch_with_its_step(lib):
+@pytest.fixture
+def per_gemm_launches(lib):
+    """The launch-per-GEMM path for small slices too (by default they run as one kernel per slice,
+    tests/test_gpu_slice_kernel.py)."""
+    old = lib.osdp_get_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES)
+    lib.osdp_set_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES, 0)
+    yield
+    lib.osdp_set_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES, old)
+
+
+def test_trace_records_every_launch_with_its_step(lib, per_gemm_launches):
     """osdp_trace_*: one (step id, milliseconds) entry per kernel launch, in launch order, both split axes."""
     T, h, f, k = 600, 128, 512, 3
     d = I.mlp_inputs(T, h, f, torch.bfloat16, seed=17).to("cuda")
@@ -369,7 +380,7 @@ def test_error_codes(lib):
     assert lib.osdp_last_launch_count() == 0
 
 
-def test_backward_overwrites_and_accepts_null_b2(lib):
+def test_backward_overwrites_and_accepts_null_b2(lib, per_gemm_launches):
     """Reading S11 (overwrite, not accumulate) and S4 (b2 unused)."""
     T, h, f = 200, 64, 256
     inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=2)

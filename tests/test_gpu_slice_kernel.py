@@ -136,6 +136,18 @@ def test_slice_kernel_step_can_be_captured_in_a_cuda_graph(lib, slice_kernel):
         assert np.array_equal(got[n].double().cpu().numpy(), want[n]), n
 
 
+def test_default_threshold_takes_small_slices_only(lib):
+    """Default OSDP_TUNE_SLICE_KERNEL_MAX_TILES = 96 tiles of the [T_s x ffn] GEMMs: small slices run as one kernel per
+    slice, large ones keep one launch per GEMM."""
+    assert lib.osdp_get_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES) == 96
+    for (T, h, f, k), per_slice in (((2048, 256, 1024, 2), 1), ((8192, 512, 4096, 1), 6)):
+        d = I.mlp_inputs(T, h, f, torch.bfloat16, seed=36).to("cuda")
+        op = lib.SplitMlp(T, h, f, torch.bfloat16, k)
+        op.backward(d.X, d.W1, d.b1, d.W2, d.dY)
+        torch.cuda.synchronize()
+        assert lib.osdp_last_launch_count() == 2 + k * per_slice, (T, h, f, k)
+
+
 def test_slice_kernel_trace_and_fallback(lib, slice_kernel):
     """One traced launch per slice (steps 21 / 22); fp32 and over-sized calls keep the launch-per-GEMM path."""
     T, h, f, k = 600, 128, 512, 3
