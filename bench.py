@@ -679,6 +679,52 @@ def zdp_bench(args, lib, cfg):
     return 0
 
 
+def vendor_dw_bench(args, cfg):
+    """cuBLAS on the dW GEMM shapes (A5: [f x T_s] x [T_s x h], A6: [h x T_s] x [T_s x f]; bf16 operands, fp32 output,
+    beta = 0 and beta = 1), each timed in a ~2 s back-to-back loop.  A library reference for the dominant kernel's shape,
+    not part of the product path."""
+    T, h, f = cfg["tokens"], cfg["hidden"], cfg["ffn"]
+    ts = (T + args.k - 1) // args.k
+    peaks = load_peaks()
+
+    def sustained(fn, secs=2.0):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(10):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        n = max(10, int(secs * 1e3 / (e0.elapsed_time(e1) / 10)))
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n
+
+    rows = []
+    for name, (m, n) in (("A5 dW2 = H_s^T dY_s", (f, h)), ("A6 dW1 = X_s^T dZ_s", (h, f))):
+        a = torch.randn(ts, m, device="cuda", dtype=torch.bfloat16)
+        b = torch.randn(ts, n, device="cuda", dtype=torch.bfloat16)
+        c = torch.zeros(m, n, device="cuda", dtype=torch.float32)
+        flops = 2.0 * m * n * ts
+        ms0 = sustained(lambda: torch.mm(a.t(), b, out_dtype=torch.float32, out=c))
+        ms1 = sustained(lambda: torch.addmm(c, a.t(), b, out_dtype=torch.float32, out=c))
+        rows.append({"gemm": name, "M": m, "N": n, "K": ts, "beta0_ms": ms0, "beta0_tflops": flops / ms0 / 1e9,
+                     "beta1_ms": ms1, "beta1_tflops": flops / ms1 / 1e9})
+        del a, b, c
+    sus = peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"])
+    print(json.dumps({"what": "cuBLAS (torch.mm / torch.addmm, out_dtype = fp32) on the dW GEMM shapes, ~2 s back-to-back loops",
+                      "config": {"workload": workload_name(args, cfg), "k": args.k, "slice_tokens": ts}, "rows": rows,
+                      "peak_bf16_sustained_tflops": sus,
+                      "frac_of_sustained_beta1": [r["beta1_tflops"] / sus for r in rows]}))
+    return 0
+
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -706,6 +752,13 @@ def main():
     ap.add_argument("--stack", action="store_true",
                     help="with --config C5: instead of the bench line, run the 24-layer MLP stack with the split count "
                          "per layer chosen by osdp_plan from gamma/delta calibrated on this GPU (BASELINE.json config 5)")
+    ap.add_argument("--slice-kernel-max-tiles", type=int, default=None, metavar="N",
+                    help="set OSDP_TUNE_SLICE_KERNEL_MAX_TILES before the run (0 = one launch per GEMM for small slices too; "
+                         "library default 96): the A/B of the one-kernel-per-slice path")
+    ap.add_argument("--vendor-dw", action="store_true",
+                    help="instead of the bench line: the vendor library (cuBLAS through torch.mm / torch.addmm, fp32 output) "
+                         "on the shapes of the dW GEMMs A5 / A6 of --config at --k, timed back to back for ~2 s each "
+                         "(sustained, power-capped): the context for the dominant kernel's roofline fraction")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -720,12 +773,16 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the osdp-b200 hot path has no CPU fallback")
     from paper_2305_09940_b200 import binding as lib     # raises if the library was not built
+    if args.slice_kernel_max_tiles is not None:
+        lib.osdp_set_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES, args.slice_kernel_max_tiles)
     if args.granularity_sweep:
         return granularity_sweep(args, lib)
     if args.stack:
         return stack_bench(args, lib, cfg)
     if args.zdp:
         return zdp_bench(args, lib, cfg)
+    if args.vendor_dw:
+        return vendor_dw_bench(args, cfg)
     from paper_2305_09940_b200 import dist as D
     world, rank, local = D.init("nccl")
     peaks = load_peaks()
@@ -870,7 +927,8 @@ def main():
                 "vs_baseline": None, "dtype": cfg["dtype"], "data": "synthetic",
                 "config": {"workload": workload_name(args, cfg), "tokens_per_gpu": T, "hidden": h, "ffn": f,
                            "k": args.k, "split_axis": args.axis, "flops_per_step": flops, "flops_counted": "14*T*h*f executed (12*T*h*f model)",
-                           "l2": l2_note, "parallelism": f"dp{world} (independent token batches, no collective)"},
+                           "l2": l2_note, "parallelism": f"dp{world} (independent token batches, no collective)",
+                           "slice_kernel_max_tiles": lib.osdp_get_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES)},
                 "value_model_flops_12x": value * 12.0 / 14.0,
                 "frac_of_sustained_peak": value / world / peak if peak else None,
                 "frac_of_nominal_peak": value / world / NOMINAL_BF16_TFLOPS,

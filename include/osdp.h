@@ -210,7 +210,7 @@ typedef enum osdp_tune_key {
                                       C5 layer shape, neutral to -1 % at C3 / C4, which the default excludes); 0 = always
                                       in sequence */
   OSDP_TUNE_SLICE_KERNEL_MAX_TILES = 7
-                                   /* default 96.  Token split, bf16: when the [T_s x ffn] GEMMs of a slice have at most
+                                   /* default 128.  Token split, bf16: when the [T_s x ffn] GEMMs of a slice have at most
                                       this many 256 x 256 output tiles (small slices: about one wave), the whole slice
                                       runs as ONE persistent kernel (forward A1 -> A2; backward (A3 + A4 fused per tile)
                                       -> A7 | A5 | A6 and the db1 sum): CTA pairs claim tiles of all GEMMs from one list

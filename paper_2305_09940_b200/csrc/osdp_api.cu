@@ -254,8 +254,9 @@ inline int64_t tiles_256(int64_t m, int64_t n) { return ((m + 255) / 256) * ((n 
 // ---- one persistent kernel per slice (slice_sm100.cuh) ----------------------------------------------------------
 // Taken for bf16 when the slice is small in TOKENS: its [T_s x ffn] GEMMs (A1, A3, A4) have at most
 // OSDP_TUNE_SLICE_KERNEL_MAX_TILES tiles of 256 x 256, i.e. about one wave, which is where a launch per GEMM is mostly
-// fill and drain (measured crossover: C2 k = 4 / C5 layer k = 16 at 128 tiles break even, 64 tiles gain 8-26 %; the dW
-// GEMMs' tile count does not matter), and the call's flags fit the per-call block.  A2 / A7 (long contraction, few
+// fill and drain (measured: at 128 tiles C2 k = 4 +7 %, C5 layer k = 16 +1 %, C4 k = 32 +6 %; at 64 tiles +10-27 %; at 256
+// tiles the launch-per-GEMM path with its 512 x 256 tiles wins; the dW GEMMs' tile count does not matter), and the call's
+// flags fit the per-call block.  A2 / A7 (long contraction, few
 // output tiles) take 128-column tiles when that still fits one wave of CTA pairs, so they spread over twice as many SMs.
 struct SlicePlan {
   bool use = false;
@@ -269,11 +270,11 @@ int slice_plan(const osdp_mlp_desc* d, int pass, SlicePlan* out) {
   sm100::DeviceInfo dev;
   OSDP_TRY(sm100::current_device(&dev));
   const int64_t ts = (d->tokens + d->k - 1) / d->k;
-  const int64_t t_tf = tiles_256(ts, d->ffn), t_th = tiles_256(ts, d->hidden), t_fh = tiles_256(d->ffn, d->hidden);
+  (void)pass;
+  const int64_t t_tf = tiles_256(ts, d->ffn), t_th = tiles_256(ts, d->hidden);
   if (t_tf > max_tiles) return OSDP_OK;
   out->bn_narrow = 2 * t_th <= dev.sms / 2 ? 128 : 256;
-  const int64_t t_narrow = ((ts + 255) / 256) * ((d->hidden + out->bn_narrow - 1) / out->bn_narrow);
-  const int64_t per_slice = sm100::kSliceFlags0 + 2 * (pass == OSDP_FWD ? t_tf + t_narrow : 2 * t_tf + t_narrow + 2 * t_fh);
+  const int64_t per_slice = sm100::kSliceFlags0 + 2 * t_tf;   // flags of the publishing phase (A1 / fused A3 + A4) only
   if (per_slice * d->k > sm100::kSliceSyncWords) return OSDP_OK;
   out->use = true;
   out->words_per_slice = (int)per_slice;

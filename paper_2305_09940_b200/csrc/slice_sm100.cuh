@@ -46,8 +46,8 @@ namespace sm100 {
 
 constexpr int kSliceMaxPhases = 5;
 constexpr int kSliceQueue = 4;              // tile indices a pair may hold ahead of its epilogue
-constexpr int kSliceCallSlots = 32;         // calls in flight on one device that get separate counters
-constexpr int kSliceSyncWords = 16384;      // words per call: k x (2 + 2 x tiles of a slice) must fit
+constexpr int kSliceCallSlots = 16;         // calls in flight on one device that get separate counters
+constexpr int kSliceSyncWords = 32768;      // words per call: k x (kSliceFlags0 + 2 x publishing tiles of a slice) must fit
 constexpr unsigned int kPublishersPerTile = 2 * kNumEpiWarps;   // arrivals that hand a TMEM stage back
 constexpr int kSliceFlags0 = 4;             // first flag word of a launch's part of the array
 // A3 and A4 of the backward in one tile (they have the same output tile grid): accumulator 0 = X_s W1, accumulator 1 =
@@ -80,6 +80,7 @@ struct SlicePhase {
 };
 struct SliceParams {
   int num_phases, total_tiles;
+  int flag_tiles;      // tiles that have flags: list indices below this (the publishing phases come first in the list)
   unsigned int* sync;  // [0]: next list index to claim; [1]: pairs that have drawn their sentinel; [2]: CTAs that have left;
                        // [kSliceFlags0 + 2 t + r]: epoch once CTA r of the owning pair has published tile t
   unsigned int epoch;  // this launch's flag value (never 0; no two launches that can see the same flags share one)
@@ -680,7 +681,7 @@ mlp_slice_kernel(const __grid_constant__ SliceMaps maps, const __grid_constant__
     unsigned int last = 0;
     if (lane == 0) last = atomicAdd(P.sync + 2, 1u) == gridDim.x - 1 ? 1u : 0u;
     if (__shfl_sync(0xFFFFFFFFu, last, 0)) {
-      for (int i = lane; i < 2 * P.total_tiles; i += 32) flags[i] = 0u;
+      for (int i = lane; i < 2 * P.flag_tiles; i += 32) flags[i] = 0u;
       if (lane == 0) P.sync[2] = 0u;
     }
   }
@@ -768,6 +769,10 @@ inline int launch_mlp_slice(const SliceGemm* g, int n, unsigned int* sync, unsig
     S.fused = G.epi == kEpiFusedA34 ? 1 : 0;
     S.ep = G.ep;
     tiles += S.num_m * S.num_n;
+    if (G.publish) {
+      if (P.flag_tiles != S.tile_begin) return OSDP_ERR_ARG;   // publishing phases must lead the list
+      P.flag_tiles = tiles;
+    }
     int rc;
     if (G.a_major == MAJOR_K) rc = make_tmap(&maps.m[p][0], G.A, G.s.K, G.s.M, G.lda, BLOCK_K, BLOCK_M);
     else                      rc = make_tmap(&maps.m[p][0], G.A, G.s.M, G.s.K, G.lda, 64, BLOCK_K);

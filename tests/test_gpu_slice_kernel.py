@@ -137,9 +137,9 @@ def test_slice_kernel_step_can_be_captured_in_a_cuda_graph(lib, slice_kernel):
 
 
 def test_default_threshold_takes_small_slices_only(lib):
-    """Default OSDP_TUNE_SLICE_KERNEL_MAX_TILES = 96 tiles of the [T_s x ffn] GEMMs: small slices run as one kernel per
+    """Default OSDP_TUNE_SLICE_KERNEL_MAX_TILES = 128 tiles of the [T_s x ffn] GEMMs: small slices run as one kernel per
     slice, large ones keep one launch per GEMM."""
-    assert lib.osdp_get_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES) == 96
+    assert lib.osdp_get_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES) == 128
     for (T, h, f, k), per_slice in (((2048, 256, 1024, 2), 1), ((8192, 512, 4096, 1), 6)):
         d = I.mlp_inputs(T, h, f, torch.bfloat16, seed=36).to("cuda")
         op = lib.SplitMlp(T, h, f, torch.bfloat16, k)
