@@ -165,3 +165,47 @@ def test_slice_kernel_trace_and_fallback(lib, slice_kernel):
     op32 = lib.SplitMlp(96, 32, 64, torch.float32, 2)
     op32.forward(d32.X, d32.W1, d32.b1, d32.W2, d32.b2)
     assert lib.osdp_last_launch_count() == 2 * 2               # fp32: one launch per GEMM
+
+
+def test_many_tiny_slices_pipeline_and_single_buffer_forward(lib, slice_kernel):
+    """k = 64 slices of 24 tokens: 64 forward launches that alternate the two H_s buffers without waiting for each other
+    (late programmatic wait), 64 backward launches with their own flags; and the forward with its own minimum workspace
+    (one H_s buffer: slices strictly in sequence) gives the same bits."""
+    T, h, f, k = 1536, 264, 520, 64
+    inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=37)
+    ref = O.mlp_forward_backward(**inp.as_f64())
+    got = run_gpu(lib, inp, k)
+    errs = {n: rel_err(got[n], ref[n]) for n in NAMES}
+    assert all(e <= 2e-2 for e in errs.values()), errs
+    want = per_gemm(lib, lambda: run_gpu(lib, inp, k))
+    for n in NAMES:
+        assert np.array_equal(got[n], want[n]), n
+    d = inp.to("cuda")
+    desc = lib.make_desc(T, h, f, torch.bfloat16, k)
+    nbytes = lib.osdp_split_mlp_workspace_bytes(desc, lib.OSDP_FWD)
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    for _ in range(3):                                          # back to back: the next call's first slice waits for this one
+        Y = torch.empty_like(d.X)
+        lib.osdp_split_mlp_forward(desc, d.X, d.W1, d.b1, d.W2, d.b2, Y, ws, workspace_bytes=nbytes)
+    torch.cuda.synchronize()
+    assert lib.osdp_last_launch_count() == k
+    assert np.array_equal(Y.double().cpu().numpy(), got["Y"])
+
+
+def test_back_to_back_steps_reuse_buffers_safely(lib, slice_kernel):
+    """Forward, backward, forward, ... on one stream with one workspace: the pipelined forward of step i + 1 must not
+    touch the buffers the backward of step i still reads (the first slice of every call waits for everything before it)."""
+    T, h, f, k = 2048, 512, 2048, 4
+    inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=38)
+    want = run_gpu(lib, inp, k)
+    d = inp.to("cuda")
+    op = lib.SplitMlp(T, h, f, torch.bfloat16, k)
+    outs = []
+    for _ in range(6):
+        Y = op.forward(d.X, d.W1, d.b1, d.W2, d.b2)
+        g = op.backward(d.X, d.W1, d.b1, d.W2, d.dY)
+        outs.append(dict(Y=Y, **g))
+    torch.cuda.synchronize()
+    for o in outs:
+        for n in NAMES:
+            assert np.array_equal(o[n].double().cpu().numpy(), want[n]), n
