@@ -116,6 +116,11 @@ __global__ void __launch_bounds__(F32_THREADS) gemm_f32_kernel(StridedOperands o
     }
   };
 
+  // Programmatic dependent launch: the index arithmetic above overlapped the tail of the previous kernel of the stream;
+  // from here on this kernel reads what that kernel wrote.  These launches are a few microseconds each and several CTAs
+  // fit an SM, so the next kernel's CTAs are resident and waiting here when the previous grid completes.
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   float acc[4][4] = {};
   int buf = 0;
   if (k_begin < k_end) {
@@ -193,13 +198,15 @@ inline int launch_gemm_f32(const StridedOperands& op, const GemmShape& s, const 
   cfg.gridDim = dim3((unsigned)(tiles_m * tiles_n * split));
   cfg.blockDim = dim3(F32_THREADS);
   cfg.stream = st;
-  cudaLaunchAttribute attr[1];
+  cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = (unsigned)split;
   attr[0].val.clusterDim.y = 1;
   attr[0].val.clusterDim.z = 1;
+  attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // see griddepcontrol in the kernel
+  attr[1].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
-  cfg.numAttrs = 1;
+  cfg.numAttrs = 2;
   cudaError_t err;
   {
     LaunchTrace tr(st);
