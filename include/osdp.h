@@ -14,7 +14,9 @@
  *     accumulate in fp32.  dW1, dW2, db1, db2 are ALWAYS fp32.
  *   - "device pointer" = CUDA device memory of the current device, owned by the caller, 16-byte aligned
  *     (workspace: 256-byte aligned).  The library never allocates, frees or synchronises device memory; it
- *     only enqueues work on `stream` (a cudaStream_t passed as void*; NULL = the legacy default stream).
+ *     only enqueues work on `stream` (a cudaStream_t passed as void*; NULL = the legacy default stream).  Its own
+ *     device state is static (module memory: wave-sync counters, 2 MiB of tile flags of the one-kernel-per-slice path;
+ *     up to 16 calls of that path in flight on one device get separate flags).
  *     Outputs must not alias inputs or each other.
  *   - Every call returns an osdp_status; OSDP_OK = 0.  Nothing is printed, nothing aborts.  On any error
  *     before the first launch the outputs are untouched.
