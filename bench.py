@@ -755,6 +755,9 @@ def main():
     ap.add_argument("--slice-kernel-max-tiles", type=int, default=None, metavar="N",
                     help="set OSDP_TUNE_SLICE_KERNEL_MAX_TILES before the run (0 = one launch per GEMM for small slices too; "
                          "library default 96): the A/B of the one-kernel-per-slice path")
+    ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
+                    help="osdp_set_tuning before the run, e.g. --tune mt2_min_k=2048 (keys: the OSDP_TUNE_* names of "
+                         "include/osdp.h in lower case without the prefix); for A/B runs of the kernel-selection knobs")
     ap.add_argument("--vendor-dw", action="store_true",
                     help="instead of the bench line: the vendor library (cuBLAS through torch.mm / torch.addmm, fp32 output) "
                          "on the shapes of the dW GEMMs A5 / A6 of --config at --k, timed back to back for ~2 s each "
@@ -775,6 +778,9 @@ def main():
     from paper_2305_09940_b200 import binding as lib     # raises if the library was not built
     if args.slice_kernel_max_tiles is not None:
         lib.osdp_set_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES, args.slice_kernel_max_tiles)
+    for kv in args.tune:
+        key, _, val = kv.partition("=")
+        lib.osdp_set_tuning(getattr(lib, "OSDP_TUNE_" + key.strip().upper()), int(val))
     if args.granularity_sweep:
         return granularity_sweep(args, lib)
     if args.stack:
