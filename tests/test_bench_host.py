@@ -47,3 +47,15 @@ def test_reference_arm_prints_one_json_line_on_cpu():
     d = json.loads(lines[0])
     assert d["impl"] == "reference" and d["cpu_baseline"]["kind"] == "oracle" and d["value"] > 0
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["gpu_launches"] == 0 and d["vs_baseline"] is None
+
+
+def test_gemms_per_traced_launch_cover_the_slice_kernel_steps():
+    """The trace step ids of the one-kernel-per-slice path carry 2 (forward) and 5 (backward) GEMMs of 2 T_s h f flops each;
+    the per-GEMM steps A1-A7 one.  bench.py divides by these for the per-launch TFLOP/s and the roofline fraction."""
+    import bench
+    assert bench.GEMMS_PER_LAUNCH[21] == 2 and bench.GEMMS_PER_LAUNCH[22] == 5
+    assert all(bench.GEMMS_PER_LAUNCH[s] == 1 for s in range(1, 8))
+    assert 8 not in bench.GEMMS_PER_LAUNCH and 10 not in bench.GEMMS_PER_LAUNCH      # column sums, accumulator -> output
+    # a whole step = k x (2 + 5) GEMMs = 14 T h f
+    T, h, f, k = 8192, 1024, 4096, 8
+    assert k * (bench.GEMMS_PER_LAUNCH[21] + bench.GEMMS_PER_LAUNCH[22]) * 2.0 * (T // k) * h * f == bench.executed_flops(T, h, f)
