@@ -294,6 +294,23 @@ def test_library_exports_every_declared_symbol(lib):
     assert "sm_100a" in lib.osdp_version()
 
 
+def test_tuning_keys_of_header_binding_and_library_agree(lib):
+    """Every OSDP_TUNE_* key of include/osdp.h has the same value in the binding, and the library knows it (get / set run
+    on the host: no GPU needed)."""
+    import re
+    hdr = open(os.path.join(os.path.dirname(GOLDEN), "..", "include", "osdp.h")).read()
+    keys = dict((n, int(v)) for n, v in re.findall(r"\b(OSDP_TUNE_[A-Z0-9_]+)\s*=\s*(\d+)", hdr))
+    assert len(keys) == 8 and sorted(keys.values()) == list(range(8))
+    for name, val in keys.items():
+        assert getattr(lib, name) == val, name
+        cur = lib.osdp_get_tuning(val)
+        assert cur >= 0, name
+        lib.osdp_set_tuning(val, cur)                                  # round trip leaves the default in place
+        assert lib.osdp_get_tuning(val) == cur
+    assert lib.osdp_get_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES) == 128
+    assert lib.osdp_get_tuning(len(keys)) == -1
+
+
 def test_cost_eval_matches_oracle(lib):
     rng = random.Random(5)
     for op in _ops(20, 3):
