@@ -211,7 +211,7 @@ typedef enum osdp_tune_key {
                                       (small slices: every launch is a wave or two; measured +4-8 % at C2, +5 % at the
                                       C5 layer shape, neutral to -1 % at C3 / C4, which the default excludes); 0 = always
                                       in sequence */
-  OSDP_TUNE_SLICE_KERNEL_MAX_TILES = 7
+  OSDP_TUNE_SLICE_KERNEL_MAX_TILES = 7,
                                    /* default 128.  Token split, bf16: when the [T_s x ffn] GEMMs of a slice have at most
                                       this many 256 x 256 output tiles (small slices: about one wave), the whole slice
                                       runs as ONE persistent kernel (forward A1 -> A2; backward (A3 + A4 fused per tile)
@@ -221,6 +221,12 @@ typedef enum osdp_tune_key {
                                       If the workspace passed to the forward has room for two slice buffers (the
                                       backward's size), consecutive forward slices alternate buffers and overlap.
                                       0 = never */
+  OSDP_TUNE_SLICE_KERNEL_FFN_MAX_TILES = 8
+                                   /* default 0 (off).  The same path for the ffn-axis split (osdp_ffn_split_mlp_*), taken
+                                      when the [tokens x f_s] GEMMs of a slice have at most this many 256 x 256 tiles.
+                                      Bit-identical results; faster for many narrow slices of a long token axis (C3
+                                      k = 64 +35 %, C5 layer shape k = 16 / 32 +31 / +37 %), slower on C2 and on C4 at
+                                      k = 32 (-10 ... -17 %), hence opt-in */
 } osdp_tune_key;
 int osdp_set_tuning(int key, int64_t value);
 int64_t osdp_get_tuning(int key);

@@ -55,6 +55,7 @@ struct Tuning {
   std::atomic<int64_t> band_mib{0};         // 0: square-wave raster bands; > 0: band = tile rows whose A rows fit this many MiB of L2
   std::atomic<int64_t> cluster_min_tiles{0};   // > 0: multicast clusters for launches of at least this many pair tiles
   std::atomic<int64_t> fork_max_tiles{256};    // backward: A5 | A6 | A7 | column sums run concurrently when each GEMM has at most this many 256 x 256 tiles
+  std::atomic<int64_t> slice_kernel_ffn_max_tiles{0};   // the same for the ffn-axis split ([T x f_s] GEMMs); off by default: wins and losses are mixed
   std::atomic<int64_t> slice_kernel_max_tiles{128}; // token split: one persistent kernel per slice (slice_sm100.cuh) when the slice's [T_s x ffn] GEMMs have at most this many 256 x 256 tiles; 0 = never
 };
 inline Tuning& tuning() {

@@ -282,6 +282,32 @@ int slice_plan(const osdp_mlp_desc* d, int pass, SlicePlan* out) {
   return OSDP_OK;
 }
 
+// The same for the ffn-axis split: a slice is ffn columns [lo, hi), its [T x fs] GEMMs (A1 / A3 + A4) decide.  Its own
+// knob, off by default: measured C3 k = 64 +35 %, C5 layer shape k = 16 / 32 +31 / +37 %, but C2 k = 4 / 8 -17 / -15 % and C4
+// k = 32 -10 % (the slice's dW GEMMs are few tiles with K = T, and they then run beside the dX tiles instead of alone).
+int ffn_slice_plan(const osdp_mlp_desc* d, int64_t fs_max, SlicePlan* out) {
+  *out = SlicePlan{};
+  const int64_t max_tiles = sm100::tuning().slice_kernel_ffn_max_tiles.load();
+  if (d->dtype != OSDP_BF16 || max_tiles <= 0) return OSDP_OK;
+  sm100::DeviceInfo dev;
+  OSDP_TRY(sm100::current_device(&dev));
+  const int64_t t_tf = tiles_256(d->tokens, fs_max), t_th = tiles_256(d->tokens, d->hidden);
+  if (t_tf > max_tiles) return OSDP_OK;
+  out->bn_narrow = 2 * t_th <= dev.sms / 2 ? 128 : 256;
+  const int64_t per_slice = sm100::kSliceFlags0 + 2 * t_tf;
+  if (per_slice * d->k > sm100::kSliceSyncWords) return OSDP_OK;
+  out->use = true;
+  out->words_per_slice = (int)per_slice;
+  out->words = (int)(per_slice * d->k);
+  return OSDP_OK;
+}
+// One-kernel-per-slice launch context of an ffn-split call (sync == nullptr: one launch per GEMM)
+struct FfnSliceKernel {
+  unsigned int* sync = nullptr;   // this slice's flags
+  unsigned int epoch = 0;
+  int bn_narrow = 256;
+};
+
 // ---- one slice of the ffn-axis split.  The slice's weights are given by pointer + leading
 // dimension, so the same code serves weights sliced in place (W1 + lo, ld = f) and gathered slice buffers (ZDP, ld = fs).
 struct FfnSliceW {
@@ -298,7 +324,20 @@ struct FfnSliceG {
 };
 // H_s = gelu(X W1s + b1s); Y (+)= H_s W2s.  single = the operator has one slice (Y written directly, + b2).
 int ffn_slice_forward(int dt, int64_t T, int64_t h, int fs, const void* X, const FfnSliceW& w, const void* b2, void* Y,
-                      void* Hs, float* Yacc, bool single, bool first, cudaStream_t st) {
+                      void* Hs, float* Yacc, bool single, bool first, cudaStream_t st, const FfnSliceKernel* sk = nullptr) {
+  if (sk && sk->sync) {   // A1 -> A2 in one launch (slice_sm100.cuh); Y (+)= goes through the fp32 reduce-add epilogue
+    trace_set_step(21);
+    sm100::SliceGemm g[2] = {};
+    g[0] = {X, h, w.W1s, w.ldw1, MAJOR_K, MAJOR_MN, EPI_BIAS_GELU, GemmShape{(int)T, fs, (int)h},
+            EpiParams{w.b1s, Hs, nullptr, nullptr, fs, 0}, sm100::DEP_NONE, 0, 256, 1, 0};
+    if (single)
+      g[1] = {Hs, fs, w.W2s, h, MAJOR_K, MAJOR_MN, EPI_BIAS, GemmShape{(int)T, (int)h, fs},
+              EpiParams{b2, Y, nullptr, nullptr, h, 0}, sm100::DEP_ROW, 0, sk->bn_narrow, 0, 0};
+    else
+      g[1] = {Hs, fs, w.W2s, h, MAJOR_K, MAJOR_MN, EPI_ACCUM_F32, GemmShape{(int)T, (int)h, fs},
+              EpiParams{nullptr, Yacc, nullptr, nullptr, h, first ? 0 : 1}, sm100::DEP_ROW, 0, 256, 0, 0};
+    return sm100::launch_mlp_slice(g, 2, sk->sync, sk->epoch, nullptr, false, st);
+  }
   trace_set_step(1);
   EpiParams e1 = {w.b1s, Hs, nullptr, nullptr, fs, 0};
   OSDP_TRY((gemm<MAJOR_K, MAJOR_MN, EPI_BIAS_GELU>(dt, X, h, w.W1s, w.ldw1, GemmShape{(int)T, fs, (int)h}, e1, st)));
@@ -317,7 +356,33 @@ int ffn_slice_forward(int dt, int64_t T, int64_t h, int fs, const void* X, const
 // db2 != nullptr: also db2 = colsum(dY) (once per call, with the first slice).
 int ffn_slice_backward(int dt, int64_t T, int64_t h, int fs, const void* X, const void* dY, const FfnSliceW& w,
                        const FfnSliceG& g, void* Zs, void* Hs, void* dX, float* dXacc, float* scratch1, float* scratch2,
-                       float* db2, bool single, bool first, cudaStream_t st) {
+                       float* db2, bool single, bool first, cudaStream_t st, const FfnSliceKernel* sk = nullptr) {
+  if (sk && sk->sync) {   // (A3 + A4) -> A7 | A5 | A6 (+ db1) in one launch; the slice's dW / db1 parts are written once
+    if (db2) {
+      trace_set_step(8);
+      OSDP_TRY(colsum_rows(dt, dY, (int)h, db2, (int)T, scratch2, 0, st));
+    }
+    trace_set_step(22);
+    sm100::SliceGemm ph[4] = {};
+    ph[0] = {X, h, w.W1s, w.ldw1, MAJOR_K, MAJOR_MN, sm100::kEpiFusedA34, GemmShape{(int)T, fs, (int)h},
+            EpiParams{w.b1s, Zs, Hs, nullptr, fs, 0, scratch1, fs}, sm100::DEP_NONE, 0, 256, 1, 0,
+            dY, h, w.W2s, h, MAJOR_K, MAJOR_K, (int)h};
+    // list order = claim order: everything after the fused tiles is ready at the same time, so the phase with the
+    // longest contraction (fewest, longest tiles) goes first: here usually the dW GEMMs (K = T), dX (K = fs) fills in
+    const int ix = T > fs ? 3 : 1, i5 = T > fs ? 1 : 2, i6 = T > fs ? 2 : 3;
+    if (single)
+      ph[ix] = {Zs, fs, w.W1s, w.ldw1, MAJOR_K, MAJOR_K, EPI_PLAIN, GemmShape{(int)T, (int)h, fs},
+                EpiParams{nullptr, dX, nullptr, nullptr, h, 0}, sm100::DEP_ROW, 0, sk->bn_narrow, 0, 0};
+    else
+      ph[ix] = {Zs, fs, w.W1s, w.ldw1, MAJOR_K, MAJOR_K, EPI_ACCUM_F32, GemmShape{(int)T, (int)h, fs},
+                EpiParams{nullptr, dXacc, nullptr, nullptr, h, first ? 0 : 1}, sm100::DEP_ROW, 0, 256, 0, 0};
+    ph[i5] = {Hs, fs, dY, h, MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32, GemmShape{fs, (int)h, (int)T},
+              EpiParams{nullptr, g.dW2s, nullptr, nullptr, h, 0}, sm100::DEP_COL_AS_M, 0, 256, 0, 0};
+    ph[i6] = {X, h, Zs, fs, MAJOR_MN, MAJOR_MN, EPI_ACCUM_F32, GemmShape{(int)h, fs, (int)T},
+              EpiParams{nullptr, g.dW1s, nullptr, nullptr, g.ldg1, 0}, sm100::DEP_COL_AS_N, 0, 256, 0, 1};
+    const sm100::SliceDb1 dj = {scratch1, fs, g.db1s, (int)((T + kBandRows - 1) / kBandRows), 0};
+    return sm100::launch_mlp_slice(ph, 4, sk->sync, sk->epoch, &dj, false, st);
+  }
   // dW2, dW1, dX (+)= and the column sums only need dZ_s: side by side on small slices (helper streams above)
   const int64_t fork_max = sm100::tuning().fork_max_tiles.load();
   const bool fork = fork_max > 0 && tiles_256(fs, h) <= fork_max && tiles_256(T, h) <= fork_max;
@@ -416,6 +481,10 @@ int osdp_set_tuning(int key, int64_t value) {
       if (value < 0) return OSDP_ERR_ARG;
       t.slice_kernel_max_tiles = value;
       return OSDP_OK;
+    case OSDP_TUNE_SLICE_KERNEL_FFN_MAX_TILES:
+      if (value < 0) return OSDP_ERR_ARG;
+      t.slice_kernel_ffn_max_tiles = value;
+      return OSDP_OK;
     default: return OSDP_ERR_ARG;
   }
 }
@@ -431,6 +500,7 @@ int64_t osdp_get_tuning(int key) {
     case OSDP_TUNE_MT2_MIN_K_ACC: return t.mt2_min_k_acc;
     case OSDP_TUNE_FORK_MAX_TILES: return t.fork_max_tiles;
     case OSDP_TUNE_SLICE_KERNEL_MAX_TILES: return t.slice_kernel_max_tiles;
+    case OSDP_TUNE_SLICE_KERNEL_FFN_MAX_TILES: return t.slice_kernel_ffn_max_tiles;
     default: return -1;
   }
 }
@@ -712,6 +782,11 @@ int osdp_ffn_split_mlp_forward(const osdp_mlp_desc* desc, const void* X, const v
   const int dt = desc->dtype, k = desc->k;
   void* Hs = workspace;
   float* Yacc = (float*)((char*)workspace + ffn_slice_buf_bytes(desc));
+  SlicePlan sp;
+  OSDP_TRY(ffn_slice_plan(desc, ffn_slice_max(desc), &sp));
+  unsigned int* sync = nullptr;
+  unsigned int epoch0 = 0;
+  if (sp.use) OSDP_TRY(sm100::slice_sync_acquire(sp.words, k, &sync, &epoch0));
 
   for (int s = 0; s < k; ++s) {
     const int64_t lo = ffn_lo(desc, s), hi = ffn_lo(desc, s + 1);
@@ -719,7 +794,9 @@ int osdp_ffn_split_mlp_forward(const osdp_mlp_desc* desc, const void* X, const v
     if (fs == 0) continue;   // cannot happen for k <= units; kept for symmetry with the token split
     const FfnSliceW w = {(const char*)W1 + (size_t)lo * e, desc->ffn, (const char*)b1 + (size_t)lo * e,
                          (const char*)W2 + (size_t)lo * h * e};
-    OSDP_TRY(ffn_slice_forward(dt, T, h, fs, X, w, b2, Y, Hs, Yacc, k == 1, s == 0, st));
+    FfnSliceKernel sk;
+    if (sp.use) sk = FfnSliceKernel{sync + (size_t)s * sp.words_per_slice, epoch0 + (unsigned int)s, sp.bn_narrow};
+    OSDP_TRY(ffn_slice_forward(dt, T, h, fs, X, w, b2, Y, Hs, Yacc, k == 1, s == 0, st, &sk));
   }
   if (k > 1) {   // Y = storage(Yacc + b2)
     trace_set_step(10);
@@ -752,6 +829,11 @@ int osdp_ffn_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const 
   float* dXacc = (float*)((char*)workspace + 2 * buf);   // fp32 accumulator of dX        [T x h]   (k > 1)
   float* scratch1 = (float*)((char*)workspace + 2 * buf + ffn_acc_bytes(desc));                      // db1 band partials
   float* scratch2 = (float*)((char*)scratch1 + db1_scratch_bytes(T, ffn_slice_max(desc)));           // db2 chunk partials
+  SlicePlan sp;
+  OSDP_TRY(ffn_slice_plan(desc, ffn_slice_max(desc), &sp));
+  unsigned int* sync = nullptr;
+  unsigned int epoch0 = 0;
+  if (sp.use) OSDP_TRY(sm100::slice_sync_acquire(sp.words, k, &sync, &epoch0));
 
   for (int s = 0; s < k; ++s) {
     const int64_t lo = ffn_lo(desc, s), hi = ffn_lo(desc, s + 1);
@@ -760,8 +842,10 @@ int osdp_ffn_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const 
     const FfnSliceW w = {(const char*)W1 + (size_t)lo * e, f, (const char*)b1 + (size_t)lo * e,
                          (const char*)W2 + (size_t)lo * h * e};
     const FfnSliceG g = {dW1 + lo, f, db1 + lo, dW2 + (size_t)lo * h};
+    FfnSliceKernel sk;
+    if (sp.use) sk = FfnSliceKernel{sync + (size_t)s * sp.words_per_slice, epoch0 + (unsigned int)s, sp.bn_narrow};
     OSDP_TRY(ffn_slice_backward(dt, T, h, fs, X, dY, w, g, Zs, Hs, dX, dXacc, scratch1, scratch2, s == 0 ? db2 : nullptr,
-                                k == 1, s == 0, st));
+                                k == 1, s == 0, st, &sk));
   }
   if (k > 1) {   // dX = storage(dXacc)
     trace_set_step(10);

@@ -34,19 +34,25 @@ def rel_err(got, ref):
 @pytest.fixture
 def slice_kernel(lib):
     """Slice kernel for every eligible shape (the default threshold only takes small slices)."""
-    old = lib.osdp_get_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES)
-    lib.osdp_set_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES, 1 << 20)
+    keys = (lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES, lib.OSDP_TUNE_SLICE_KERNEL_FFN_MAX_TILES)
+    old = [lib.osdp_get_tuning(k) for k in keys]
+    for k in keys:
+        lib.osdp_set_tuning(k, 1 << 20)
     yield
-    lib.osdp_set_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES, old)
+    for k, v in zip(keys, old):
+        lib.osdp_set_tuning(k, v)
 
 
 def per_gemm(lib, fn):
-    old = lib.osdp_get_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES)
-    lib.osdp_set_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES, 0)
+    keys = (lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES, lib.OSDP_TUNE_SLICE_KERNEL_FFN_MAX_TILES)
+    old = [lib.osdp_get_tuning(k) for k in keys]
+    for k in keys:
+        lib.osdp_set_tuning(k, 0)
     try:
         return fn()
     finally:
-        lib.osdp_set_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES, old)
+        for k, v in zip(keys, old):
+            lib.osdp_set_tuning(k, v)
 
 
 @pytest.mark.parametrize("T,h,f,k", [
@@ -209,3 +215,39 @@ def test_back_to_back_steps_reuse_buffers_safely(lib, slice_kernel):
     for o in outs:
         for n in NAMES:
             assert np.array_equal(o[n].double().cpu().numpy(), want[n]), n
+
+
+def run_gpu_ffn(lib, inp, k):
+    T, h = inp.X.shape
+    f = inp.W1.shape[1]
+    d = inp.to("cuda")
+    op = lib.SplitMlp(T, h, f, torch.bfloat16, k, axis="ffn")
+    Y = op.forward(d.X, d.W1, d.b1, d.W2, d.b2)
+    g = op.backward(d.X, d.W1, d.b1, d.W2, d.dY)
+    torch.cuda.synchronize()
+    out = {"Y": Y}
+    out.update(g)
+    return {n: out[n].to(torch.float64).cpu().numpy() for n in NAMES}
+
+
+@pytest.mark.parametrize("T,h,f,k", [
+    (256, 256, 512, 1),
+    (333, 136, 520, 3),       # ragged everywhere, ragged ffn slices
+    (1000, 320, 1032, 4),
+    (1536, 1024, 2048, 2),    # several tile rows and columns
+    (2100, 520, 1288, 5),
+    (640, 64, 4096, 16),      # many narrow ffn slices
+])
+def test_ffn_split_slice_kernel_matches_oracle_and_the_per_gemm_path_bitwise(lib, slice_kernel, T, h, f, k):
+    """The paper-literal ffn-axis split through the same kernel: A1 -> A2 (Y accumulated in fp32 by reduce-add), and
+    (A3 + A4) -> A7 (dX accumulated) | A5 | A6 with the slice's own dW / db1 parts written once."""
+    inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=39)
+    ref = O.mlp_forward_backward(**inp.as_f64())
+    got = run_gpu_ffn(lib, inp, k)
+    n_bwd = lib.osdp_last_launch_count()
+    errs = {n: rel_err(got[n], ref[n]) for n in NAMES}
+    assert all(e <= 2e-2 for e in errs.values()), errs
+    assert n_bwd == 2 + k + (1 if k > 1 else 0), "db2 (two launches) + one kernel per slice (+ accumulator -> dX)"
+    want = per_gemm(lib, lambda: run_gpu_ffn(lib, inp, k))
+    for n in NAMES:
+        assert np.array_equal(got[n], want[n]), f"{n}: slice kernel and launch-per-GEMM path differ"

@@ -300,7 +300,7 @@ def test_tuning_keys_of_header_binding_and_library_agree(lib):
     import re
     hdr = open(os.path.join(os.path.dirname(GOLDEN), "..", "include", "osdp.h")).read()
     keys = dict((n, int(v)) for n, v in re.findall(r"\b(OSDP_TUNE_[A-Z0-9_]+)\s*=\s*(\d+)", hdr))
-    assert len(keys) == 8 and sorted(keys.values()) == list(range(8))
+    assert len(keys) == 9 and sorted(keys.values()) == list(range(9))
     for name, val in keys.items():
         assert getattr(lib, name) == val, name
         cur = lib.osdp_get_tuning(val)
@@ -308,6 +308,7 @@ def test_tuning_keys_of_header_binding_and_library_agree(lib):
         lib.osdp_set_tuning(val, cur)                                  # round trip leaves the default in place
         assert lib.osdp_get_tuning(val) == cur
     assert lib.osdp_get_tuning(lib.OSDP_TUNE_SLICE_KERNEL_MAX_TILES) == 128
+    assert lib.osdp_get_tuning(lib.OSDP_TUNE_SLICE_KERNEL_FFN_MAX_TILES) == 0
     assert lib.osdp_get_tuning(len(keys)) == -1
 
 
