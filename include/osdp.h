@@ -221,12 +221,17 @@ typedef enum osdp_tune_key {
                                       If the workspace passed to the forward has room for two slice buffers (the
                                       backward's size), consecutive forward slices alternate buffers and overlap.
                                       0 = never */
-  OSDP_TUNE_SLICE_KERNEL_FFN_MAX_TILES = 8
+  OSDP_TUNE_SLICE_KERNEL_FFN_MAX_TILES = 8,
                                    /* default 0 (off).  The same path for the ffn-axis split (osdp_ffn_split_mlp_*), taken
                                       when the [tokens x f_s] GEMMs of a slice have at most this many 256 x 256 tiles.
                                       Bit-identical results; faster for many narrow slices of a long token axis (C3
                                       k = 64 +35 %, C5 layer shape k = 16 / 32 +31 / +37 %), slower on C2 and on C4 at
                                       k = 32 (-10 ... -17 %), hence opt-in */
+  OSDP_TUNE_BALANCE_N = 9          /* default 1.  The dX GEMM (A7; K-major B, plain epilogue) takes pair tiles of 240 / 224 /
+                                      208 / 192 instead of 256 columns when that makes its tile count fill the last wave
+                                      of CTA pairs and saves at least 5 % of the launch (C4 k = 4: 128 tiles = 1.73 waves
+                                      -> 148 tiles of 224 columns = 2 waves of 0.875).  Results do not change.  0 = always
+                                      256 columns */
 } osdp_tune_key;
 int osdp_set_tuning(int key, int64_t value);
 int64_t osdp_get_tuning(int key);

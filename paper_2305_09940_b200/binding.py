@@ -164,6 +164,7 @@ OSDP_TUNE_MT2_MIN_K_ACC = 5
 OSDP_TUNE_FORK_MAX_TILES = 6
 OSDP_TUNE_SLICE_KERNEL_MAX_TILES = 7
 OSDP_TUNE_SLICE_KERNEL_FFN_MAX_TILES = 8
+OSDP_TUNE_BALANCE_N = 9
 _lib.osdp_trace_read.restype = C.c_int64
 _lib.osdp_trace_read.argtypes = [C.c_int64, C.POINTER(C.c_int32), C.POINTER(C.c_float)]
 _lib.osdp_step_name.restype = C.c_char_p

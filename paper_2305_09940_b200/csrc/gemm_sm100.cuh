@@ -55,6 +55,7 @@ struct Tuning {
   std::atomic<int64_t> band_mib{0};         // 0: square-wave raster bands; > 0: band = tile rows whose A rows fit this many MiB of L2
   std::atomic<int64_t> cluster_min_tiles{0};   // > 0: multicast clusters for launches of at least this many pair tiles
   std::atomic<int64_t> fork_max_tiles{256};    // backward: A5 | A6 | A7 | column sums run concurrently when each GEMM has at most this many 256 x 256 tiles
+  std::atomic<int64_t> balance_n{1};           // dX GEMM: narrower tiles (UMMA N < 256) when that fills the last wave; 0 = always 256 columns
   std::atomic<int64_t> slice_kernel_ffn_max_tiles{0};   // the same for the ffn-axis split ([T x f_s] GEMMs); off by default: wins and losses are mixed
   std::atomic<int64_t> slice_kernel_max_tiles{128}; // token split: one persistent kernel per slice (slice_sm100.cuh) when the slice's [T_s x ffn] GEMMs have at most this many 256 x 256 tiles; 0 = never
 };
@@ -406,7 +407,7 @@ __global__ void __launch_bounds__(kThreads, 1)
 gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_constant__ CUtensorMap tmap_b,
                        const __grid_constant__ CUtensorMap tmap_out0, const __grid_constant__ CUtensorMap tmap_out1,
                        const GemmShape shape, const EpiParams ep, const int group_m, unsigned int* wave_sync,
-                       const int sync_kb) {
+                       const int sync_kb, const int bn_arg) {
   using Cfg = TileCfg<MT, EpiTraits<EPI>::kStoreBufs>;
   constexpr int kStages = Cfg::kStages, kAccStages = Cfg::kAccStages;
   constexpr uint32_t kSmemStore = Cfg::kSmemStore;
@@ -414,6 +415,12 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
   constexpr uint32_t kAStageBytes = Cfg::kAStageBytes, kStageBytes = Cfg::kStageBytes, kSmemTiles = Cfg::kSmemTiles;
   constexpr int kPairs = CM * CN;
   constexpr int kCluster = 2 * kPairs;
+  // Tile width.  256 columns, except for the dX GEMM (K-major B, plain epilogue, no multicast cluster), whose host side
+  // may ask for a narrower UMMA N (a multiple of 16) when that makes the tile count a whole number of waves
+  // (launch_gemm_bf16_cluster: 128 tiles of 512 x 256 on 74 pairs are 1.73 waves, 148 tiles of 512 x 224 exactly two).
+  constexpr bool kVarN = (B_MAJOR == MAJOR_K && EPI == EPI_PLAIN && kPairs == 1);
+  const int bn = kVarN ? bn_arg : BLOCK_N;
+  const int half_n = bn / 2;
   static_assert(CM == 1 || CM == 2, "CM");
   static_assert(CN == 1 || CN == 2, "CN");
   extern __shared__ uint8_t smem_raw[];
@@ -436,7 +443,7 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
   const uint32_t leader_crank = crank & ~1u;
   const int pi = (int)(crank >> 1) / CN, pj = (int)(crank >> 1) % CN;   // this pair's position in the cluster
   const int cluster_id = blockIdx.x / kCluster, num_clusters = gridDim.x / kCluster;
-  const int num_m = (shape.M + kPairM - 1) / kPairM, num_n = (shape.N + BLOCK_N - 1) / BLOCK_N;   // pair tiles
+  const int num_m = (shape.M + kPairM - 1) / kPairM, num_n = (shape.N + bn - 1) / bn;   // pair tiles
   const int num_cm = (num_m + CM - 1) / CM, num_cn = (num_n + CN - 1) / CN;                         // cluster tiles
   const int num_tiles = num_cm * num_cn;
   const int num_kb = (shape.K + BLOCK_K - 1) / BLOCK_K;
@@ -499,7 +506,7 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
       }
       const TileCoord tc = tile_coord(t, num_cm, num_cn, group_m);
       const int m0 = (tc.m_blk * CM + pi) * kPairM + (int)rank * kCtaM;       // this CTA's rows of A
-      const int n0 = (tc.n_blk * CN + pj) * BLOCK_N + (int)rank * HALF_N;     // this CTA's half of the B tile
+      const int n0 = (tc.n_blk * CN + pj) * bn + (int)rank * half_n;     // this CTA's half of the B tile
       for (int kb = 0; kb < num_kb; ++kb) {
         if (wave_sync != nullptr && sync_kb > 0 && kb > 0 && kb % sync_kb == 0) {   // stay in step inside the tile too
           int ok = 1;
@@ -515,7 +522,7 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
           const uint32_t fb = mapa(fb_local, leader_crank);     // the pair leader's barrier receives both CTAs' bytes
           const uint32_t sa = smem_a + stage * kAStageBytes, sb = smem_b + stage * kBStageBytes;
           const int k0 = kb * BLOCK_K;
-          if (leader) mbar_expect_tx(fb_local, 2 * kStageBytes);
+          if (leader) mbar_expect_tx(fb_local, kVarN ? 2u * (kAStageBytes + (uint32_t)half_n * (BLOCK_K * 2)) : 2 * kStageBytes);
           if constexpr (kPairs == 1) {
             if constexpr (A_MAJOR == MAJOR_K) {
               tma_load_2d(sa, &tmap_a, fb, k0, m0, pol_a);
@@ -556,7 +563,8 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
     }
   } else if (warp == 1 && leader) {
     // ================================================================== MMA issuer (each pair's leader CTA)
-    constexpr uint32_t idesc = make_idesc<A_MAJOR, B_MAJOR>();
+    const uint32_t idesc = kVarN ? ((make_idesc<A_MAJOR, B_MAJOR>() & ~(0x3Fu << 17)) | ((uint32_t)(bn >> 3) << 17))
+                                 : make_idesc<A_MAJOR, B_MAJOR>();
     constexpr uint16_t mask_cluster = (uint16_t)((1u << kCluster) - 1u);
     const uint16_t mask_pair = (uint16_t)(3u << leader_crank);
     int stage = 0;
@@ -630,8 +638,8 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
       const TileCoord tc = tile_coord(t, num_cm, num_cn, group_m);
       const int as = it % kAccStages;
       const uint32_t aphase = (it / kAccStages) & 1;
-      const int n0 = (tc.n_blk * CN + pj) * BLOCK_N;
-      const int n_end = min(n0 + BLOCK_N, shape.N);
+      const int n0 = (tc.n_blk * CN + pj) * bn;
+      const int n_end = min(n0 + bn, shape.N);
       if constexpr (kHasBias) {
 #pragma unroll
         for (int ci = 0; ci < kBiasChunks; ++ci) {
@@ -707,6 +715,24 @@ gemm_bf16_sm100_kernel(const __grid_constant__ CUtensorMap tmap_a, const __grid_
                 pipe.put(j, pack8(v));
               }
               pipe.commit(&tmap_out0, n, row0, false);
+            }
+            if constexpr (kVarN) {
+              // a tile narrower than 256 columns ends inside this warp's last 64-column chunk: the 64-column TMA box would
+              // run over into the next tile's columns, so the chunk's 16 / 32 / 48 columns go out as 16-byte stores
+              if (n + kChunk > n0 + bn && n0 + bn < shape.N) {
+                if (row_ok) {
+                  __nv_bfloat16* dst = reinterpret_cast<__nv_bfloat16*>(ep.out0) + row * ep.ldo + n;
+#pragma unroll
+                  for (int j = 0; j < 8; ++j) {
+                    if (n + 8 * j < n_end) {
+                      float v[8];
+                      load8(&acc[8 * j], bias_cur, j, v);
+                      *reinterpret_cast<uint4*>(dst + 8 * j) = pack8(v);
+                    }
+                  }
+                }
+                continue;
+              }
             }
             pipe.begin();
 #pragma unroll
@@ -858,7 +884,22 @@ inline int launch_gemm_bf16_cluster(const void* A, int64_t lda, const void* B, i
   if (A_MAJOR == MAJOR_K) rc = make_tmap(&ta, A, s.K, s.M, lda, BLOCK_K, Cfg::kCtaM / CN);
   else                    rc = make_tmap(&ta, A, s.M, s.K, lda, 64, BLOCK_K);
   if (rc != OSDP_OK) return rc;
-  if (B_MAJOR == MAJOR_K) rc = make_tmap(&tb, B, s.K, s.N, ldb, BLOCK_K, HALF_N / CM);
+  // Tile width (see kVarN in the kernel): among 256, 240, 224, 208, 192 columns the one with the least waves x width, if
+  // that saves at least 5 % of the launch's tile-time.  Results do not depend on it (one owner per output element,
+  // ascending-k accumulation).
+  int bn = BLOCK_N;
+  DeviceInfo dev;
+  rc = current_device(&dev);
+  if (rc != OSDP_OK) return rc;
+  if (B_MAJOR == MAJOR_K && EPI == EPI_PLAIN && CM * CN == 1 && tuning().balance_n.load() != 0) {
+    const int64_t pairs = dev.sms / 2, nm = (s.M + Cfg::kPairM - 1) / Cfg::kPairM;
+    auto cost = [&](int w) { return ((nm * ((s.N + w - 1) / w) + pairs - 1) / pairs) * (int64_t)w; };
+    int64_t best = cost(BLOCK_N);
+    for (int w = BLOCK_N - 16; w >= 192; w -= 16)
+      if (cost(w) < best) { best = cost(w); bn = w; }
+    if (20 * best > 19 * cost(BLOCK_N)) bn = BLOCK_N;
+  }
+  if (B_MAJOR == MAJOR_K) rc = make_tmap(&tb, B, s.K, s.N, ldb, BLOCK_K, (bn / 2) / CM);
   else                    rc = make_tmap(&tb, B, s.N, s.K, ldb, 64, BLOCK_K);
   if (rc != OSDP_OK) return rc;
   // outputs: [M x N] row-major, leading dimension ldo; one store = 32 rows x 128 bytes
@@ -886,9 +927,6 @@ inline int launch_gemm_bf16_cluster(const void* A, int64_t lda, const void* B, i
   attr[1].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 2;
-  DeviceInfo dev;
-  rc = current_device(&dev);
-  if (rc != OSDP_OK) return rc;
   // per (kernel instantiation, device): the dynamic shared-memory opt-in and the number of co-resident clusters
   static std::atomic<int> max_clusters_of[kMaxDevices];
   int max_clusters = max_clusters_of[dev.ordinal].load(std::memory_order_acquire);
@@ -906,7 +944,7 @@ inline int launch_gemm_bf16_cluster(const void* A, int64_t lda, const void* B, i
     max_clusters = n;
     max_clusters_of[dev.ordinal].store(n, std::memory_order_release);
   }
-  const int num_m = (s.M + Cfg::kPairM - 1) / Cfg::kPairM, num_n = (s.N + BLOCK_N - 1) / BLOCK_N;   // pair tiles
+  const int num_m = (s.M + Cfg::kPairM - 1) / Cfg::kPairM, num_n = (s.N + bn - 1) / bn;   // pair tiles
   const int tiles = ((num_m + CM - 1) / CM) * ((num_n + CN - 1) / CN);                      // cluster tiles
   cfg.gridDim = dim3(kCluster * (tiles < max_clusters ? tiles : max_clusters));
   // Raster band = group_m tile rows; inside a band tiles walk m fastest, then n, so one wave of P resident clusters
@@ -949,7 +987,7 @@ inline int launch_gemm_bf16_cluster(const void* A, int64_t lda, const void* B, i
   {
     LaunchTrace tr(st);
     err = cudaLaunchKernelEx(&cfg, kernel, ta, tb, to0, to1, s, ep, (int)group_m, wave_sync,
-                             sync_mode > 1 ? (int)sync_mode : 0);
+                             sync_mode > 1 ? (int)sync_mode : 0, bn);
   }
   OSDP_CUDA_TRY(err);
   OSDP_CUDA_TRY(cudaGetLastError());

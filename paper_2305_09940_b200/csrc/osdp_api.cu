@@ -485,6 +485,10 @@ int osdp_set_tuning(int key, int64_t value) {
       if (value < 0) return OSDP_ERR_ARG;
       t.slice_kernel_ffn_max_tiles = value;
       return OSDP_OK;
+    case OSDP_TUNE_BALANCE_N:
+      if (value < 0 || value > 1) return OSDP_ERR_ARG;
+      t.balance_n = value;
+      return OSDP_OK;
     default: return OSDP_ERR_ARG;
   }
 }
@@ -501,6 +505,7 @@ int64_t osdp_get_tuning(int key) {
     case OSDP_TUNE_FORK_MAX_TILES: return t.fork_max_tiles;
     case OSDP_TUNE_SLICE_KERNEL_MAX_TILES: return t.slice_kernel_max_tiles;
     case OSDP_TUNE_SLICE_KERNEL_FFN_MAX_TILES: return t.slice_kernel_ffn_max_tiles;
+    case OSDP_TUNE_BALANCE_N: return t.balance_n;
     default: return -1;
   }
 }

@@ -447,3 +447,26 @@ def test_no_out_of_bounds_writes_guard_bands(lib, dtype, T, h, f, k):
     tol = TOL[dtype]
     for n in NAMES:
         assert rel_err(got[n].double().cpu().numpy(), ref[n]) <= tol, n
+
+
+@pytest.mark.parametrize("T,h,f,k", [
+    (1100, 3840, 264, 1),     # dX: 5 x 15 = 75 tiles of 256 columns on 74 pairs -> 192-column tiles (5 x 20 = 100, two waves of 0.75)
+    (1100, 3848, 264, 2),     # the same with a ragged last column tile and ragged row tiles
+    (2048, 8192, 512, 4),     # the headline's dX tile grid per slice (512 rows, 8192 columns)
+    (700, 2440, 136, 1),      # a width whose last 64-column chunk is 16 / 48 columns wide
+])
+def test_dx_tile_width_balancing_is_bitwise_neutral(lib, per_gemm_launches, T, h, f, k):
+    """OSDP_TUNE_BALANCE_N: the dX GEMM may take 240 / 224 / 208 / 192-column tiles to fill its last wave; every output
+    element still has one owner and ascending-k accumulation, so nothing changes but the time."""
+    inp = I.mlp_inputs(T, h, f, torch.bfloat16, seed=41)
+    assert lib.osdp_get_tuning(lib.OSDP_TUNE_BALANCE_N) == 1
+    got = run_gpu(lib, inp, k, torch.bfloat16)
+    lib.osdp_set_tuning(lib.OSDP_TUNE_BALANCE_N, 0)
+    try:
+        want = run_gpu(lib, inp, k, torch.bfloat16)
+    finally:
+        lib.osdp_set_tuning(lib.OSDP_TUNE_BALANCE_N, 1)
+    for n in NAMES:
+        assert np.array_equal(got[n], want[n]), n
+    if T * h <= 1100 * 3848:
+        check(got, O.mlp_forward_backward(**inp.as_f64()), 2e-2, f"balanced dX {T}x{h}x{f}")

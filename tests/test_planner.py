@@ -300,7 +300,7 @@ def test_tuning_keys_of_header_binding_and_library_agree(lib):
     import re
     hdr = open(os.path.join(os.path.dirname(GOLDEN), "..", "include", "osdp.h")).read()
     keys = dict((n, int(v)) for n, v in re.findall(r"\b(OSDP_TUNE_[A-Z0-9_]+)\s*=\s*(\d+)", hdr))
-    assert len(keys) == 9 and sorted(keys.values()) == list(range(9))
+    assert len(keys) == 10 and sorted(keys.values()) == list(range(10))
     for name, val in keys.items():
         assert getattr(lib, name) == val, name
         cur = lib.osdp_get_tuning(val)
