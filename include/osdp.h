@@ -51,7 +51,8 @@ typedef enum osdp_status {
   OSDP_ERR_CUDA = 8,        /* CUDA runtime/driver error; see osdp_last_cuda_error() */
   OSDP_ERR_INFEASIBLE = 9,  /* planner: no plan fits the memory limit (Algorithm 1 lines 12-14) */
   OSDP_ERR_ARG = 10,        /* other invalid argument (pass, mode, n, candidate list, ...) */
-  OSDP_ERR_SEARCH_LIMIT = 11 /* planner: node budget exhausted before the search completed */
+  OSDP_ERR_SEARCH_LIMIT = 11, /* planner: node budget exhausted before the search completed */
+  OSDP_ERR_STATIC_LIMIT = 12  /* osdp_bias_grad_static: cols > OSDP_BIAS_GRAD_STATIC_MAX_COLS (the static scratch is too small) */
 } osdp_status;
 
 typedef enum osdp_dtype { OSDP_F32 = 0, OSDP_BF16 = 1 } osdp_dtype;
@@ -179,6 +180,35 @@ int osdp_split_linear_forward(const osdp_linear_desc* desc, const void* X, const
 int osdp_split_linear_backward(const osdp_linear_desc* desc, const void* X, const void* W, const void* dY,
                                void* dX, float* dW, float* db, void* workspace, size_t workspace_bytes, void* stream);
 /* (osdp_linear_op_cost is declared below, after osdp_op_cost.) */
+
+/* ---- A8 without a workspace: the bias gradient for callers that cannot allocate device memory -------------------
+ * db[c] = sum over r of dY[r, c]  ("all computation results are summed": the bias gradient of a Linear
+ * is the sum of the output gradient over the tokens; db2 of the MLP backward, db of the Linear backward), fp32, with
+ * the same fixed summation order as osdp_split_mlp_backward's db2, so the bits agree with that call.
+ *
+ * Who this is for: a caller that holds dY and db but has no device memory to lend as a workspace and may not get
+ * any - it runs where the CUDA allocator must not be entered (inside another library's callback or allocator hook,
+ * on a device whose memory is wholly owned by a pool the caller cannot draw from), or its embedder hands it nothing
+ * but the input and output pointers.  All other entry points need a caller workspace; this one needs none, and it
+ * calls no cudaMalloc / cudaFree / allocating routine itself.  The 32 x cols floats of partial sums live in a static
+ * __device__ array inside the library (2 MiB, reserved on every GPU that loads the library until the process exits),
+ * hence the limit: cols <= OSDP_BIAS_GRAD_STATIC_MAX_COLS, otherwise OSDP_ERR_STATIC_LIMIT and nothing is launched.
+ *
+ *   dY     device pointer, [rows x cols] dense row-major of `dtype` (osdp_dtype), 16-byte aligned; read only
+ *   rows   >= 1;  cols >= 1 and a multiple of 8 (bf16) / 4 (f32)
+ *   db     device pointer, [cols] fp32, 16-byte aligned; OVERWRITTEN.  Must not alias dY
+ *   stream cudaStream_t as void* (NULL = legacy default stream); two kernels are enqueued on it, nothing else
+ * The first call on each device looks up the array's device address (cudaGetSymbolAddress, under a mutex, with the
+ * calling thread's current device) and checks the compute capability; make that first call before any stream
+ * capture begins on that device.  Later calls only enqueue the two kernels.
+ * The array is SHARED by every call on a device and keeps the previous call's partial sums.  That needs no
+ * clearing (stage 1 writes every word stage 2 reads), but two calls that overlap on the GPU - different streams
+ * without an ordering between them, or several host threads on several streams - race on it and give wrong sums.
+ * Calls on one stream, or ordered by events, are safe.  Calls on different devices never share (one array per GPU).
+ * Errors: OSDP_ERR_NULL, OSDP_ERR_DTYPE, OSDP_ERR_SHAPE, OSDP_ERR_STATIC_LIMIT, OSDP_ERR_ALIGN, OSDP_ERR_ARCH,
+ * OSDP_ERR_ARG (device ordinal >= 64), OSDP_ERR_CUDA; db is untouched on every one of them but a launch failure. */
+#define OSDP_BIAS_GRAD_STATIC_MAX_COLS 16384
+int osdp_bias_grad_static(const void* dY, int64_t rows, int64_t cols, int32_t dtype, float* db, void* stream);
 
 /* Number of kernel launches the last forward/backward call of the calling thread enqueued (for bench.py's
  * gpu_launches claim). */

@@ -24,6 +24,8 @@ _lib = C.CDLL(LIB_PATH)
 OSDP_OK = 0
 OSDP_ERR_NULL, OSDP_ERR_SHAPE, OSDP_ERR_K, OSDP_ERR_DTYPE, OSDP_ERR_WORKSPACE, OSDP_ERR_ALIGN = 1, 2, 3, 4, 5, 6
 OSDP_ERR_ARCH, OSDP_ERR_CUDA, OSDP_ERR_INFEASIBLE, OSDP_ERR_ARG, OSDP_ERR_SEARCH_LIMIT = 7, 8, 9, 10, 11
+OSDP_ERR_STATIC_LIMIT = 12
+OSDP_BIAS_GRAD_STATIC_MAX_COLS = 16384
 OSDP_F32, OSDP_BF16 = 0, 1
 OSDP_FWD, OSDP_BWD = 0, 1
 OSDP_DP, OSDP_ZDP = 0, 1
@@ -37,6 +39,7 @@ EXPORTS = (
     "osdp_split_linear_workspace_bytes", "osdp_split_linear_forward", "osdp_split_linear_backward", "osdp_linear_op_cost",
     "osdp_zdp_shard_elems", "osdp_zdp_slice_layout", "osdp_zdp_schedule", "osdp_zdp_ffn_split_mlp_workspace_bytes",
     "osdp_zdp_ffn_split_mlp_forward", "osdp_zdp_ffn_split_mlp_backward", "osdp_zdp_ffn_split_mlp_op_cost",
+    "osdp_bias_grad_static",
 )
 
 
@@ -134,6 +137,8 @@ _lib.osdp_split_linear_forward.restype = C.c_int
 _lib.osdp_split_linear_forward.argtypes = [C.POINTER(osdp_linear_desc)] + [C.c_void_p] * 5 + [C.c_size_t, C.c_void_p]
 _lib.osdp_split_linear_backward.restype = C.c_int
 _lib.osdp_split_linear_backward.argtypes = [C.POINTER(osdp_linear_desc)] + [C.c_void_p] * 7 + [C.c_size_t, C.c_void_p]
+_lib.osdp_bias_grad_static.restype = C.c_int
+_lib.osdp_bias_grad_static.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p]
 _lib.osdp_linear_op_cost.restype = C.c_int
 _lib.osdp_linear_op_cost.argtypes = [C.POINTER(osdp_linear_desc), C.c_int, C.POINTER(osdp_op_cost)]
 _lib.osdp_zdp_shard_elems.restype = C.c_int
@@ -453,6 +458,37 @@ def osdp_split_linear_backward(desc, X, W, dY, dX, dW, db, workspace=None, works
                                              _ptr(workspace), int(workspace_bytes), _stream_ptr(stream))
     if check and st != OSDP_OK:
         raise OsdpError(st, "osdp_split_linear_backward")
+    return st
+
+
+def osdp_bias_grad_static(dY, db, stream=None, check=True) -> int:
+    """db = column sums of dY ([rows x cols] bf16 / fp32 -> [cols] fp32) WITHOUT a workspace: the entry point for
+    callers that cannot allocate device memory where they need the bias gradient (code running inside another
+    library's callback or allocator hook, a device whose memory belongs to a pool the caller may not draw from, a host
+    that is only handed the input and output pointers).  The partial sums go to a 2 MiB static array inside the library
+    instead, so cols <= OSDP_BIAS_GRAD_STATIC_MAX_COLS (else OSDP_ERR_STATIC_LIMIT), the first call on a device should
+    come before any stream capture (it looks the array's address up), and calls that overlap on one GPU race on that
+    array - keep them on one stream or order them.  Same bits as the db2 of osdp_split_mlp_backward.  This wrapper only
+    marshals: dY and db are dense CUDA tensors the caller already owns."""
+    where = "osdp_bias_grad_static"
+    vs, detail = OSDP_OK, ""
+    if not (isinstance(dY, torch.Tensor) and isinstance(db, torch.Tensor) and dY.is_cuda and db.is_cuda):
+        vs, detail = OSDP_ERR_ARG, "dY and db must be CUDA tensors"
+    elif dY.dim() != 2 or not dY.is_contiguous() or not db.is_contiguous():
+        vs, detail = OSDP_ERR_ARG, "dY must be a dense [rows x cols] tensor, db dense"
+    elif db.dtype != torch.float32 or db.numel() != dY.shape[1]:
+        vs, detail = OSDP_ERR_SHAPE, "db must hold cols fp32 values"
+    elif db.device != dY.device:
+        vs, detail = OSDP_ERR_ARG, f"db is on {db.device}, dY on {dY.device}"
+    if vs != OSDP_OK:
+        if check:
+            raise OsdpError(vs, where, detail)
+        return vs
+    with _on_device(dY.device):
+        st = _lib.osdp_bias_grad_static(_ptr(dY), int(dY.shape[0]), int(dY.shape[1]), _dtype_code(dY.dtype), _ptr(db),
+                                        _stream_ptr(stream))
+    if check and st != OSDP_OK:
+        raise OsdpError(st, where)
     return st
 
 

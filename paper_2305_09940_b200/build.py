@@ -15,7 +15,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libosdp_b200.so")
-SOURCES = ["osdp_api.cu", "planner.cpp"]
+SOURCES = ["osdp_api.cu", "bias_grad_static.cu", "planner.cpp"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-shared", "-Xcompiler", "-fPIC,-fvisibility=hidden", "--cudart", "static",
