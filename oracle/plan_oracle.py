@@ -182,24 +182,14 @@ def schedule_brute_force(ops, dev: Device, k_candidates, b_max: int = 1 << 20):
 # definition of operators (e.g., types and shapes)"); written from DESIGN.md "Cost model", not from the
 # library source. -------------------------------------------------------------------------------------
 def mlp_workspace_bytes(T: int, h: int, f: int, e: int, k: int, backward: bool) -> int:
-    """Bytes of caller workspace one call needs: per-slice T_s x f buffers (1 fwd: H_s; 2 bwd: Z_s/dZ_s
-    and H_s), each rounded up to 256 B, plus (bwd) the column-sum scratch of one slice."""
+    """Bytes of per-slice tensors one call keeps beside the caller's tensors - what PAPER.md:167 fixes ("the extra
+    memory required for one slice is size / slice_granularity") and SURVEY.md section 8(d) prints: one T_s x f tensor
+    forward (H_s), two backward (Z_s / dZ_s and H_s), T_s = ceil(T / k), each rounded up to 256 B.  Nothing else: any
+    scratch an implementation adds on top (partial sums of the bias gradients, synchronisation words) is ITS choice,
+    not the method's, so it is not stated here; the tests bound it instead (reading W1)."""
     Ts = ceil_div(T, k)
     buf = ceil_div(Ts * f * e, 256) * 256
-    if not backward:
-        return buf
-    return 2 * buf + mlp_reduce_scratch_bytes(Ts, h, f)
-
-
-BAND_ROWS = 32
-REDUCE_ROW_CHUNKS = 32
-
-
-def mlp_reduce_scratch_bytes(Ts: int, h: int, f: int) -> int:
-    """fp32 partial column sums: db1 keeps one partial row per BAND_ROWS-row band of the slice's
-    dZ_s (ceil(T_s / 32) x f floats, written by the A4 epilogue), db2 REDUCE_ROW_CHUNKS partial rows of dY (32 x h
-    floats); each part rounded up to 256 B."""
-    return ceil_div(ceil_div(Ts, BAND_ROWS) * f * 4, 256) * 256 + ceil_div(REDUCE_ROW_CHUNKS * h * 4, 256) * 256
+    return 2 * buf if backward else buf
 
 
 def mlp_persistent_bytes(T: int, h: int, f: int, e: int, backward: bool) -> int:
