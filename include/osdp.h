@@ -15,8 +15,11 @@
  *   - "device pointer" = CUDA device memory of the current device, owned by the caller, 16-byte aligned
  *     (workspace: 256-byte aligned).  The library never allocates, frees or synchronises device memory; it
  *     only enqueues work on `stream` (a cudaStream_t passed as void*; NULL = the legacy default stream).  Its own
- *     device state is static (module memory: wave-sync counters, 2 MiB of tile flags of the one-kernel-per-slice path;
- *     up to 16 calls of that path in flight on one device get separate flags).
+ *     device state is static module memory: 256 wave-sync counters per device (a scheduling hint with a 200 us give-up,
+ *     never a correctness dependency) and the scratch of osdp_bias_grad_static.  The tile counter and flags of the
+ *     one-kernel-per-slice path live in the caller's workspace (counted by the *_workspace_bytes queries), so a workspace
+ *     must be exclusive to ONE call in flight: calls that may overlap on the GPU - other streams, or captured graphs
+ *     replayed side by side - each need their own.  Any number of such calls may be in flight.
  *     Outputs must not alias inputs or each other.
  *   - Every call returns an osdp_status; OSDP_OK = 0.  Nothing is printed, nothing aborts.  On any error
  *     before the first launch the outputs are untouched.
@@ -78,7 +81,8 @@ const char* osdp_version(void);
  * Bytes of caller workspace one forward (OSDP_FWD) or backward (OSDP_BWD) call needs.  Pure host function.
  *   FWD: one [T_s x f] tensor (H_s);  BWD: two (Z_s, overwritten by dZ_s; H_s) + the fp32 column-sum partials:
  *   ceil(T_s / 32) x ffn floats (one row per 32-row band of dZ_s, written by the A4 epilogue: db1) and 32 x hidden
- *   floats (db2);
+ *   floats (db2); both passes, bf16: + the tile counter and flag words of the one-kernel-per-slice path,
+ *   4 k (4 + 2 t) bytes, t = the 256 x 256 tiles of a [T_s x ffn] tensor, when that is <= 128 KiB, else none;
  *   T_s = ceil(T/k); each part rounded up to 256 B.  Returns 0 on an invalid descriptor. */
 size_t osdp_split_mlp_workspace_bytes(const osdp_mlp_desc* desc, int pass);
 

@@ -120,11 +120,27 @@ inline size_t db1_scratch_bytes(int64_t slice_rows, int64_t cols) {
   return align_up((size_t)((slice_rows + kBandRows - 1) / kBandRows) * (size_t)cols * 4, 256);
 }
 inline size_t db2_scratch_bytes(int64_t h) { return align_up((size_t)kReduceRowChunks * (size_t)h * 4, 256); }
-size_t workspace_bytes(const osdp_mlp_desc* d, int pass) {
+// Tile counter and per-tile flags of the one-kernel-per-slice path (slice_sm100.cuh): kSliceFlags0 + 2 words per 256 x 256
+// tile of a slice's [rows x cols] GEMM, for each of the k slices.  They live at the END of the caller's workspace, which
+// is exclusive to one call in flight by contract, so any number of calls on any number of streams, and captured graphs
+// replayed side by side, have their own words (round 2 kept 16 static blocks handed out round-robin).  Pure host
+// arithmetic, independent of the tuning knobs: the bytes are reserved whenever the path COULD be chosen (bf16, the
+// call's words fit kSliceSyncWords = 128 KiB), else 0.
+inline int64_t tiles_256(int64_t m, int64_t n) { return ((m + 255) / 256) * ((n + 255) / 256); }
+inline int64_t slice_sync_words(int dtype, int64_t rows, int64_t cols, int64_t k) {
+  if (dtype != OSDP_BF16) return 0;
+  const int64_t per_slice = sm100::kSliceFlags0 + 2 * tiles_256(rows, cols);
+  return per_slice * k > sm100::kSliceSyncWords ? 0 : per_slice * k;
+}
+inline size_t slice_sync_bytes(const osdp_mlp_desc* d) {
+  return align_up((size_t)slice_sync_words(d->dtype, (d->tokens + d->k - 1) / d->k, d->ffn, d->k) * 4, 256);
+}
+inline size_t workspace_tensor_bytes(const osdp_mlp_desc* d, int pass) {   // everything but the sync words
   if (pass == OSDP_FWD) return slice_buf_bytes(d);
   const int64_t ts = (d->tokens + d->k - 1) / d->k;
   return 2 * slice_buf_bytes(d) + db1_scratch_bytes(ts, d->ffn) + db2_scratch_bytes(d->hidden);
 }
+size_t workspace_bytes(const osdp_mlp_desc* d, int pass) { return workspace_tensor_bytes(d, pass) + slice_sync_bytes(d); }
 
 // ---- ffn-axis split: slice s owns ffn columns [ffn_lo(s), ffn_lo(s + 1)), whole 16-byte units
 inline int64_t ffn_unit(const osdp_mlp_desc* d) { return 16 / (int64_t)elem_size(d->dtype); }
@@ -152,10 +168,16 @@ inline size_t ffn_slice_buf_bytes(const osdp_mlp_desc* d) {
 inline size_t ffn_acc_bytes(const osdp_mlp_desc* d) {   // fp32 accumulator of Y / dX across slices; not needed at k = 1
   return d->k == 1 ? 0 : align_up((size_t)d->tokens * (size_t)d->hidden * 4, 256);
 }
-size_t ffn_workspace_bytes(const osdp_mlp_desc* d, int pass) {
+inline size_t ffn_slice_sync_bytes(const osdp_mlp_desc* d) {   // slice-kernel words of the call (see slice_sync_words)
+  return align_up((size_t)slice_sync_words(d->dtype, d->tokens, ffn_slice_max(d), d->k) * 4, 256);
+}
+inline size_t ffn_workspace_tensor_bytes(const osdp_mlp_desc* d, int pass) {   // everything but the sync words
   if (pass == OSDP_FWD) return ffn_slice_buf_bytes(d) + ffn_acc_bytes(d);
   return 2 * ffn_slice_buf_bytes(d) + ffn_acc_bytes(d) + db1_scratch_bytes(d->tokens, ffn_slice_max(d)) +
          db2_scratch_bytes(d->hidden);
+}
+size_t ffn_workspace_bytes(const osdp_mlp_desc* d, int pass) {
+  return ffn_workspace_tensor_bytes(d, pass) + ffn_slice_sync_bytes(d);
 }
 
 inline bool misaligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) != 0; }
@@ -248,7 +270,6 @@ int join_into(ForkCtx* c, cudaStream_t st) {
   }
   return OSDP_OK;
 }
-inline int64_t tiles_256(int64_t m, int64_t n) { return ((m + 255) / 256) * ((n + 255) / 256); }
 
 
 // ---- one persistent kernel per slice (slice_sm100.cuh) ----------------------------------------------------------
@@ -279,6 +300,16 @@ int slice_plan(const osdp_mlp_desc* d, int pass, SlicePlan* out) {
   out->use = true;
   out->words_per_slice = (int)per_slice;
   out->words = (int)(per_slice * d->k);
+  return OSDP_OK;
+}
+
+// The call's tile counter / flag words: `bytes_before` into the caller's workspace (exclusive to this call), zeroed on
+// the call's stream before its first launch - the workspace holds whatever the caller left there.
+int slice_sync_setup(const SlicePlan& sp, void* workspace, size_t bytes_before, int launches, cudaStream_t st,
+                     unsigned int** sync, unsigned int* epoch0) {
+  *sync = reinterpret_cast<unsigned int*>((char*)workspace + bytes_before);
+  OSDP_CUDA_TRY(cudaMemsetAsync(*sync, 0, (size_t)sp.words * 4, st));
+  *epoch0 = sm100::slice_epochs(launches);
   return OSDP_OK;
 }
 
@@ -575,12 +606,12 @@ int osdp_mlp_op_cost(const osdp_mlp_desc* desc, int pass, osdp_op_cost* out) {
     c.model_bytes = (2 * h * f + f + h) * e;                          // W1, W2, b1, b2
     c.act_bytes = 2 * T * h * e;                                      // X, Y
     c.extra_transient = T * f * e;                                    // H
-    c.extra_fixed = 0;
+    c.extra_fixed = slice_sync_bytes(desc);                           // tile counter / flags of the one-kernel-per-slice path
   } else {
     c.model_bytes = (2 * h * f + f + h) * e + (2 * h * f + f + h) * 4;   // W, b; fp32 dW, db
     c.act_bytes = 3 * T * h * e;                                      // X, dY, dX
     c.extra_transient = 2 * T * f * e + (T * f * 4) / kBandRows;      // Z/dZ, H and the db1 band partials: all per slice
-    c.extra_fixed = db2_scratch_bytes(h);
+    c.extra_fixed = db2_scratch_bytes(h) + slice_sync_bytes(desc);
   }
   *out = c;
   return OSDP_OK;
@@ -606,7 +637,12 @@ int osdp_split_mlp_forward(const osdp_mlp_desc* desc, const void* X, const void*
   OSDP_TRY(slice_plan(desc, OSDP_FWD, &sp));
   unsigned int* sync = nullptr;
   unsigned int epoch0 = 0;
-  if (sp.use) OSDP_TRY(sm100::slice_sync_acquire(sp.words, desc->k, &sync, &epoch0));
+  // A workspace with room for two H_s buffers (the backward's is: callers that train pass the same workspace to both
+  // passes) lets consecutive slices alternate buffers, and slice s then need not wait for slice s - 1 at all (see
+  // late_wait in slice_sm100.cuh); with the forward's own minimum the slices run one after another as the paper says.
+  const bool two_bufs = workspace_bytes_given >= 2 * slice_buf_bytes(desc) + slice_sync_bytes(desc);
+  if (sp.use)
+    OSDP_TRY(slice_sync_setup(sp, workspace, (two_bufs ? 2 : 1) * slice_buf_bytes(desc), desc->k, st, &sync, &epoch0));
   bool first_launch = true;
 
   for (int s = 0; s < desc->k; ++s) {
@@ -616,10 +652,6 @@ int osdp_split_mlp_forward(const osdp_mlp_desc* desc, const void* X, const void*
     const char* Xs = (const char*)X + (size_t)lo * h * e;
     char* Ys = (char*)Y + (size_t)lo * h * e;
     if (sp.use) {   // A1 -> A2 in one launch: an A2 tile starts when its 256 rows of H_s are complete
-      // A workspace with room for two H_s buffers (the backward's is: callers that train pass the same workspace to both
-      // passes) lets consecutive slices alternate buffers, and slice s then need not wait for slice s - 1 at all (see
-      // late_wait in slice_sm100.cuh); with the forward's own minimum the slices run one after another as the paper says.
-      const bool two_bufs = workspace_bytes_given >= 2 * slice_buf_bytes(desc);
       void* Hb = two_bufs ? (char*)workspace + (size_t)(s & 1) * slice_buf_bytes(desc) : Hs;
       trace_set_step(21);
       sm100::SliceGemm g[2] = {};
@@ -679,7 +711,7 @@ int osdp_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const void
   OSDP_TRY(slice_plan(desc, OSDP_BWD, &sp));
   unsigned int* sync = nullptr;
   unsigned int epoch0 = 0;
-  if (sp.use) OSDP_TRY(sm100::slice_sync_acquire(sp.words, desc->k, &sync, &epoch0));
+  if (sp.use) OSDP_TRY(slice_sync_setup(sp, workspace, workspace_tensor_bytes(desc, OSDP_BWD), desc->k, st, &sync, &epoch0));
   if (fork && !sp.use) OSDP_TRY(fork_ctx(&fc));
 
   int first = 1;
@@ -761,12 +793,12 @@ int osdp_ffn_split_mlp_op_cost(const osdp_mlp_desc* desc, int pass, osdp_op_cost
     c.model_bytes = (2 * h * f + f + h) * e;
     c.act_bytes = 2 * T * h * e;
     c.extra_transient = T * f * e;
-    c.extra_fixed = acc;
+    c.extra_fixed = acc + ffn_slice_sync_bytes(desc);
   } else {
     c.model_bytes = (2 * h * f + f + h) * e + (2 * h * f + f + h) * 4;
     c.act_bytes = 3 * T * h * e;
     c.extra_transient = 2 * T * f * e + db1_scratch_bytes(T, f);     // db1 band partials of one slice: ceil(T / 32) x f / k floats
-    c.extra_fixed = acc + db2_scratch_bytes(h);
+    c.extra_fixed = acc + db2_scratch_bytes(h) + ffn_slice_sync_bytes(desc);
   }
   *out = c;
   return OSDP_OK;
@@ -792,7 +824,7 @@ int osdp_ffn_split_mlp_forward(const osdp_mlp_desc* desc, const void* X, const v
   OSDP_TRY(ffn_slice_plan(desc, ffn_slice_max(desc), &sp));
   unsigned int* sync = nullptr;
   unsigned int epoch0 = 0;
-  if (sp.use) OSDP_TRY(sm100::slice_sync_acquire(sp.words, k, &sync, &epoch0));
+  if (sp.use) OSDP_TRY(slice_sync_setup(sp, workspace, ffn_workspace_tensor_bytes(desc, OSDP_FWD), k, st, &sync, &epoch0));
 
   for (int s = 0; s < k; ++s) {
     const int64_t lo = ffn_lo(desc, s), hi = ffn_lo(desc, s + 1);
@@ -839,7 +871,7 @@ int osdp_ffn_split_mlp_backward(const osdp_mlp_desc* desc, const void* X, const 
   OSDP_TRY(ffn_slice_plan(desc, ffn_slice_max(desc), &sp));
   unsigned int* sync = nullptr;
   unsigned int epoch0 = 0;
-  if (sp.use) OSDP_TRY(sm100::slice_sync_acquire(sp.words, k, &sync, &epoch0));
+  if (sp.use) OSDP_TRY(slice_sync_setup(sp, workspace, ffn_workspace_tensor_bytes(desc, OSDP_BWD), k, st, &sync, &epoch0));
 
   for (int s = 0; s < k; ++s) {
     const int64_t lo = ffn_lo(desc, s), hi = ffn_lo(desc, s + 1);

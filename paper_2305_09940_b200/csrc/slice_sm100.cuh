@@ -23,10 +23,11 @@
 //     and fences the async proxy, the 8 epilogue warps of the CTA meet at a named barrier, and one thread stores the
 //     launch's EPOCH (release, gpu scope) into the tile's flag of this CTA; a tile is complete when both CTAs' flags
 //     hold the epoch.  Consumers poll with ld.acquire.gpu, then fence.proxy.async before their TMA loads.  Flags and
-//     the tile counter live in a static __device__ array that the host never touches: the last pair to draw a
-//     sentinel puts the tile counter back to zero and the last CTA to leave clears the flags (so a captured launch can
-//     be replayed); the per-launch epoch only guards against flags an earlier launch could not clear.  Every launch in
-//     flight owns its own part of the array (osdp_api.cu).
+//     the tile counter live at the end of the CALLER'S WORKSPACE (osdp_api.cu: slice_sync_words), which one call in
+//     flight owns exclusively, so concurrent calls and concurrently replayed graphs never share them; the call zeroes
+//     its words on its stream before the first launch (a memset node when captured).  The last pair to draw a
+//     sentinel still puts the tile counter back to zero and the last CTA to leave clears the flags; the per-launch
+//     epoch keeps the slices of one call apart.
 //   * Forward slices pipeline: with room for two H_s buffers in the caller's workspace, slice s does not wait for
 //     slice s - 1 (late_wait below), so its A1 tiles run beside the few long A2 tiles of the slice before.
 //   * db1: the A6 tiles of the first tile row also add up the 32-row band sums that the fused epilogue left in the
@@ -46,8 +47,7 @@ namespace sm100 {
 
 constexpr int kSliceMaxPhases = 5;
 constexpr int kSliceQueue = 4;              // tile indices a pair may hold ahead of its epilogue
-constexpr int kSliceCallSlots = 16;         // calls in flight on one device that get separate counters
-constexpr int kSliceSyncWords = 32768;      // words per call: k x (kSliceFlags0 + 2 x publishing tiles of a slice) must fit
+constexpr int kSliceSyncWords = 32768;      // most words a call may take from the workspace: k x (kSliceFlags0 + 2 x publishing tiles of a slice)
 constexpr unsigned int kPublishersPerTile = 2 * kNumEpiWarps;   // arrivals that hand a TMEM stage back
 constexpr int kSliceFlags0 = 4;             // first flag word of a launch's part of the array
 // A3 and A4 of the backward in one tile (they have the same output tile grid): accumulator 0 = X_s W1, accumulator 1 =
@@ -95,8 +95,6 @@ struct SliceParams {
 struct SliceMaps {
   CUtensorMap m[kSliceMaxPhases][4];   // A, B, out0, out1 of each phase
 };
-
-__device__ unsigned int g_slice_sync[kSliceCallSlots * kSliceSyncWords];
 
 // ------------------------------------------------------------------------------------------------ PTX wrappers
 __device__ __forceinline__ uint32_t mbar_try_wait_cluster(uint32_t bar, uint32_t parity) {
@@ -716,25 +714,10 @@ struct SliceDb1 {
 
 inline int slice_tiles(const GemmShape& s, int bn) { return ((s.M + UMMA_M - 1) / UMMA_M) * ((s.N + bn - 1) / bn); }
 
-// This device's counter / flag block for one call, and the epoch of the call's first launch (launch s uses epoch + s).
-inline int slice_sync_acquire(int words, int launches, unsigned int** out, unsigned int* epoch0) {
-  if (words > kSliceSyncWords) return OSDP_ERR_ARG;
-  DeviceInfo dev;
-  int rc = current_device(&dev);
-  if (rc != OSDP_OK) return rc;
-  static std::atomic<unsigned int*> base_of[kMaxDevices];
-  static std::atomic<unsigned int> seq{0};
-  unsigned int* base = base_of[dev.ordinal].load(std::memory_order_acquire);
-  if (!base) {
-    OSDP_CUDA_TRY(cudaGetSymbolAddress(reinterpret_cast<void**>(&base), g_slice_sync));
-    base_of[dev.ordinal].store(base, std::memory_order_release);
-  }
-  *out = base + (size_t)(seq.fetch_add(1) % kSliceCallSlots) * kSliceSyncWords;
-  // consecutive epochs for the call's launches, never 0 and never wrapping inside a call
+// Epoch of a call's first launch (launch s uses epoch + s): consecutive, never 0, never wrapping inside a call.
+inline unsigned int slice_epochs(int launches) {
   static std::atomic<uint64_t> epoch_seq{0};
-  const unsigned int e = (unsigned int)(epoch_seq.fetch_add((uint64_t)launches) % 0xF0000000ull) + 1u;
-  *epoch0 = e;
-  return OSDP_OK;
+  return (unsigned int)(epoch_seq.fetch_add((uint64_t)launches) % 0xF0000000ull) + 1u;
 }
 
 inline int launch_mlp_slice(const SliceGemm* g, int n, unsigned int* sync, unsigned int epoch, const SliceDb1* db1,

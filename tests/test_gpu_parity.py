@@ -316,8 +316,10 @@ def test_ffn_split_error_codes_and_workspace(lib):
     desc = lib.make_desc(T, h, f, torch.bfloat16, 4)
     fwd, bwd = (lib.osdp_ffn_split_mlp_workspace_bytes(desc, p) for p in (lib.OSDP_FWD, lib.OSDP_BWD))
     # bwd: two slice buffers, the fp32 dX accumulator, db1 band partials (T / 32 rows x 32 columns) and db2 partials (32 x h)
-    assert fwd == T * 32 * 2 + T * h * 4 and bwd == 2 * T * 32 * 2 + T * h * 4 + (T // 32) * 32 * 4 + 32 * h * 4
-    assert lib.osdp_ffn_split_mlp_workspace_bytes(lib.make_desc(T, h, f, torch.bfloat16, 1), lib.OSDP_FWD) == T * f * 2
+    # (+ at most 128 KiB of tile counter / flag words of the one-kernel-per-slice path and their 256 B padding)
+    assert 0 <= fwd - (T * 32 * 2 + T * h * 4) <= 129 << 10
+    assert 0 <= bwd - (2 * T * 32 * 2 + T * h * 4 + (T // 32) * 32 * 4 + 32 * h * 4) <= 129 << 10
+    assert 0 <= lib.osdp_ffn_split_mlp_workspace_bytes(lib.make_desc(T, h, f, torch.bfloat16, 1), lib.OSDP_FWD) - T * f * 2 <= 129 << 10
     assert lib.osdp_ffn_split_mlp_workspace_bytes(lib.make_desc(T, h, f, torch.bfloat16, f // 8 + 1), lib.OSDP_FWD) == 0
     ws = torch.empty(bwd, dtype=torch.uint8, device="cuda")
     Y = torch.full_like(inp.X, 3.0)

@@ -1,5 +1,6 @@
 """The one-kernel-per-slice path of the token split (csrc/slice_sm100.cuh, OSDP_TUNE_SLICE_KERNEL_MAX_TILES): parity
-with the fp64 oracle, bit-identity with the launch-per-GEMM path, concurrency on two streams, CUDA-graph capture.
+with the fp64 oracle, bit-identity with the launch-per-GEMM path, concurrency on 2 and on 24 streams, CUDA-graph capture, two graphs replayed
+side by side.
 GPU only (-m gpu)."""
 import numpy as np
 import pytest
@@ -140,6 +141,77 @@ def test_slice_kernel_step_can_be_captured_in_a_cuda_graph(lib, slice_kernel):
     got = dict(Y=Y, **g)
     for n in NAMES:
         assert np.array_equal(got[n].double().cpu().numpy(), want[n]), n
+
+
+def test_24_calls_in_flight_on_24_streams_each_with_its_own_workspace(lib):
+    """The tile counter and flags of a call sit in ITS workspace (round 2: 16 static blocks handed out round-robin, so a
+    17th call in flight shared a live call's tile counter).  24 operators, 24 streams, three rounds without a host
+    synchronisation in between: every call gives the bits of the same call made alone."""
+    T, h, f, k, n = 1024, 256, 1024, 4, 24
+    inps = [I.mlp_inputs(T, h, f, torch.bfloat16, seed=s) for s in (50, 51, 52)]
+    want = [run_gpu(lib, inp, k) for inp in inps]
+    assert lib.osdp_last_launch_count() == 2 + k                     # the backward ran as one kernel per slice
+    devs = [inp.to("cuda") for inp in inps]
+    ops = [lib.SplitMlp(T, h, f, torch.bfloat16, k) for _ in range(n)]
+    streams = [torch.cuda.Stream() for _ in range(n)]
+    torch.cuda.synchronize()
+    outs = [None] * n
+    for _ in range(3):
+        for i, (op, st) in enumerate(zip(ops, streams)):
+            d = devs[i % 3]
+            with torch.cuda.stream(st):
+                Y = op.forward(d.X, d.W1, d.b1, d.W2, d.b2, stream=st)
+                g = op.backward(d.X, d.W1, d.b1, d.W2, d.dY, stream=st)
+            outs[i] = dict(Y=Y, **g)
+    torch.cuda.synchronize()
+    for i, o in enumerate(outs):
+        for name in NAMES:
+            assert np.array_equal(o[name].double().cpu().numpy(), want[i % 3][name]), (i, name)
+
+
+def test_two_captured_graphs_replayed_side_by_side_with_eager_calls(lib):
+    """Two captured steps (each operator with its own workspace, so its own counter and flags are what the graph holds)
+    replayed at the same time on two streams while a third stream makes eager calls: all three give the serial bits."""
+    T, h, f, k = 1000, 320, 1032, 4
+    inps = [I.mlp_inputs(T, h, f, torch.bfloat16, seed=s) for s in (53, 54, 55)]
+    want = [run_gpu(lib, inp, k) for inp in inps]
+    devs = [inp.to("cuda") for inp in inps]
+    ops = [lib.SplitMlp(T, h, f, torch.bfloat16, k) for _ in inps]
+    streams = [torch.cuda.Stream() for _ in inps]
+    outs = [dict(Y=torch.empty_like(d.X), dX=torch.empty_like(d.X), dW1=torch.empty(h, f, device="cuda"),
+                 db1=torch.empty(f, device="cuda"), dW2=torch.empty(f, h, device="cuda"), db2=torch.empty(h, device="cuda"))
+            for d in devs]
+
+    def step(i):
+        d, o, s = devs[i], outs[i], streams[i]
+        ops[i].forward(d.X, d.W1, d.b1, d.W2, d.b2, Y=o["Y"], stream=s)
+        ops[i].backward(d.X, d.W1, d.b1, d.W2, d.dY, out={n: o[n] for n in NAMES if n != "Y"}, stream=s)
+
+    graphs = []
+    for i in (0, 1):
+        s = streams[i]
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            step(i)                                                   # warm-up outside the capture
+            s.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=s):
+                step(i)
+        graphs.append(graph)
+    for o in outs:
+        for t in o.values():
+            t.fill_(7.0)
+    torch.cuda.synchronize()
+    for _ in range(6):
+        for i in (0, 1):
+            with torch.cuda.stream(streams[i]):
+                graphs[i].replay()
+        with torch.cuda.stream(streams[2]):
+            step(2)
+    torch.cuda.synchronize()
+    for i, o in enumerate(outs):
+        for name in NAMES:
+            assert np.array_equal(o[name].double().cpu().numpy(), want[i][name]), (i, name)
 
 
 def test_default_threshold_takes_small_slices_only(lib):
