@@ -213,12 +213,18 @@ int osdp_zdp_ffn_split_mlp_op_cost(const osdp_zdp_desc* desc, int pass, osdp_op_
   c.S = (double)(params * e);
   c.model_bytes = params * e + (pass == OSDP_BWD ? params * 4 : 0);       // sharded: osdp_cost_eval divides by N in ZDP mode
   c.act_bytes = (pass == OSDP_FWD ? 2 : 3) * T * h * e;
-  // sliceable: two gathered parameter slices, in the backward also two fp32 gradient staging slices, and
-  // the slice activations, all proportional to the slice width
-  const uint64_t slice_params = 2 * h * f + f;
-  c.extra_transient = 2 * slice_params * e + (pass == OSDP_BWD ? 2 * slice_params * 4 + db1_scratch_bytes(T, f) : 0) +
-                      (pass == OSDP_FWD ? 1 : 2) * T * f * e;
-  c.extra_fixed = align_up((size_t)T * h * 4, 256) + (pass == OSDP_BWD ? db2_scratch_bytes(h) + h * 4 : h * e);
+  // sliceable: two gathered parameter slices, in the backward also two fp32 gradient staging slices, the
+  // db1 band partials and the slice activations - all proportional to the slice width, stated per ffn column
+  const uint64_t per_col = 2 * (2 * h + 1) * e + (pass == OSDP_BWD ? 2 * (2 * h + 1) * 4 + ((T + kBandRows - 1) / kBandRows) * 4 : 0) +
+                           (pass == OSDP_FWD ? 1 : 2) * T * e;
+  c.extra_transient = per_col * f;
+  // fixed: the fp32 accumulator of Y / dX (charged at k = 1 too, where the call needs none), the b2 / db2 pieces, and
+  // what makes the estimate an UPPER bound of osdp_zdp_ffn_split_mlp_workspace_bytes for every (N, k): a slice is whole
+  // groups of N x 16 bytes of columns, so the widest slice has up to one group more than f / k, and each of the at
+  // most 24 parts of the workspace is padded to 256 B (the planner's M_limit check must not pass a plan that does not fit)
+  const uint64_t group_cols = (uint64_t)g.N * (uint64_t)g.unit;
+  c.extra_fixed = align_up((size_t)T * h * 4, 256) + (pass == OSDP_BWD ? db2_scratch_bytes(h) + h * 4 : h * e) +
+                  group_cols * per_col + 24 * 256;
   *out = c;
   return OSDP_OK;
 }
