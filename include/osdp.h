@@ -55,7 +55,9 @@ typedef enum osdp_status {
   OSDP_ERR_INFEASIBLE = 9,  /* planner: no plan fits the memory limit (Algorithm 1 lines 12-14) */
   OSDP_ERR_ARG = 10,        /* other invalid argument (pass, mode, n, candidate list, ...) */
   OSDP_ERR_SEARCH_LIMIT = 11, /* planner: node budget exhausted before the search completed */
-  OSDP_ERR_STATIC_LIMIT = 12  /* osdp_bias_grad_static: cols > OSDP_BIAS_GRAD_STATIC_MAX_COLS (the static scratch is too small) */
+  OSDP_ERR_STATIC_LIMIT = 12, /* osdp_bias_grad_static: cols > OSDP_BIAS_GRAD_STATIC_MAX_COLS (the static scratch is too small) */
+  OSDP_ERR_COMM = 13          /* osdp_zdp_*: a caller-supplied collective returned non-zero.  Work enqueued before it stays
+                                 enqueued, comm_stream is joined back into compute_stream, the outputs are UNDEFINED */
 } osdp_status;
 
 typedef enum osdp_dtype { OSDP_F32 = 0, OSDP_BF16 = 1 } osdp_dtype;
@@ -404,8 +406,11 @@ int osdp_plan_batch(const osdp_op_cost* ops, int32_t n, const osdp_device* dev, 
  * and the bytes one rank contributes (slice = k: the b2 / db2 vector).  osdp_zdp_ffn_split_mlp_op_cost: cost-model
  * factors of the ZDP execution: model_bytes = the WHOLE operator's model states (osdp_cost_eval divides them by N in
  * ZDP mode), extra_transient = two gathered slices at k = 1 (sliceable: / k), extra_fixed / act_bytes as the ffn split.
- * Status on one B200: the N = 1 path is parity-tested on the GPU; N > 1 is covered by a world_size-2 CPU run of the
- * same schedule and layout (tests/test_zdp.py); no multi-GPU timing exists. */
+ * Status on one B200: N = 1 is parity-tested on the GPU; N = 2 and 3 run the same executor as host threads of one
+ * process on one GPU over an in-process loopback osdp_comm (tests/test_gpu_zdp.py), and a world_size-2 CPU run covers
+ * the schedule and layout (tests/test_zdp.py); no multi-GPU timing exists.
+ * A collective that returns non-zero ends the call with OSDP_ERR_COMM: comm_stream is still joined back into
+ * compute_stream, the outputs are undefined. */
 typedef struct osdp_zdp_desc {
   osdp_mlp_desc mlp;   /* tokens = THIS rank's token batch; k = number of ffn slices */
   int32_t world;       /* N >= 1 */

@@ -25,6 +25,7 @@ OSDP_OK = 0
 OSDP_ERR_NULL, OSDP_ERR_SHAPE, OSDP_ERR_K, OSDP_ERR_DTYPE, OSDP_ERR_WORKSPACE, OSDP_ERR_ALIGN = 1, 2, 3, 4, 5, 6
 OSDP_ERR_ARCH, OSDP_ERR_CUDA, OSDP_ERR_INFEASIBLE, OSDP_ERR_ARG, OSDP_ERR_SEARCH_LIMIT = 7, 8, 9, 10, 11
 OSDP_ERR_STATIC_LIMIT = 12
+OSDP_ERR_COMM = 13
 OSDP_BIAS_GRAD_STATIC_MAX_COLS = 16384
 OSDP_F32, OSDP_BF16 = 0, 1
 OSDP_FWD, OSDP_BWD = 0, 1
@@ -654,28 +655,78 @@ class TorchDistComm:
             return 1
 
 
+def _validate_zdp(desc, spec, workspace):
+    """Marshalling checks for the ZDP calls, as _validate does for the others: dense CUDA tensors of the dtype and element
+    count the descriptor implies, all on one device (returned, so the call runs with it current).  Raw integer addresses
+    are taken on trust.  Returns (device, status, detail)."""
+    T, h = desc.mlp.tokens, desc.mlp.hidden
+    st = _TORCH_DTYPE.get(desc.mlp.dtype)
+    try:
+        shard = osdp_zdp_shard_elems(desc)
+    except OsdpError as e:
+        return None, e.status, "invalid ZDP descriptor"
+    numel = {"param_shard": shard, "grad_shard": shard, "X": T * h, "Y": T * h, "dY": T * h, "dX": T * h}
+    dev = None
+    for name, t in spec:
+        if t is None or isinstance(t, int):
+            continue
+        if not isinstance(t, torch.Tensor) or not t.is_cuda:
+            return None, OSDP_ERR_ARG, f"{name} is not a CUDA tensor"
+        if not t.is_contiguous():
+            return None, OSDP_ERR_ARG, f"{name} is not dense row-major"
+        want = torch.float32 if name == "grad_shard" else st
+        if t.dtype != want:
+            return None, OSDP_ERR_DTYPE, f"{name} has dtype {t.dtype}, descriptor needs {want}"
+        if t.numel() != numel[name]:
+            return None, OSDP_ERR_SHAPE, f"{name} has {t.numel()} elements, descriptor needs {numel[name]}"
+        if dev is not None and t.device != dev:
+            return None, OSDP_ERR_ARG, f"{name} is on {t.device}, other tensors on {dev}"
+        dev = t.device
+    if isinstance(workspace, torch.Tensor):
+        if not workspace.is_cuda or not workspace.is_contiguous():
+            return None, OSDP_ERR_WORKSPACE, "workspace must be a dense CUDA tensor"
+        if dev is not None and workspace.device != dev:
+            return None, OSDP_ERR_ARG, f"workspace is on {workspace.device}, tensors on {dev}"
+    return dev, OSDP_OK, ""
+
+
 def osdp_zdp_ffn_split_mlp_forward(desc, param_shard, X, Y, workspace, comm=None, compute_stream=None, comm_stream=None,
                                    check=True):
-    cs = _stream_ptr(compute_stream)
-    ms = cs if comm_stream is None else _stream_ptr(comm_stream)
-    st = _lib.osdp_zdp_ffn_split_mlp_forward(C.byref(desc), _ptr(param_shard), _ptr(X), _ptr(Y), _ptr(workspace),
-                                             workspace.numel() * workspace.element_size(),
-                                             C.byref(comm.struct) if comm is not None else None, cs, ms)
+    where = "osdp_zdp_ffn_split_mlp_forward"
+    dev, vs, detail = _validate_zdp(desc, (("param_shard", param_shard), ("X", X), ("Y", Y)), workspace)
+    if vs != OSDP_OK:
+        if check:
+            raise OsdpError(vs, where, detail)
+        return vs
+    with _on_device(dev):
+        cs = _stream_ptr(compute_stream)
+        ms = cs if comm_stream is None else _stream_ptr(comm_stream)
+        st = _lib.osdp_zdp_ffn_split_mlp_forward(C.byref(desc), _ptr(param_shard), _ptr(X), _ptr(Y), _ptr(workspace),
+                                                 0 if workspace is None else workspace.numel() * workspace.element_size(),
+                                                 C.byref(comm.struct) if comm is not None else None, cs, ms)
     if check and st != OSDP_OK:
-        raise OsdpError(st, "osdp_zdp_ffn_split_mlp_forward", str(getattr(comm, "error", "") or ""))
+        raise OsdpError(st, where, str(getattr(comm, "error", "") or ""))
     return st
 
 
 def osdp_zdp_ffn_split_mlp_backward(desc, param_shard, X, dY, dX, grad_shard, workspace, comm=None, compute_stream=None,
                                     comm_stream=None, check=True):
-    cs = _stream_ptr(compute_stream)
-    ms = cs if comm_stream is None else _stream_ptr(comm_stream)
-    st = _lib.osdp_zdp_ffn_split_mlp_backward(C.byref(desc), _ptr(param_shard), _ptr(X), _ptr(dY), _ptr(dX),
-                                              _ptr(grad_shard), _ptr(workspace),
-                                              workspace.numel() * workspace.element_size(),
-                                              C.byref(comm.struct) if comm is not None else None, cs, ms)
+    where = "osdp_zdp_ffn_split_mlp_backward"
+    dev, vs, detail = _validate_zdp(desc, (("param_shard", param_shard), ("X", X), ("dY", dY), ("dX", dX),
+                                           ("grad_shard", grad_shard)), workspace)
+    if vs != OSDP_OK:
+        if check:
+            raise OsdpError(vs, where, detail)
+        return vs
+    with _on_device(dev):
+        cs = _stream_ptr(compute_stream)
+        ms = cs if comm_stream is None else _stream_ptr(comm_stream)
+        st = _lib.osdp_zdp_ffn_split_mlp_backward(C.byref(desc), _ptr(param_shard), _ptr(X), _ptr(dY), _ptr(dX),
+                                                  _ptr(grad_shard), _ptr(workspace),
+                                                  0 if workspace is None else workspace.numel() * workspace.element_size(),
+                                                  C.byref(comm.struct) if comm is not None else None, cs, ms)
     if check and st != OSDP_OK:
-        raise OsdpError(st, "osdp_zdp_ffn_split_mlp_backward", str(getattr(comm, "error", "") or ""))
+        raise OsdpError(st, where, str(getattr(comm, "error", "") or ""))
     return st
 
 

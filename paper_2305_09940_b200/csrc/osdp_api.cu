@@ -469,6 +469,7 @@ const char* osdp_status_string(int status) {
     case OSDP_ERR_INFEASIBLE: return "no plan fits the memory limit";
     case OSDP_ERR_ARG: return "invalid argument";
     case OSDP_ERR_SEARCH_LIMIT: return "planner node budget exhausted";
+    case OSDP_ERR_COMM: return "a caller-supplied collective failed";
     case OSDP_ERR_STATIC_LIMIT: return "more columns than the static scratch of osdp_bias_grad_static holds";
     default: return "unknown status";
   }

@@ -141,7 +141,7 @@ int zdp_all_gather(const osdp_comm* comm, const void* send, void* recv, size_t b
     OSDP_CUDA_TRY(cudaMemcpyAsync(recv, send, bytes, cudaMemcpyDeviceToDevice, st));
     return OSDP_OK;
   }
-  return comm->all_gather(comm->ctx, send, recv, bytes, (void*)st) == 0 ? OSDP_OK : OSDP_ERR_ARG;
+  return comm->all_gather(comm->ctx, send, recv, bytes, (void*)st) == 0 ? OSDP_OK : OSDP_ERR_COMM;
 }
 int zdp_reduce_scatter(const osdp_comm* comm, const float* send, float* recv, size_t floats, cudaStream_t st) {
   if (floats == 0) return OSDP_OK;
@@ -149,8 +149,19 @@ int zdp_reduce_scatter(const osdp_comm* comm, const float* send, float* recv, si
     OSDP_CUDA_TRY(cudaMemcpyAsync(recv, send, floats * 4, cudaMemcpyDeviceToDevice, st));
     return OSDP_OK;
   }
-  return comm->reduce_scatter_f32(comm->ctx, send, recv, floats, (void*)st) == 0 ? OSDP_OK : OSDP_ERR_ARG;
+  return comm->reduce_scatter_f32(comm->ctx, send, recv, floats, (void*)st) == 0 ? OSDP_OK : OSDP_ERR_COMM;
 }
+
+// An error return after comm_stream was forked from compute_stream (a failed collective, a failed launch) still joins
+// it back, so a stream capture the call was part of is not left with an unjoined stream.  Disarmed on the normal path.
+struct ZdpJoin {
+  cudaStream_t cs, ms;
+  cudaEvent_t tail;
+  bool armed;
+  ~ZdpJoin() {
+    if (armed && cudaEventRecord(tail, ms) == cudaSuccess) cudaStreamWaitEvent(cs, tail, 0);
+  }
+};
 
 int zdp_check_call(const osdp_zdp_desc* desc, ZdpGeom* g, int pass, const void* workspace, size_t given, const osdp_comm* comm) {
   OSDP_TRY(zdp_geom(desc, g));
@@ -249,6 +260,7 @@ int osdp_zdp_ffn_split_mlp_forward(const osdp_zdp_desc* desc, const void* param_
     OSDP_CUDA_TRY(cudaEventRecord(ev->entry, cs));
     OSDP_CUDA_TRY(cudaStreamWaitEvent(ms, ev->entry, 0));
   }
+  ZdpJoin join{cs, ms, ev->tail, two};
   std::vector<osdp_zdp_step> steps;
   zdp_steps(g, OSDP_FWD, &steps);
   int used[2] = {0, 0};   // how many computes have used each gathered buffer so far
@@ -288,6 +300,7 @@ int osdp_zdp_ffn_split_mlp_forward(const osdp_zdp_desc* desc, const void* param_
     OSDP_TRY(sm100::current_device(&dev));
     OSDP_TRY(launch_acc_to_out(g.dt, (const float*)(ws + w.acc), ws + w.b2g, Y, g.T, (int)g.h, dev.sms, cs));
   }
+  join.armed = false;
   return OSDP_OK;   // every gather was waited for by a compute step: comm_stream has joined compute_stream
 }
 
@@ -312,6 +325,7 @@ int osdp_zdp_ffn_split_mlp_backward(const osdp_zdp_desc* desc, const void* param
     OSDP_CUDA_TRY(cudaEventRecord(ev->entry, cs));
     OSDP_CUDA_TRY(cudaStreamWaitEvent(ms, ev->entry, 0));
   }
+  ZdpJoin join{cs, ms, ev->tail, two};
   std::vector<osdp_zdp_step> steps;
   zdp_steps(g, OSDP_BWD, &steps);
   int used[2] = {0, 0}, scattered[2] = {0, 0};
@@ -369,6 +383,7 @@ int osdp_zdp_ffn_split_mlp_backward(const osdp_zdp_desc* desc, const void* param
     OSDP_CUDA_TRY(cudaEventRecord(ev->tail, ms));
     OSDP_CUDA_TRY(cudaStreamWaitEvent(cs, ev->tail, 0));
   }
+  join.armed = false;
   return OSDP_OK;
 }
 
