@@ -407,7 +407,7 @@ int osdp_plan_batch(const osdp_op_cost* ops, int32_t n, const osdp_device* dev, 
  * factors of the ZDP execution: model_bytes = the WHOLE operator's model states (osdp_cost_eval divides them by N in
  * ZDP mode), extra_transient = two gathered slices at k = 1 (sliceable: / k), extra_fixed / act_bytes as the ffn split.
  * Status on one B200: N = 1 is parity-tested on the GPU; N = 2 and 3 run the same executor as host threads of one
- * process on one GPU over an in-process loopback osdp_comm (tests/test_gpu_zdp.py), and a world_size-2 CPU run covers
+ * process on one GPU over an in-process loopback communicator (tests/test_gpu_zdp.py), and a world_size-2 CPU run covers
  * the schedule and layout (tests/test_zdp.py); no multi-GPU timing exists.
  * A collective that returns non-zero ends the call with OSDP_ERR_COMM: comm_stream is still joined back into
  * compute_stream, the outputs are undefined. */
