@@ -583,3 +583,25 @@ def test_descriptor_validation(lib):
     assert lib.osdp_split_mlp_workspace_bytes(lib.make_desc(8, 8, 8, 7, 1), 0) == 0        # dtype
     assert lib.osdp_split_mlp_workspace_bytes(lib.make_desc(8, 8, 8, 1, 1), 2) == 0        # pass
     assert lib.osdp_split_mlp_workspace_bytes(lib.make_desc(8, 4, 4, 0, 8), 1) > 0
+
+
+def test_bias_grad_static_rejects_bad_arguments_before_touching_the_device(lib):
+    """osdp_bias_grad_static (the entry point for callers that cannot allocate device memory) checks pointers, dtype,
+    shape, its column limit and alignment on the host, in that order, before any CUDA call - so these cases run here
+    without a GPU.  The addresses below are never dereferenced."""
+    import ctypes
+    f = lib._lib.osdp_bias_grad_static
+    a, b = 0x7000000000, 0x7000100000                      # 16-byte aligned stand-ins for device pointers
+    big = lib.OSDP_BIAS_GRAD_STATIC_MAX_COLS
+    assert f(None, 8, 8, lib.OSDP_BF16, b, None) == lib.OSDP_ERR_NULL
+    assert f(a, 8, 8, lib.OSDP_BF16, None, None) == lib.OSDP_ERR_NULL
+    assert f(a, 8, 8, 7, b, None) == lib.OSDP_ERR_DTYPE
+    assert f(a, 0, 8, lib.OSDP_BF16, b, None) == lib.OSDP_ERR_SHAPE
+    assert f(a, 8, 12, lib.OSDP_BF16, b, None) == lib.OSDP_ERR_SHAPE          # 12 bf16 columns are not whole 16-byte units
+    assert f(a, 8, 12, lib.OSDP_F32, b + 4, None) == lib.OSDP_ERR_ALIGN        # ... 12 fp32 columns are
+    assert f(a, 8, big + 8, lib.OSDP_BF16, b, None) == lib.OSDP_ERR_STATIC_LIMIT
+    assert f(a, 1 << 40, big + 4, lib.OSDP_F32, b, None) == lib.OSDP_ERR_STATIC_LIMIT
+    assert f(a + 2, 8, big, lib.OSDP_BF16, b, None) == lib.OSDP_ERR_ALIGN
+    hdr = open(os.path.join(os.path.dirname(GOLDEN), "..", "include", "osdp.h")).read()
+    assert f"#define OSDP_BIAS_GRAD_STATIC_MAX_COLS {big}" in hdr
+    assert "static scratch" in lib.osdp_status_string(lib.OSDP_ERR_STATIC_LIMIT)
